@@ -1,0 +1,140 @@
+/* pct.h -- C-ABI of libpct.so: the single-B200 hot path of proton-CT reconstruction (arxiv 1802.01070).
+ *
+ *   PAPER.md:7   "calculating the individual proton's most likely path [3] ... large and sparse linear system
+ *                 Ax = b ... A is a m x n matrix containing the path data, b is the m x 1 WEPLs vector, and x is
+ *                 the n x 1 relative stopping powers (RSP) vector"                      -> pct_generate_mlp
+ *   PAPER.md:98  "block iterative technique Diagonally-Relaxed Orthogonal Projections (DROP [11])", "the block
+ *                 size is the number of protons to be processed in parallel"            -> pct_solve
+ *   PAPER.md:7   b = A x                                                               -> pct_forward_project
+ * The paper prints no formula; the exact operations are the readings R1..R20 in DESIGN.md.
+ *
+ * Conventions
+ *   - Plain C, no C++/torch types.  Every pointer is documented as HOST or DEVICE memory; buffers are owned by
+ *     the caller and never retained or freed by the library, except the opaque pct_ctx / pct_paths objects,
+ *     which the library owns until pct_destroy / pct_paths_free.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Work is enqueued on it; device
+ *     results are valid once the caller has synchronised the stream.  pct_generate_mlp and the *_host calls
+ *     synchronise the stream themselves (they need sizes on the host).
+ *   - Return value: PCT_OK (0) or a negative PCT_E_* code; never throws, never aborts.  pct_last_error(ctx)
+ *     gives a human-readable message for the last failure on that context.
+ *   - Frames (R1): grid frame (x,y,z), z = rotation axis, voxel (ix,iy,iz) = origin + [i, i+1]*h per axis,
+ *     linear index j = ix + nx*(iy + ny*iz).  Gantry frame (u,t,v): x = u cos(phi) - t sin(phi),
+ *     y = u sin(phi) + t cos(phi), z = v.  Slopes are dt/du, dv/du (R2).
+ *   - Rejected histories (flags & PCT_REJECT_MASK) have N_i = 0 and contribute nothing anywhere.
+ */
+#ifndef PCT_H
+#define PCT_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PCT_OK 0
+#define PCT_E_INVALID_ARG (-1)
+#define PCT_E_OOM (-2)
+#define PCT_E_CUDA (-3)
+#define PCT_E_CAPACITY (-4)
+
+/* per-history flag bits */
+#define PCT_REJ_MISS 0x01      /* entry or exit ray misses the grid box / the hull (R4)            */
+#define PCT_REJ_ORDER 0x02     /* hull exit not behind hull entry (u2 <= u0)                       */
+#define PCT_REJ_DEPTH 0x04     /* u2 - u0 > poly_max_depth_mm (R6)                                 */
+#define PCT_REJ_LEFT_GRID 0x08 /* the walk stepped outside the grid (R10)                          */
+#define PCT_TIE 0x10           /* some stepping decision was closer than tie_eps_mm (R9); logged   */
+#define PCT_END_MISMATCH 0x20  /* walk did not end in the exit hull voxel (R10); list kept         */
+#define PCT_REJ_CAPACITY 0x40  /* more than max_visits path entries                                */
+#define PCT_REJ_NONFINITE 0x80 /* NaN/Inf tracker record                                           */
+#define PCT_REJECT_MASK (PCT_REJ_MISS | PCT_REJ_ORDER | PCT_REJ_DEPTH | PCT_REJ_LEFT_GRID | PCT_REJ_CAPACITY | PCT_REJ_NONFINITE)
+
+typedef struct pct_ctx pct_ctx;     /* opaque: geometry, MLP constants, device scratch            */
+typedef struct pct_paths pct_paths; /* opaque: device-resident encoded rows of A (R9-R12)         */
+
+typedef struct {
+    int32_t nx, ny, nz;
+    double h_mm;
+    double origin_mm[3]; /* lower corner of voxel (0,0,0), grid frame */
+} pct_geometry;
+
+typedef struct {
+    double poly[6];           /* 1/(beta^2 p^2) = sum a_i w^i, w = depth from hull entry in mm (R6)   */
+    double poly_max_depth_mm; /* validity range of poly; deeper histories are rejected                 */
+    double X0_mm;             /* radiation length (361 mm, water)                                      */
+    double log_coeff;         /* 0.038; 0 => pure Fermi-Eyges                                          */
+    double step_frac;         /* nominal MLP step = step_frac * h (R8; 0.5)                            */
+    double tie_eps_mm;        /* 1e-9 (R9)                                                             */
+    int32_t max_visits;       /* capacity of one encoded row, <= 8192                                  */
+} pct_mlp_params;
+
+typedef struct {
+    int64_t m;
+    /* m doubles each: gantry angle [rad]; entry tracker position/slope; exit tracker position/slope.
+     * DEVICE pointers for pct_generate_mlp, HOST pointers for pct_reconstruct_host. */
+    const double *phi, *t_in, *v_in, *dt_in, *dv_in, *t_out, *v_out, *dt_out, *dv_out;
+    double u_in_mm, u_out_mm; /* tracker plane depths in the gantry frame */
+} pct_protons;
+
+typedef struct {
+    int64_t m, total_visits, n_rejected, n_ties, code_bytes, header_bytes;
+} pct_paths_stats;
+
+typedef struct {
+    int64_t m, total_visits, n_rejected, n_ties;
+    double ms_h2d, ms_mlp, ms_solve, ms_d2h; /* CUDA-event times of the four phases */
+} pct_recon_stats;
+
+/* Create a context on CUDA device `device`.  Validates geometry/params.  HOST pointers. */
+int pct_create(const pct_geometry* geom, const pct_mlp_params* params, int device, pct_ctx** out);
+void pct_destroy(pct_ctx* ctx);
+const char* pct_last_error(const pct_ctx* ctx);
+
+/* A1-A3: tracker records -> most likely path -> visit list, stored as start voxel + 3-bit face
+ * step codes.  protons: struct on HOST holding DEVICE arrays.  hull: DEVICE uint8[n], NULL = every voxel is
+ * hull.  *out receives a new pct_paths.  Synchronises `stream`. */
+int pct_generate_mlp(pct_ctx* ctx, const pct_protons* protons, const uint8_t* hull, void* stream, pct_paths** out);
+int pct_paths_info(const pct_paths* paths, pct_paths_stats* out /* HOST */);
+void pct_paths_free(pct_paths* paths);
+
+/* Parity/debug: expand rows [i0,i1) to explicit voxel lists.  All outputs DEVICE; any of voxels/ell/flags may
+ * be NULL.  row_ptr: int64[i1-i0+1]; voxels: int32[cap] (PCT_E_CAPACITY if cap is too small; row_ptr is
+ * still valid then); ell: float32[i1-i0] mean chord l_i; flags: uint8[i1-i0].  Synchronises `stream`. */
+int pct_paths_decode(pct_ctx* ctx, const pct_paths* paths, int64_t i0, int64_t i1, int64_t* row_ptr, int32_t* voxels,
+                     int64_t cap, float* ell, uint8_t* flags, void* stream);
+
+/* A9 (R19): b_out[i] = l_i * sum over visits of x[j].  x: DEVICE float32[n]; b_out: DEVICE float32[m]. */
+int pct_forward_project(pct_ctx* ctx, const pct_paths* paths, const float* x, float* b_out, void* stream);
+
+/* A4 (R20): counts[j] = visits of voxel j by histories [i0,i1).  counts: DEVICE uint32[n] (overwritten). */
+int pct_column_counts(pct_ctx* ctx, const pct_paths* paths, int64_t i0, int64_t i1, uint32_t* counts, void* stream);
+
+/* A5-A8 (R13-R18): `iters` sweeps of block-iterative DROP with unit weights,
+ *   x <- x + lambda * diag(1/max(1,s_j^t)) * sum_{i in block t} [(b_i - <a_i,x>)/||a_i||^2] a_i,
+ * blocks = consecutive ranges of block_size histories.  b: DEVICE float32[m]; x0, x_out: DEVICE float32[n],
+ * x_out may alias x0.  FP32 arithmetic, FP32 atomics (result unique up to summation order). */
+int pct_solve(pct_ctx* ctx, const pct_paths* paths, const float* b, const float* x0, int iters, int64_t block_size,
+              float lambda, float* x_out, void* stream);
+
+/* The whole hot path on HOST buffers (bench e2e): H2D of the tracker arrays, hull and b; pct_generate_mlp;
+ * pct_solve; D2H of x.  protons: HOST struct with HOST arrays; hull_host: uint8[n] or NULL; b_host: float32[m];
+ * x0_host: float32[n] or NULL (= all ones); x_out_host: float32[n]; stats may be NULL.  Blocking. */
+int pct_reconstruct_host(pct_ctx* ctx, const pct_protons* protons, const uint8_t* hull_host, const float* b_host,
+                         const float* x0_host, int iters, int64_t block_size, float lambda, float* x_out_host,
+                         pct_recon_stats* stats, void* stream);
+
+/* Number of kernel launches issued by this context so far (bench.py reports it as gpu_launches). */
+int64_t pct_launch_count(const pct_ctx* ctx);
+
+/* Per-kernel timing for the roofline report.  pct_profile_enable(ctx, 1) makes the launchers bracket every launch
+ * of the three hot kernels with CUDA events on the launching stream; pct_profile_read synchronises the device,
+ * ADDS the elapsed times since the last read to out (HOST) and clears the event list.  kind: 0 = MLP + walk (K1),
+ * 1 = block project + scatter (K2), 2 = voxel update (K3). */
+typedef struct {
+    double ms[3];
+    int64_t launches[3];
+} pct_profile;
+int pct_profile_enable(pct_ctx* ctx, int on);
+int pct_profile_read(pct_ctx* ctx, pct_profile* out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

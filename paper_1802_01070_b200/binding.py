@@ -1,0 +1,256 @@
+"""Thin ctypes binding of libpct.so (include/pct.h).  Argument marshalling only: every step of the hot path
+runs in the CUDA kernels behind the C-ABI.  torch is used for device memory and streams, nothing else.
+
+There is NO CPU fallback: if libpct.so is missing or CUDA is unavailable the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Dict, Optional
+
+import torch
+
+from . import build as _build
+
+OK, E_INVALID_ARG, E_OOM, E_CUDA, E_CAPACITY = 0, -1, -2, -3, -4
+REJ_MISS, REJ_ORDER, REJ_DEPTH, REJ_LEFT_GRID, TIE, END_MISMATCH, REJ_CAPACITY, REJ_NONFINITE = (
+    0x01, 0x02, 0x04, 0x08, 0x10, 0x20, 0x40, 0x80)
+REJECT_MASK = REJ_MISS | REJ_ORDER | REJ_DEPTH | REJ_LEFT_GRID | REJ_CAPACITY | REJ_NONFINITE
+
+EXPORTS = ("pct_create", "pct_destroy", "pct_last_error", "pct_generate_mlp", "pct_paths_info", "pct_paths_free",
+           "pct_paths_decode", "pct_forward_project", "pct_column_counts", "pct_solve", "pct_reconstruct_host",
+           "pct_launch_count", "pct_profile_enable", "pct_profile_read")
+
+
+class Geometry(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32), ("h_mm", C.c_double),
+                ("origin_mm", C.c_double * 3)]
+
+
+class MlpParams(C.Structure):
+    _fields_ = [("poly", C.c_double * 6), ("poly_max_depth_mm", C.c_double), ("X0_mm", C.c_double),
+                ("log_coeff", C.c_double), ("step_frac", C.c_double), ("tie_eps_mm", C.c_double),
+                ("max_visits", C.c_int32)]
+
+
+class Protons(C.Structure):
+    _fields_ = [("m", C.c_int64)] + [(k, C.c_void_p) for k in (
+        "phi", "t_in", "v_in", "dt_in", "dv_in", "t_out", "v_out", "dt_out", "dv_out")] + [
+        ("u_in_mm", C.c_double), ("u_out_mm", C.c_double)]
+
+
+class PathsStats(C.Structure):
+    _fields_ = [(k, C.c_int64) for k in ("m", "total_visits", "n_rejected", "n_ties", "code_bytes", "header_bytes")]
+
+
+class ReconStats(C.Structure):
+    _fields_ = [(k, C.c_int64) for k in ("m", "total_visits", "n_rejected", "n_ties")] + [
+        (k, C.c_double) for k in ("ms_h2d", "ms_mlp", "ms_solve", "ms_d2h")]
+
+
+class Profile(C.Structure):
+    _fields_ = [("ms", C.c_double * 3), ("launches", C.c_int64 * 3)]
+
+
+PROTON_KEYS = ("phi", "t_in", "v_in", "dt_in", "dv_in", "t_out", "v_out", "dt_out", "dv_out")
+_lib = None
+
+
+class PctError(RuntimeError):
+    pass
+
+
+def load_library(path: Optional[str] = None):
+    """dlopen libpct.so and declare the prototypes.  Needs no GPU (used by the CPU-side export test)."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    path = path or _build.LIB
+    if not os.path.exists(path):
+        raise PctError(f"{path} is missing: run `python -m paper_1802_01070_b200.build` (no CPU fallback exists)")
+    L = C.CDLL(path)
+    vp, i64 = C.c_void_p, C.c_int64
+    L.pct_create.argtypes = [C.POINTER(Geometry), C.POINTER(MlpParams), C.c_int, C.POINTER(vp)]
+    L.pct_destroy.argtypes = [vp]
+    L.pct_destroy.restype = None
+    L.pct_last_error.argtypes = [vp]
+    L.pct_last_error.restype = C.c_char_p
+    L.pct_generate_mlp.argtypes = [vp, C.POINTER(Protons), vp, vp, C.POINTER(vp)]
+    L.pct_paths_info.argtypes = [vp, C.POINTER(PathsStats)]
+    L.pct_paths_free.argtypes = [vp]
+    L.pct_paths_free.restype = None
+    L.pct_paths_decode.argtypes = [vp, vp, i64, i64, vp, vp, i64, vp, vp, vp]
+    L.pct_forward_project.argtypes = [vp, vp, vp, vp, vp]
+    L.pct_column_counts.argtypes = [vp, vp, i64, i64, vp, vp]
+    L.pct_solve.argtypes = [vp, vp, vp, vp, C.c_int, i64, C.c_float, vp, vp]
+    L.pct_reconstruct_host.argtypes = [vp, C.POINTER(Protons), vp, vp, vp, C.c_int, i64, C.c_float, vp,
+                                       C.POINTER(ReconStats), vp]
+    L.pct_launch_count.argtypes = [vp]
+    L.pct_launch_count.restype = i64
+    L.pct_profile_enable.argtypes = [vp, C.c_int]
+    L.pct_profile_read.argtypes = [vp, C.POINTER(Profile)]
+    if path == _build.LIB:
+        _lib = L
+    return L
+
+
+def _stream_ptr(device) -> int:
+    return torch.cuda.current_stream(device).cuda_stream
+
+
+def _dev_ptr(t: Optional[torch.Tensor], dtype, numel=None, device=None):
+    if t is None:
+        return None
+    if not t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+        raise PctError(f"expected a contiguous CUDA tensor of {dtype}")
+    if device is not None and t.device != device:
+        raise PctError("tensor on the wrong device")
+    if numel is not None and t.numel() != numel:
+        raise PctError(f"expected {numel} elements, got {t.numel()}")
+    return t.data_ptr()
+
+
+class Paths:
+    """Handle of the device-resident encoded rows (pct_paths)."""
+
+    def __init__(self, ctx: "Context", handle: int):
+        self.ctx, self._h = ctx, handle
+        st = PathsStats()
+        ctx._check(ctx._L.pct_paths_info(handle, C.byref(st)))
+        self.m, self.total_visits, self.n_rejected, self.n_ties = st.m, st.total_visits, st.n_rejected, st.n_ties
+        self.code_bytes, self.header_bytes = st.code_bytes, st.header_bytes
+
+    def free(self):
+        if self._h:
+            self.ctx._L.pct_paths_free(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+
+class Context:
+    """pct_ctx: geometry + MLP constants + device scratch on one CUDA device."""
+
+    def __init__(self, geometry: dict, params: dict, device: int = 0):
+        if not torch.cuda.is_available():
+            raise PctError("CUDA is not available: the pCT hot path only runs on the GPU (no CPU fallback)")
+        self._L = load_library()
+        self.device = torch.device("cuda", device)
+        torch.cuda.init()
+        with torch.cuda.device(self.device):
+            torch.cuda.current_stream()          # make sure the primary context exists
+        g = Geometry(int(geometry["nx"]), int(geometry["ny"]), int(geometry["nz"]), float(geometry["h_mm"]),
+                     (C.c_double * 3)(*[float(v) for v in geometry["origin_mm"]]))
+        p = MlpParams((C.c_double * 6)(*[float(a) for a in params["poly"]]), float(params["poly_max_depth_mm"]),
+                      float(params["X0_mm"]), float(params["log_coeff"]), float(params["step_frac"]),
+                      float(params["tie_eps_mm"]), int(params["max_visits"]))
+        self.n = g.nx * g.ny * g.nz
+        h = C.c_void_p()
+        rc = self._L.pct_create(C.byref(g), C.byref(p), device, C.byref(h))
+        if rc != OK:
+            raise PctError(f"pct_create failed with code {rc}")
+        self._h = h.value
+
+    # -- plumbing ------------------------------------------------------------------------------------------
+    def _check(self, rc: int):
+        if rc != OK:
+            msg = self._L.pct_last_error(self._h)
+            raise PctError(f"libpct error {rc}: {msg.decode() if msg else ''}")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.pct_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def launch_count(self) -> int:
+        return int(self._L.pct_launch_count(self._h))
+
+    def profile_enable(self, on: bool):
+        self._check(self._L.pct_profile_enable(self._h, 1 if on else 0))
+
+    def profile_read(self) -> dict:
+        """{kind: (ms, launches)} for kind in mlp / project_scatter / update since the last read."""
+        pr = Profile()
+        self._check(self._L.pct_profile_read(self._h, C.byref(pr)))
+        return {k: (pr.ms[i], pr.launches[i]) for i, k in enumerate(("mlp", "project_scatter", "update"))}
+
+    # -- the C-ABI calls, same names --------------------------------------------------------------------------
+    def generate_mlp(self, protons: Dict[str, torch.Tensor], u_in_mm: float, u_out_mm: float,
+                     hull: Optional[torch.Tensor] = None) -> Paths:
+        m = int(protons["phi"].numel())
+        ptrs = [_dev_ptr(protons[k], torch.float64, m, self.device) for k in PROTON_KEYS]
+        pr = Protons(m, *ptrs, float(u_in_mm), float(u_out_mm))
+        out = C.c_void_p()
+        self._check(self._L.pct_generate_mlp(self._h, C.byref(pr), _dev_ptr(hull, torch.uint8, self.n, self.device),
+                                             _stream_ptr(self.device), C.byref(out)))
+        return Paths(self, out.value)
+
+    def paths_decode(self, paths: Paths, i0: int = 0, i1: Optional[int] = None):
+        """-> row_ptr int64[k+1], voxels int32[P], ell float32[k], flags uint8[k] (CUDA tensors)."""
+        i1 = paths.m if i1 is None else i1
+        k = i1 - i0
+        row_ptr = torch.empty(k + 1, dtype=torch.int64, device=self.device)
+        ell = torch.empty(k, dtype=torch.float32, device=self.device)
+        flags = torch.empty(k, dtype=torch.uint8, device=self.device)
+        st = _stream_ptr(self.device)
+        self._check(self._L.pct_paths_decode(self._h, paths._h, i0, i1, row_ptr.data_ptr(), None, 0, ell.data_ptr(),
+                                             flags.data_ptr(), st))
+        total = int(row_ptr[-1].item())
+        vox = torch.empty(max(total, 1), dtype=torch.int32, device=self.device)
+        self._check(self._L.pct_paths_decode(self._h, paths._h, i0, i1, row_ptr.data_ptr(), vox.data_ptr(), total, None,
+                                             None, st))
+        return row_ptr, vox[:total], ell, flags
+
+    def forward_project(self, paths: Paths, x: torch.Tensor, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+        b = out if out is not None else torch.empty(paths.m, dtype=torch.float32, device=self.device)
+        self._check(self._L.pct_forward_project(self._h, paths._h, _dev_ptr(x, torch.float32, self.n, self.device),
+                                                _dev_ptr(b, torch.float32, paths.m, self.device),
+                                                _stream_ptr(self.device)))
+        return b
+
+    def column_counts(self, paths: Paths, i0: int, i1: int) -> torch.Tensor:
+        c = torch.empty(self.n, dtype=torch.int32, device=self.device)      # uint32 payload
+        self._check(self._L.pct_column_counts(self._h, paths._h, i0, i1, c.data_ptr(), _stream_ptr(self.device)))
+        return c
+
+    def solve(self, paths: Paths, b: torch.Tensor, x0: torch.Tensor, iters: int, block_size: int, lam: float,
+              out: Optional[torch.Tensor] = None) -> torch.Tensor:
+        x = out if out is not None else torch.empty(self.n, dtype=torch.float32, device=self.device)
+        self._check(self._L.pct_solve(self._h, paths._h, _dev_ptr(b, torch.float32, paths.m, self.device),
+                                      _dev_ptr(x0, torch.float32, self.n, self.device), int(iters), int(block_size),
+                                      float(lam), _dev_ptr(x, torch.float32, self.n, self.device),
+                                      _stream_ptr(self.device)))
+        return x
+
+    def reconstruct_host(self, protons: Dict[str, torch.Tensor], u_in_mm: float, u_out_mm: float,
+                         hull: Optional[torch.Tensor], b: torch.Tensor, x0: Optional[torch.Tensor], iters: int,
+                         block_size: int, lam: float, x_out: torch.Tensor) -> dict:
+        """Whole hot path on HOST (ideally pinned) tensors; returns the phase times and counts."""
+        m = int(protons["phi"].numel())
+        for k in PROTON_KEYS:
+            t = protons[k]
+            if t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous() or t.numel() != m:
+                raise PctError("reconstruct_host expects contiguous float64 HOST tensors")
+        for t, dt, ne in ((hull, torch.uint8, self.n), (b, torch.float32, m), (x0, torch.float32, self.n),
+                          (x_out, torch.float32, self.n)):
+            if t is not None and (t.is_cuda or t.dtype != dt or not t.is_contiguous() or t.numel() != ne):
+                raise PctError("reconstruct_host: bad host tensor")
+        pr = Protons(m, *[protons[k].data_ptr() for k in PROTON_KEYS], float(u_in_mm), float(u_out_mm))
+        st = ReconStats()
+        self._check(self._L.pct_reconstruct_host(self._h, C.byref(pr), hull.data_ptr() if hull is not None else None,
+                                                 b.data_ptr(), x0.data_ptr() if x0 is not None else None, int(iters),
+                                                 int(block_size), float(lam), x_out.data_ptr(), C.byref(st),
+                                                 _stream_ptr(self.device)))
+        return {k: getattr(st, k) for k, _ in ReconStats._fields_}

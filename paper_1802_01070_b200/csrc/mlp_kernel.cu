@@ -1,0 +1,437 @@
+// mlp_kernel.cu -- K1: tracker record -> hull entry/exit (A1) -> most likely path (A2) -> voxel walk + 3-bit
+// step codes (A3).  PAPER.md:7 ("calculating the individual proton's most likely path [3]" gives the rows of A),
+// PAPER.md:26 ("each proton as an individual thread").  FP64 throughout; readings R1-R12 of DESIGN.md.
+//
+// One thread per history.  The kernel is bound by the FP64 pipe (a few hundred flop per MLP sample, K ~ 2*depth
+// samples) and by divergence in the walk, not by memory: 72 B in, ~60-170 B out per history.
+// Codes go to a staging buffer laid out [chunk][history-in-batch] (so that a warp's k-th chunks are contiguous)
+// and are compacted to their final 16-byte-aligned position once the batch's sizes are known.
+#include "pct_internal.cuh"
+
+namespace pct {
+
+__device__ __forceinline__ double face_coord(const DevCfg& g, int a, int i) { return fma((double)i, g.h, g.lo[a]); }
+
+struct Step { int axis, dir; double s; bool tie; };
+
+// R9 closed-voxel lazy stepping.  0: B inside closed box(c), 1: stepped, 2: stepped out of the grid.
+__device__ __forceinline__ int lazy_step(const DevCfg& g, const double (&A)[3], const double (&B)[3], double seg_len,
+                                         int (&c)[3], Step& st) {
+    double s[3];
+    int dir[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double f_lo = face_coord(g, a, c[a]), f_hi = face_coord(g, a, c[a] + 1);
+        dir[a] = 0; s[a] = 0.0;
+        if (B[a] > f_hi) { dir[a] = 1; s[a] = (f_hi - A[a]) / (B[a] - A[a]); }
+        else if (B[a] < f_lo) { dir[a] = -1; s[a] = (f_lo - A[a]) / (B[a] - A[a]); }
+    }
+    int best = -1;
+    double sb = 0.0;
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+        if (dir[a] != 0 && (best < 0 || s[a] < sb)) { best = a; sb = s[a]; }
+    if (best < 0) return 0;
+    bool tie = false;
+    int db = 0;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        if (a != best && dir[a] != 0 && (s[a] - sb) * seg_len < g.tie_eps) tie = true;
+        if (a == best) { c[a] += dir[a]; db = dir[a]; }
+    }
+    st.axis = best; st.dir = db; st.s = sb; st.tie = tie;
+    const bool in = c[0] >= 0 && c[0] < g.nx && c[1] >= 0 && c[1] < g.ny && c[2] >= 0 && c[2] < g.nz;
+    return in ? 1 : 2;
+}
+
+struct Hit { bool ok, tie; int c[3]; double P[3]; };
+
+// A1 / R3-R4: slab-clip the ray {T + s d, s >= 0} to the grid box, then walk the chord to the first hull voxel.
+__device__ __noinline__ void find_hull(const DevCfg& g, const uint8_t* __restrict__ hull, const double (&T)[3],
+                                       const double (&d)[3], Hit& hit) {
+    hit.ok = false; hit.tie = false;
+    double s_min = 0.0, s_max = INFINITY, near_s[3];
+    int enter_axis = -1;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        near_s[a] = -INFINITY;
+        if (d[a] != 0.0) {
+            const double s1 = (g.lo[a] - T[a]) / d[a], s2 = (g.hi[a] - T[a]) / d[a];
+            near_s[a] = fmin(s1, s2);
+            if (near_s[a] > s_min) { s_min = near_s[a]; enter_axis = a; }
+            s_max = fmin(s_max, fmax(s1, s2));
+        } else if (T[a] < g.lo[a] || T[a] > g.hi[a]) return;
+    }
+    if (!(s_min < s_max)) return;
+    const double d_len = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+    double A[3], B[3];
+    int c[3];
+    const int nn[3] = {g.nx, g.ny, g.nz};
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        A[a] = T[a] + s_min * d[a];
+        B[a] = T[a] + s_max * d[a];
+        if (a == enter_axis) {
+            A[a] = d[a] > 0 ? g.lo[a] : g.hi[a];
+            c[a] = d[a] > 0 ? 0 : nn[a] - 1;
+        } else {
+            if (enter_axis >= 0 && (s_min - near_s[a]) * d_len < g.tie_eps) hit.tie = true;
+            const int i = (int)floor((A[a] - g.lo[a]) / g.h);
+            c[a] = min(max(i, 0), nn[a] - 1);
+        }
+    }
+    const double dx = B[0] - A[0], dy = B[1] - A[1], dz = B[2] - A[2];
+    const double seg_len = sqrt(dx * dx + dy * dy + dz * dz);
+    Step last; last.axis = -1; last.dir = 0; last.s = 0.0; last.tie = false;
+    if (hull != nullptr) {
+        while (hull[c[0] + g.nx * (c[1] + g.ny * c[2])] == 0) {
+            Step st;
+            if (lazy_step(g, A, B, seg_len, c, st) != 1) return;
+            if (st.tie) hit.tie = true;
+            last = st;
+        }
+    }
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        hit.c[a] = c[a];
+        double p = last.axis < 0 ? A[a] : A[a] + last.s * (B[a] - A[a]);
+        if (a == last.axis) p = last.dir > 0 ? face_coord(g, a, c[a]) : face_coord(g, a, c[a] + 1);
+        hit.P[a] = p;
+    }
+    hit.ok = true;
+}
+
+__device__ __forceinline__ double horner6(const double (&c)[6], double x) {
+    double r = c[5];
+#pragma unroll
+    for (int i = 4; i >= 0; --i) r = fma(r, x, c[i]);
+    return r;
+}
+
+// 16-byte chunk writer: 42 codes, field k at bits 3(k%21) of word k/21; unused fields stay 7 (pad).
+struct CodeWriter {
+    unsigned long long w0, w1;
+    int nc, chunk;
+    ulonglong2* stage;       // stage[chunk * stride + p]
+    size_t stride;
+    __device__ __forceinline__ void init(ulonglong2* s, size_t str) { w0 = w1 = ~0ull; nc = 0; chunk = 0; stage = s; stride = str; }
+    __device__ __forceinline__ void flush() {
+        stage[(size_t)chunk * stride] = make_ulonglong2(w0, w1);
+        w0 = w1 = ~0ull; nc = 0; ++chunk;
+    }
+    __device__ __forceinline__ void push(int code) {
+        const unsigned long long x = (unsigned long long)(7 ^ code);
+        if (nc < CODES_PER_WORD) w0 ^= x << (3 * nc); else w1 ^= x << (3 * (nc - CODES_PER_WORD));
+        if (++nc == CODES_PER_CHUNK) flush();
+    }
+    __device__ __forceinline__ int finish() { if (nc > 0) flush(); return chunk; }
+};
+
+__global__ void __launch_bounds__(128)
+k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const uint8_t* __restrict__ hull, int64_t i_base,
+           int count, int stage_stride, ulonglong2* __restrict__ stage, uint32_t* __restrict__ nchunks, uint32_t* __restrict__ Nout,
+           int32_t* __restrict__ start_out, float* __restrict__ ell_out, uint8_t* __restrict__ flags_out,
+           GenStats* __restrict__ stats) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool active = p < count;
+    unsigned flags = 0;
+    unsigned N = 0;
+    int n_chunks = 0;
+    if (active) {
+        const int64_t i = i_base + p;
+        const double phi = pr.phi[i], t_in = pr.t_in[i], v_in = pr.v_in[i], dt_in = pr.dt_in[i], dv_in = pr.dv_in[i];
+        const double t_out = pr.t_out[i], v_out = pr.v_out[i], dt_out = pr.dt_out[i], dv_out = pr.dv_out[i];
+        int32_t start_v = -1;
+        float ell = 0.f;
+        do {
+            if (!(isfinite(phi) && isfinite(t_in) && isfinite(v_in) && isfinite(dt_in) && isfinite(dv_in) &&
+                  isfinite(t_out) && isfinite(v_out) && isfinite(dt_out) && isfinite(dv_out))) {
+                flags = PCT_REJ_NONFINITE; break;
+            }
+            double sph, cph;
+            sincos(phi, &sph, &cph);
+            // R4: entry ray, reversed exit ray (grid frame, R1)
+            Hit h_in, h_out;
+            {
+                const double T[3] = {g.u_in * cph - t_in * sph, g.u_in * sph + t_in * cph, v_in};
+                const double d[3] = {cph - dt_in * sph, sph + dt_in * cph, dv_in};
+                find_hull(g, hull, T, d, h_in);
+            }
+            {
+                const double T[3] = {g.u_out * cph - t_out * sph, g.u_out * sph + t_out * cph, v_out};
+                const double d[3] = {-(cph - dt_out * sph), -(sph + dt_out * cph), -dv_out};
+                find_hull(g, hull, T, d, h_out);
+            }
+            if (!h_in.ok || !h_out.ok) { flags = PCT_REJ_MISS; break; }
+            if (h_in.tie || h_out.tie) flags |= PCT_TIE;
+            // R5: MLP end states in the gantry frame
+            const double u0 = h_in.P[0] * cph + h_in.P[1] * sph, t0 = -h_in.P[0] * sph + h_in.P[1] * cph, v0 = h_in.P[2];
+            const double u2 = h_out.P[0] * cph + h_out.P[1] * sph, t2 = -h_out.P[0] * sph + h_out.P[1] * cph, v2 = h_out.P[2];
+            const double D = u2 - u0;
+            if (!(D > 0.0)) { flags = PCT_REJ_ORDER; break; }
+            if (D > g.max_depth) { flags = PCT_REJ_DEPTH; break; }
+            const int K = max(1, (int)ceil(D / (g.step_frac * g.h) - 1e-9));     // R8
+            const double du = D / (double)K;
+            // Sigma2 moments: J_q(d2) = int_0^d2 r^q f(D-r) dr = d2^(q+1) sum_j cq[q][j] d2^j,
+            // f(D-r) = sum_j c_j r^j (Taylor shift of the polynomial about the exit depth D)
+            double cq[3][6];
+            {
+                const double binom[6][6] = {{1, 0, 0, 0, 0, 0}, {1, 1, 0, 0, 0, 0}, {1, 2, 1, 0, 0, 0},
+                                            {1, 3, 3, 1, 0, 0}, {1, 4, 6, 4, 1, 0}, {1, 5, 10, 10, 5, 1}};
+                double Dp[6];
+                Dp[0] = 1.0;
+#pragma unroll
+                for (int e = 1; e < 6; ++e) Dp[e] = Dp[e - 1] * D;
+#pragma unroll
+                for (int j = 0; j < 6; ++j) {
+                    double cj = 0.0;
+#pragma unroll
+                    for (int ii = j; ii < 6; ++ii) cj += g.a[ii] * binom[ii][j] * Dp[ii - j];
+                    if (j & 1) cj = -cj;
+#pragma unroll
+                    for (int q = 0; q < 3; ++q) cq[q][j] = cj / (double)(j + q + 1);
+                }
+            }
+            const double nu_t1 = dt_out - dt_in, nu_v1 = dv_out - dv_in;
+            const double inv_X0 = 1.0 / g.X0;
+            // R9-R11 walk state
+            int c[3] = {h_in.c[0], h_in.c[1], h_in.c[2]};
+            start_v = c[0] + g.nx * (c[1] + g.ny * c[2]);
+            CodeWriter cw;
+            cw.init(stage + p, (size_t)stage_stride);
+            double A[3] = {h_in.P[0], h_in.P[1], h_in.P[2]};
+            double L = 0.0;
+            unsigned n_vis = 1;
+            bool tie = false, bad = false;
+            for (int k = 1; k <= K && !bad; ++k) {
+                double B[3];
+                if (k < K) {
+                    // A2 / R7: Gaussian-conditioning form of the MLP of ref [3] (positions only):
+                    // y = mu + Sigma1 R1^T (R1 Sigma1 R1^T + Sigma2)^-1 (y2 - R1 mu), mu = R0 y0
+                    const double w1 = (double)k * du, d2 = D - w1;
+                    const double l1 = fma(g.log_coeff, log(w1 * inv_X0), 1.0), l2 = fma(g.log_coeff, log(d2 * inv_X0), 1.0);
+                    const double g1 = l1 * l1, g2 = l2 * l2;
+                    const double w1_2 = w1 * w1, d2_2 = d2 * d2;
+                    const double C1 = g1 * w1 * horner6(g.s1c[0], w1);
+                    const double B1 = g1 * w1_2 * horner6(g.s1c[1], w1);
+                    const double A1 = g1 * w1_2 * w1 * horner6(g.s1c[2], w1);
+                    const double C2 = g2 * d2 * horner6(cq[0], d2);
+                    const double B2 = g2 * d2_2 * horner6(cq[1], d2);
+                    const double A2 = g2 * d2_2 * d2 * horner6(cq[2], d2);
+                    const double P0 = fma(d2, B1, A1), P1 = fma(d2, C1, B1);      // first row / col of Sigma1 R1^T
+                    const double S00 = fma(d2, P1, P0) + A2, S01 = P1 + B2, S11 = C1 + C2;
+                    const double inv_det = 1.0 / (S00 * S11 - S01 * S01);
+                    const double G00 = (P0 * S11 - B1 * S01) * inv_det, G01 = (B1 * S00 - P0 * S01) * inv_det;
+                    const double mu_t = fma(w1, dt_in, t0), mu_v = fma(w1, dv_in, v0);
+                    const double tk = mu_t + G00 * (t2 - fma(d2, dt_in, mu_t)) + G01 * nu_t1;
+                    const double vk = mu_v + G00 * (v2 - fma(d2, dv_in, mu_v)) + G01 * nu_v1;
+                    const double uk = u0 + w1;
+                    B[0] = uk * cph - tk * sph; B[1] = uk * sph + tk * cph; B[2] = vk;
+                } else {
+                    B[0] = h_out.P[0]; B[1] = h_out.P[1]; B[2] = h_out.P[2];
+                }
+                const double dx = B[0] - A[0], dy = B[1] - A[1], dz = B[2] - A[2];
+                const double seg_len = sqrt(dx * dx + dy * dy + dz * dz);
+                L += seg_len;
+                for (;;) {
+                    Step st;
+                    const int r = lazy_step(g, A, B, seg_len, c, st);
+                    if (r == 0) break;
+                    if (r == 2) { flags = PCT_REJ_LEFT_GRID; bad = true; break; }
+                    if (st.tie) tie = true;
+                    if (++n_vis > (unsigned)g.max_visits) { flags = PCT_REJ_CAPACITY; bad = true; break; }
+                    cw.push(2 * st.axis + (st.dir < 0 ? 1 : 0));
+                }
+                A[0] = B[0]; A[1] = B[1]; A[2] = B[2];
+            }
+            if (bad) break;
+            n_chunks = cw.finish();
+            N = n_vis;
+            if (tie) flags |= PCT_TIE;
+            if (c[0] != h_out.c[0] || c[1] != h_out.c[1] || c[2] != h_out.c[2]) flags |= PCT_END_MISMATCH;   // R10
+            ell = (float)(L / (double)N);                                                                    // R11
+        } while (false);
+        if (N == 0) { n_chunks = 0; start_v = -1; ell = 0.f; }
+        nchunks[p] = (uint32_t)n_chunks;
+        Nout[i] = N;
+        start_out[i] = start_v;
+        ell_out[i] = ell;
+        flags_out[i] = (uint8_t)flags;
+    }
+    // statistics: one atomic per warp
+    const unsigned vis = __reduce_add_sync(0xffffffffu, N);
+    const unsigned rej = __reduce_add_sync(0xffffffffu, (active && N == 0) ? 1u : 0u);
+    const unsigned tie_n = __reduce_add_sync(0xffffffffu, (flags & PCT_TIE) ? 1u : 0u);
+    if ((threadIdx.x & 31) == 0) {
+        if (vis) atomicAdd(&stats->total_visits, (unsigned long long)vis);
+        if (rej) atomicAdd(&stats->n_rejected, (unsigned long long)rej);
+        if (tie_n) atomicAdd(&stats->n_ties, (unsigned long long)tie_n);
+    }
+}
+
+int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, int64_t i_base, int count, int stage_stride,
+                     ulonglong2* stage, uint32_t* nchunks, pct_paths* P, cudaStream_t st) {
+    const int threads = 128;
+    const int blocks = (count + threads - 1) / threads;
+    ProfScope prof(ctx, 0, st);
+    k_mlp_walk<<<blocks, threads, 0, st>>>(ctx->cfg, pr, hull, i_base, count, stage_stride, stage, nchunks, P->N, P->start, P->ell,
+                                           P->flags, ctx->d_stats);
+    ++ctx->launches;
+    PCT_CUDA(ctx, cudaGetLastError());
+    return PCT_OK;
+}
+
+// ---- exclusive scan uint32 -> uint64 (three passes; sizes here are at most a few hundred M) ---------------------
+constexpr int SCAN_THREADS = 256;
+constexpr int SCAN_ITEMS = 8;
+constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
+
+__device__ __forceinline__ unsigned long long block_exclusive_scan(unsigned long long v, unsigned long long* total) {
+    __shared__ unsigned long long warp_sums[SCAN_THREADS / 32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    unsigned long long incl = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const unsigned long long y = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += y;
+    }
+    if (lane == 31) warp_sums[w] = incl;
+    __syncthreads();
+    unsigned long long pre = 0, tot = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_THREADS / 32; ++k) {
+        const unsigned long long s = warp_sums[k];
+        if (k < w) pre += s;
+        tot += s;
+    }
+    __syncthreads();
+    *total = tot;
+    return pre + incl - v;
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_tile_sums(const uint32_t* __restrict__ in, int64_t n,
+                                                                 unsigned long long* __restrict__ sums) {
+    const int64_t base = (int64_t)blockIdx.x * SCAN_TILE;
+    unsigned long long v = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+        const int64_t i = base + (int64_t)k * SCAN_THREADS + threadIdx.x;
+        if (i < n) v += in[i];
+    }
+    unsigned long long tot;
+    block_exclusive_scan(v, &tot);
+    if (threadIdx.x == 0) sums[blockIdx.x] = tot;
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_sums(unsigned long long* sums, int64_t nb, unsigned long long base,
+                                                            unsigned long long* total_out) {
+    unsigned long long carry = base;
+    for (int64_t b0 = 0; b0 < nb; b0 += SCAN_THREADS) {
+        const int64_t i = b0 + threadIdx.x;
+        const unsigned long long v = i < nb ? sums[i] : 0ull;
+        unsigned long long tot;
+        const unsigned long long ex = block_exclusive_scan(v, &tot);
+        if (i < nb) sums[i] = carry + ex;
+        carry += tot;
+    }
+    if (threadIdx.x == 0 && total_out) *total_out = carry - base;
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_finish(const uint32_t* __restrict__ in, int64_t n,
+                                                              const unsigned long long* __restrict__ sums,
+                                                              uint64_t* __restrict__ out) {
+    // thread owns SCAN_ITEMS consecutive items
+    const int64_t base = (int64_t)blockIdx.x * SCAN_TILE + (int64_t)threadIdx.x * SCAN_ITEMS;
+    uint32_t x[SCAN_ITEMS];
+    unsigned long long v = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) { x[k] = (base + k < n) ? in[base + k] : 0u; v += x[k]; }
+    unsigned long long tot;
+    unsigned long long run = sums[blockIdx.x] + block_exclusive_scan(v, &tot);
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+        if (base + k < n) out[base + k] = run;
+        run += x[k];
+    }
+}
+
+int launch_scan_u32(pct_ctx* ctx, const uint32_t* in, uint64_t* out, int64_t n, uint64_t base,
+                    unsigned long long* d_total, cudaStream_t st) {
+    if (n <= 0) {
+        if (d_total) PCT_CUDA(ctx, cudaMemsetAsync(d_total, 0, sizeof(unsigned long long), st));
+        return PCT_OK;
+    }
+    const int64_t nb = (n + SCAN_TILE - 1) / SCAN_TILE;
+    const int64_t need = nb * (int64_t)sizeof(unsigned long long);
+    if (need > ctx->scan_tmp_bytes) {
+        if (ctx->scan_tmp) PCT_CUDA(ctx, cudaFree(ctx->scan_tmp));
+        ctx->scan_tmp = nullptr; ctx->scan_tmp_bytes = 0;
+        PCT_CUDA(ctx, cudaMalloc(&ctx->scan_tmp, (size_t)need));
+        ctx->scan_tmp_bytes = need;
+    }
+    unsigned long long* sums = (unsigned long long*)ctx->scan_tmp;
+    k_scan_tile_sums<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(in, n, sums);
+    k_scan_sums<<<1, SCAN_THREADS, 0, st>>>(sums, nb, base, d_total);
+    k_scan_finish<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(in, n, sums, out);
+    ctx->launches += 3;
+    PCT_CUDA(ctx, cudaGetLastError());
+    return PCT_OK;
+}
+
+// ---- compaction: staging [chunk][history] -> final stream at 16-byte granularity ---------------------------------
+__global__ void __launch_bounds__(256) k_compact(const ulonglong2* __restrict__ stage, const uint32_t* __restrict__ nchunks,
+                                                 const uint64_t* __restrict__ off, int count, int stage_stride,
+                                                 ulonglong2* __restrict__ codes) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= count) return;
+    const uint32_t nc = nchunks[p];
+    const uint64_t o = off[p];
+    for (uint32_t k = 0; k < nc; ++k) codes[o + k] = stage[(size_t)k * stage_stride + p];
+}
+
+int launch_compact(pct_ctx* ctx, const ulonglong2* stage, const uint32_t* nchunks, const uint64_t* off, int count,
+                   int stage_stride, ulonglong2* codes, cudaStream_t st) {
+    if (count <= 0) return PCT_OK;
+    k_compact<<<(count + 255) / 256, 256, 0, st>>>(stage, nchunks, off, count, stage_stride, codes);
+    ++ctx->launches;
+    PCT_CUDA(ctx, cudaGetLastError());
+    return PCT_OK;
+}
+
+// ---- decode (parity / debug): one thread per history expands its codes to voxel indices -------------------------
+__global__ void __launch_bounds__(128) k_decode(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N,
+                                                const int32_t* __restrict__ start, const uint64_t* __restrict__ code_off,
+                                                const ulonglong2* __restrict__ codes, int64_t i0, int64_t i1,
+                                                const uint64_t* __restrict__ row_ptr, int32_t* __restrict__ voxels) {
+    const int64_t i = i0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= i1) return;
+    const uint32_t n = N[i];
+    if (n == 0) return;
+    int32_t* out = voxels + row_ptr[i - i0];
+    int32_t v = start[i];
+    out[0] = v;
+    const ulonglong2* cp = codes + code_off[i];
+    for (uint32_t k = 1; k < n; ++k) {
+        const uint32_t ci = k - 1, w = ci % CODES_PER_CHUNK;
+        const ulonglong2 ch = cp[ci / CODES_PER_CHUNK];
+        const unsigned long long word = w < CODES_PER_WORD ? ch.x : ch.y;
+        const int code = (int)((word >> (3 * (w % CODES_PER_WORD))) & 7ull);
+        const int axis = code >> 1;
+        const int mag = axis == 0 ? g.sx : (axis == 1 ? g.sy : g.sz);
+        v += (code & 1) ? -mag : mag;
+        out[k] = v;
+    }
+}
+
+int launch_decode(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, const uint64_t* row_ptr, int32_t* voxels,
+                  cudaStream_t st) {
+    const int64_t cnt = i1 - i0;
+    if (cnt <= 0) return PCT_OK;
+    k_decode<<<(unsigned)((cnt + 127) / 128), 128, 0, st>>>(ctx->cfg, P->N, P->start, P->code_off, P->codes, i0, i1,
+                                                            row_ptr, voxels);
+    ++ctx->launches;
+    PCT_CUDA(ctx, cudaGetLastError());
+    return PCT_OK;
+}
+
+}  // namespace pct

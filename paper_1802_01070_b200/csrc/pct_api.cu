@@ -1,0 +1,353 @@
+// pct_api.cu -- the extern "C" boundary of libpct.so (include/pct.h) and the iteration driver (A8).
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "pct_internal.cuh"
+
+namespace pct {
+
+int set_error(pct_ctx* ctx, int code, const char* fmt, ...) {
+    if (ctx) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(ctx->err, sizeof(ctx->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+ProfScope::ProfScope(pct_ctx* c, int k, cudaStream_t s) : ctx(c), kind(k), st(s), on(c && c->profiling) {
+    if (!on) return;
+    cudaEvent_t e;
+    if (cudaEventCreate(&e) != cudaSuccess) { on = false; return; }
+    cudaEventRecord(e, st);
+    ctx->prof_events[kind]->push_back(e);
+}
+ProfScope::~ProfScope() {
+    if (!on) return;
+    cudaEvent_t e;
+    if (cudaEventCreate(&e) != cudaSuccess) { cudaEventDestroy(ctx->prof_events[kind]->back()); ctx->prof_events[kind]->pop_back(); return; }
+    cudaEventRecord(e, st);
+    ctx->prof_events[kind]->push_back(e);
+}
+
+static double factorial(int k) { double r = 1.0; for (int i = 2; i <= k; ++i) r *= i; return r; }
+
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev) { cudaGetDevice(&prev); if (prev != dev) cudaSetDevice(dev); else prev = -1; }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+static void free_paths_arrays(pct_paths* P) {
+    cudaFree(P->N); cudaFree(P->start); cudaFree(P->ell); cudaFree(P->flags); cudaFree(P->code_off); cudaFree(P->codes);
+    P->N = nullptr; P->start = nullptr; P->ell = nullptr; P->flags = nullptr; P->code_off = nullptr; P->codes = nullptr;
+}
+
+static int ensure_ds(pct_ctx* ctx, cudaStream_t st) {
+    if (ctx->ds_cap >= ctx->n_vox) return PCT_OK;
+    if (ctx->ds) PCT_CUDA(ctx, cudaFree(ctx->ds));
+    ctx->ds = nullptr; ctx->ds_cap = 0;
+    PCT_CUDA(ctx, cudaMalloc(&ctx->ds, sizeof(float2) * (size_t)ctx->n_vox));
+    ctx->ds_cap = ctx->n_vox;
+    PCT_CUDA(ctx, cudaMemsetAsync(ctx->ds, 0, sizeof(float2) * (size_t)ctx->n_vox, st));
+    return PCT_OK;
+}
+
+// grow the code stream to hold at least `need` chunks (keeps the first `used` chunks)
+static int ensure_codes(pct_ctx* ctx, pct_paths* P, int64_t need, cudaStream_t st) {
+    if (need <= P->chunks_cap) return PCT_OK;
+    int64_t cap = P->chunks_cap + P->chunks_cap / 2;
+    if (cap < need) cap = need;
+    ulonglong2* fresh = nullptr;
+    cudaError_t e = cudaMalloc(&fresh, sizeof(ulonglong2) * (size_t)cap);
+    if (e != cudaSuccess && cap > need) { cudaGetLastError(); cap = need; e = cudaMalloc(&fresh, sizeof(ulonglong2) * (size_t)cap); }
+    if (e != cudaSuccess) { cudaGetLastError(); return set_error(ctx, PCT_E_OOM, "code stream of %lld chunks does not fit", (long long)cap); }
+    if (P->chunks_used > 0)
+        PCT_CUDA(ctx, cudaMemcpyAsync(fresh, P->codes, sizeof(ulonglong2) * (size_t)P->chunks_used, cudaMemcpyDeviceToDevice, st));
+    PCT_CUDA(ctx, cudaStreamSynchronize(st));
+    if (P->codes) PCT_CUDA(ctx, cudaFree(P->codes));
+    P->codes = fresh;
+    P->chunks_cap = cap;
+    return PCT_OK;
+}
+
+}  // namespace pct
+
+using namespace pct;
+
+extern "C" {
+
+int pct_create(const pct_geometry* geom, const pct_mlp_params* params, int device, pct_ctx** out) {
+    if (!out) return PCT_E_INVALID_ARG;
+    *out = nullptr;
+    if (!geom || !params) return PCT_E_INVALID_ARG;
+    if (geom->nx <= 0 || geom->ny <= 0 || geom->nz <= 0 || !(geom->h_mm > 0.0) || !std::isfinite(geom->h_mm)) return PCT_E_INVALID_ARG;
+    if ((int64_t)geom->nx * geom->ny * geom->nz > 0x7fffffffLL) return PCT_E_INVALID_ARG;
+    if (!(params->step_frac > 0.0) || !(params->X0_mm > 0.0) || !(params->tie_eps_mm >= 0.0) || params->max_visits < 1 ||
+        params->max_visits > MAX_VISITS_LIMIT || !(params->poly_max_depth_mm > 0.0)) return PCT_E_INVALID_ARG;
+    for (int i = 0; i < 6; ++i) if (!std::isfinite(params->poly[i])) return PCT_E_INVALID_ARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { cudaGetLastError(); return PCT_E_CUDA; }
+    pct_ctx* ctx = new (std::nothrow) pct_ctx();
+    if (!ctx) return PCT_E_OOM;
+    std::memset(ctx, 0, sizeof(*ctx));
+    for (auto& v : ctx->prof_events) v = new std::vector<cudaEvent_t>();
+    ctx->geom = *geom;
+    ctx->params = *params;
+    ctx->device = device;
+    ctx->n_vox = (int64_t)geom->nx * geom->ny * geom->nz;
+    DevCfg& c = ctx->cfg;
+    c.nx = geom->nx; c.ny = geom->ny; c.nz = geom->nz;
+    c.sx = 1; c.sy = geom->nx; c.sz = geom->nx * geom->ny;
+    c.h = geom->h_mm; c.inv_h = 1.0 / geom->h_mm;
+    const int nn[3] = {geom->nx, geom->ny, geom->nz};
+    for (int a = 0; a < 3; ++a) { c.lo[a] = geom->origin_mm[a]; c.hi[a] = geom->origin_mm[a] + nn[a] * geom->h_mm; }
+    for (int i = 0; i < 6; ++i) {
+        c.a[i] = params->poly[i];
+        // int_0^W (W-w)^q w^i dw = W^(i+q+1) q! i! / (i+q+1)!
+        for (int q = 0; q < 3; ++q) c.s1c[q][i] = params->poly[i] * factorial(q) * factorial(i) / factorial(i + q + 1);
+    }
+    c.X0 = params->X0_mm; c.log_coeff = params->log_coeff; c.step_frac = params->step_frac;
+    c.tie_eps = params->tie_eps_mm; c.max_depth = params->poly_max_depth_mm; c.max_visits = params->max_visits;
+    c.stage_chunks = (params->max_visits - 1 + CODES_PER_CHUNK - 1) / CODES_PER_CHUNK;
+    if (c.stage_chunks < 1) c.stage_chunks = 1;
+    DeviceGuard guard(device);
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { cudaGetLastError(); pct_destroy(ctx); return PCT_E_CUDA; }
+    ctx->num_sms = prop.multiProcessorCount;
+    if (cudaMalloc(&ctx->d_stats, sizeof(GenStats)) != cudaSuccess || cudaMalloc(&ctx->d_total, sizeof(unsigned long long)) != cudaSuccess) {
+        cudaGetLastError(); pct_destroy(ctx); return PCT_E_OOM;
+    }
+    *out = ctx;
+    return PCT_OK;
+}
+
+void pct_destroy(pct_ctx* ctx) {
+    if (!ctx) return;
+    DeviceGuard guard(ctx->device);
+    cudaFree(ctx->ds); cudaFree(ctx->scan_tmp); cudaFree(ctx->d_stats); cudaFree(ctx->d_total);
+    for (auto& v : ctx->prof_events) { if (v) { for (cudaEvent_t e : *v) cudaEventDestroy(e); delete v; } }
+    delete ctx;
+}
+
+int pct_profile_enable(pct_ctx* ctx, int on) {
+    if (!ctx) return PCT_E_INVALID_ARG;
+    ctx->profiling = on != 0;
+    return PCT_OK;
+}
+
+int pct_profile_read(pct_ctx* ctx, pct_profile* out) {
+    if (!ctx || !out) return PCT_E_INVALID_ARG;
+    DeviceGuard guard(ctx->device);
+    PCT_CUDA(ctx, cudaDeviceSynchronize());
+    for (int k = 0; k < 3; ++k) {
+        std::vector<cudaEvent_t>& v = *ctx->prof_events[k];
+        for (size_t i = 0; i + 1 < v.size(); i += 2) {
+            float ms = 0.f;
+            if (cudaEventElapsedTime(&ms, v[i], v[i + 1]) == cudaSuccess) { out->ms[k] += ms; out->launches[k] += 1; }
+        }
+        for (cudaEvent_t e : v) cudaEventDestroy(e);
+        v.clear();
+    }
+    cudaGetLastError();
+    return PCT_OK;
+}
+
+const char* pct_last_error(const pct_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+int64_t pct_launch_count(const pct_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int pct_generate_mlp(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hull, void* stream, pct_paths** out) {
+    if (!ctx) return PCT_E_INVALID_ARG;
+    if (!out) return set_error(ctx, PCT_E_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (!pr || pr->m < 0) return set_error(ctx, PCT_E_INVALID_ARG, "bad protons");
+    if (pr->m > 0 && (!pr->phi || !pr->t_in || !pr->v_in || !pr->dt_in || !pr->dv_in || !pr->t_out || !pr->v_out || !pr->dt_out || !pr->dv_out))
+        return set_error(ctx, PCT_E_INVALID_ARG, "NULL tracker array");
+    if (!std::isfinite(pr->u_in_mm) || !std::isfinite(pr->u_out_mm)) return set_error(ctx, PCT_E_INVALID_ARG, "bad tracker planes");
+    DeviceGuard guard(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    ctx->cfg.u_in = pr->u_in_mm; ctx->cfg.u_out = pr->u_out_mm;
+    pct_paths* P = new (std::nothrow) pct_paths();
+    if (!P) return set_error(ctx, PCT_E_OOM, "host allocation");
+    std::memset(P, 0, sizeof(*P));
+    P->device = ctx->device; P->m = pr->m; P->n_vox = ctx->n_vox;
+    const int64_t m = pr->m;
+    const size_t mm = (size_t)(m > 0 ? m : 1);
+    ulonglong2* stage = nullptr;
+    uint32_t* nchunks = nullptr;
+    int rc = PCT_OK;
+    auto fail = [&](int code) { cudaFree(stage); cudaFree(nchunks); free_paths_arrays(P); delete P; return code; };
+#define GEN_CUDA(call)                                                                                          \
+    do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { cudaGetLastError();                               \
+        return fail(set_error(ctx, e__ == cudaErrorMemoryAllocation ? PCT_E_OOM : PCT_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e__))); } } while (0)
+    GEN_CUDA(cudaMalloc(&P->N, sizeof(uint32_t) * mm));
+    GEN_CUDA(cudaMalloc(&P->start, sizeof(int32_t) * mm));
+    GEN_CUDA(cudaMalloc(&P->ell, sizeof(float) * mm));
+    GEN_CUDA(cudaMalloc(&P->flags, sizeof(uint8_t) * mm));
+    GEN_CUDA(cudaMalloc(&P->code_off, sizeof(uint64_t) * mm));
+    const int batch_max = (int)(m < GEN_BATCH ? (m > 0 ? m : 1) : GEN_BATCH);
+    GEN_CUDA(cudaMalloc(&stage, sizeof(ulonglong2) * (size_t)batch_max * (size_t)ctx->cfg.stage_chunks));
+    GEN_CUDA(cudaMalloc(&nchunks, sizeof(uint32_t) * (size_t)batch_max));
+    GEN_CUDA(cudaMemsetAsync(ctx->d_stats, 0, sizeof(GenStats), st));
+    const ProtonPtrs pp = {pr->phi, pr->t_in, pr->v_in, pr->dt_in, pr->dv_in, pr->t_out, pr->v_out, pr->dt_out, pr->dv_out};
+    for (int64_t i0 = 0; i0 < m; i0 += GEN_BATCH) {
+        const int count = (int)((m - i0) < GEN_BATCH ? (m - i0) : GEN_BATCH);
+        if ((rc = launch_mlp_batch(ctx, pp, hull, i0, count, batch_max, stage, nchunks, P, st)) != PCT_OK) return fail(rc);
+        if ((rc = launch_scan_u32(ctx, nchunks, P->code_off + i0, count, (uint64_t)P->chunks_used, ctx->d_total, st)) != PCT_OK) return fail(rc);
+        unsigned long long batch_chunks = 0;
+        GEN_CUDA(cudaMemcpyAsync(&batch_chunks, ctx->d_total, sizeof(batch_chunks), cudaMemcpyDeviceToHost, st));
+        GEN_CUDA(cudaStreamSynchronize(st));
+        int64_t need = P->chunks_used + (int64_t)batch_chunks;
+        if (need > P->chunks_cap) {
+            // first batch: extrapolate to all histories (+25 %); later: ensure_codes grows by 1.5x
+            int64_t guess = need;
+            if (i0 == 0 && m > count) guess = (int64_t)((double)batch_chunks * ((double)m / (double)count) * 1.25) + 1024;
+            if ((rc = ensure_codes(ctx, P, guess > need ? guess : need, st)) != PCT_OK) {
+                if (guess > need && (rc = ensure_codes(ctx, P, need, st)) != PCT_OK) return fail(rc);
+            }
+        }
+        if ((rc = launch_compact(ctx, stage, nchunks, P->code_off + i0, count, batch_max, P->codes, st)) != PCT_OK) return fail(rc);
+        P->chunks_used = need;
+    }
+    GenStats hs;
+    GEN_CUDA(cudaMemcpyAsync(&hs, ctx->d_stats, sizeof(hs), cudaMemcpyDeviceToHost, st));
+    GEN_CUDA(cudaStreamSynchronize(st));
+#undef GEN_CUDA
+    cudaFree(stage); cudaFree(nchunks);
+    P->total_visits = (int64_t)hs.total_visits; P->n_rejected = (int64_t)hs.n_rejected; P->n_ties = (int64_t)hs.n_ties;
+    *out = P;
+    return PCT_OK;
+}
+
+int pct_paths_info(const pct_paths* P, pct_paths_stats* out) {
+    if (!P || !out) return PCT_E_INVALID_ARG;
+    out->m = P->m; out->total_visits = P->total_visits; out->n_rejected = P->n_rejected; out->n_ties = P->n_ties;
+    out->code_bytes = P->chunks_used * (int64_t)sizeof(ulonglong2);
+    out->header_bytes = P->m * (int64_t)(sizeof(uint32_t) + sizeof(int32_t) + sizeof(float) + sizeof(uint8_t) + sizeof(uint64_t));
+    return PCT_OK;
+}
+
+void pct_paths_free(pct_paths* P) {
+    if (!P) return;
+    DeviceGuard guard(P->device);
+    free_paths_arrays(P);
+    delete P;
+}
+
+int pct_paths_decode(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, int64_t* row_ptr, int32_t* voxels, int64_t cap,
+                     float* ell, uint8_t* flags, void* stream) {
+    if (!ctx) return PCT_E_INVALID_ARG;
+    if (!P || !row_ptr || i0 < 0 || i1 > P->m || i0 > i1) return set_error(ctx, PCT_E_INVALID_ARG, "bad decode range");
+    DeviceGuard guard(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t cnt = i1 - i0;
+    int rc;
+    if ((rc = launch_scan_u32(ctx, P->N + i0, (uint64_t*)row_ptr, cnt, 0, ctx->d_total, st)) != PCT_OK) return rc;
+    PCT_CUDA(ctx, cudaMemcpyAsync(row_ptr + cnt, ctx->d_total, sizeof(int64_t), cudaMemcpyDeviceToDevice, st));
+    unsigned long long total = 0;
+    PCT_CUDA(ctx, cudaMemcpyAsync(&total, ctx->d_total, sizeof(total), cudaMemcpyDeviceToHost, st));
+    if (ell && cnt) PCT_CUDA(ctx, cudaMemcpyAsync(ell, P->ell + i0, sizeof(float) * (size_t)cnt, cudaMemcpyDeviceToDevice, st));
+    if (flags && cnt) PCT_CUDA(ctx, cudaMemcpyAsync(flags, P->flags + i0, (size_t)cnt, cudaMemcpyDeviceToDevice, st));
+    PCT_CUDA(ctx, cudaStreamSynchronize(st));
+    if (voxels) {
+        if ((int64_t)total > cap) return set_error(ctx, PCT_E_CAPACITY, "decode needs %llu voxel slots, cap is %lld", total, (long long)cap);
+        if ((rc = launch_decode(ctx, P, i0, i1, (const uint64_t*)row_ptr, voxels, st)) != PCT_OK) return rc;
+        PCT_CUDA(ctx, cudaStreamSynchronize(st));
+    }
+    return PCT_OK;
+}
+
+int pct_forward_project(pct_ctx* ctx, const pct_paths* P, const float* x, float* b_out, void* stream) {
+    if (!ctx) return PCT_E_INVALID_ARG;
+    if (!P || !x || !b_out || P->n_vox != ctx->n_vox) return set_error(ctx, PCT_E_INVALID_ARG, "bad forward_project arguments");
+    DeviceGuard guard(ctx->device);
+    return launch_forward_project(ctx, P, x, b_out, (cudaStream_t)stream);
+}
+
+int pct_column_counts(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, uint32_t* counts, void* stream) {
+    if (!ctx) return PCT_E_INVALID_ARG;
+    if (!P || !counts || i0 < 0 || i1 > P->m || i0 > i1 || P->n_vox != ctx->n_vox) return set_error(ctx, PCT_E_INVALID_ARG, "bad column_counts arguments");
+    DeviceGuard guard(ctx->device);
+    return launch_column_counts(ctx, P, i0, i1, counts, (cudaStream_t)stream);
+}
+
+// A8: the iteration driver.  iters x ceil(m/B) x (project+scatter, update) on one stream, no host sync inside.
+int pct_solve(pct_ctx* ctx, const pct_paths* P, const float* b, const float* x0, int iters, int64_t block_size, float lambda,
+              float* x_out, void* stream) {
+    if (!ctx) return PCT_E_INVALID_ARG;
+    if (!P || !b || !x0 || !x_out || iters < 0 || block_size < 1 || P->n_vox != ctx->n_vox || !std::isfinite(lambda))
+        return set_error(ctx, PCT_E_INVALID_ARG, "bad solve arguments");
+    DeviceGuard guard(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc;
+    if ((rc = ensure_ds(ctx, st)) != PCT_OK) return rc;
+    if (x_out != x0) PCT_CUDA(ctx, cudaMemcpyAsync(x_out, x0, sizeof(float) * (size_t)ctx->n_vox, cudaMemcpyDeviceToDevice, st));
+    for (int it = 0; it < iters; ++it) {
+        for (int64_t i0 = 0; i0 < P->m; i0 += block_size) {
+            const int64_t i1 = (P->m - i0) < block_size ? P->m : i0 + block_size;
+            if ((rc = launch_block_project_scatter(ctx, P, i0, i1, b, x_out, ctx->ds, st)) != PCT_OK) return rc;
+            if ((rc = launch_block_update(ctx, x_out, ctx->ds, lambda, st)) != PCT_OK) return rc;
+        }
+    }
+    return PCT_OK;
+}
+
+int pct_reconstruct_host(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hull_host, const float* b_host, const float* x0_host,
+                         int iters, int64_t block_size, float lambda, float* x_out_host, pct_recon_stats* stats, void* stream) {
+    if (!ctx) return PCT_E_INVALID_ARG;
+    if (!pr || pr->m < 0 || !b_host || !x_out_host || iters < 0 || block_size < 1) return set_error(ctx, PCT_E_INVALID_ARG, "bad reconstruct arguments");
+    DeviceGuard guard(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t m = pr->m, n = ctx->n_vox;
+    const size_t mm = (size_t)(m > 0 ? m : 1);
+    double* d_tr = nullptr; float* d_b = nullptr; float* d_x = nullptr; uint8_t* d_hull = nullptr;
+    pct_paths* P = nullptr;
+    cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    int rc = PCT_OK;
+    auto cleanup = [&]() {
+        cudaFree(d_tr); cudaFree(d_b); cudaFree(d_x); cudaFree(d_hull);
+        if (P) pct_paths_free(P);
+        for (auto& e : ev) if (e) cudaEventDestroy(e);
+    };
+#define REC_CUDA(call)                                                                                          \
+    do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { cudaGetLastError(); cleanup();                    \
+        return set_error(ctx, e__ == cudaErrorMemoryAllocation ? PCT_E_OOM : PCT_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e__)); } } while (0)
+    for (auto& e : ev) REC_CUDA(cudaEventCreate(&e));
+    REC_CUDA(cudaMalloc(&d_tr, sizeof(double) * 9 * mm));
+    REC_CUDA(cudaMalloc(&d_b, sizeof(float) * mm));
+    REC_CUDA(cudaMalloc(&d_x, sizeof(float) * (size_t)n));
+    if (hull_host) REC_CUDA(cudaMalloc(&d_hull, (size_t)n));
+    REC_CUDA(cudaEventRecord(ev[0], st));
+    const double* src[9] = {pr->phi, pr->t_in, pr->v_in, pr->dt_in, pr->dv_in, pr->t_out, pr->v_out, pr->dt_out, pr->dv_out};
+    for (int k = 0; k < 9 && m > 0; ++k) REC_CUDA(cudaMemcpyAsync(d_tr + (size_t)k * mm, src[k], sizeof(double) * (size_t)m, cudaMemcpyHostToDevice, st));
+    if (m > 0) REC_CUDA(cudaMemcpyAsync(d_b, b_host, sizeof(float) * (size_t)m, cudaMemcpyHostToDevice, st));
+    if (hull_host) REC_CUDA(cudaMemcpyAsync(d_hull, hull_host, (size_t)n, cudaMemcpyHostToDevice, st));
+    if (x0_host) REC_CUDA(cudaMemcpyAsync(d_x, x0_host, sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, st));
+    REC_CUDA(cudaEventRecord(ev[1], st));
+    pct_protons dev = *pr;
+    dev.phi = d_tr; dev.t_in = d_tr + mm; dev.v_in = d_tr + 2 * mm; dev.dt_in = d_tr + 3 * mm; dev.dv_in = d_tr + 4 * mm;
+    dev.t_out = d_tr + 5 * mm; dev.v_out = d_tr + 6 * mm; dev.dt_out = d_tr + 7 * mm; dev.dv_out = d_tr + 8 * mm;
+    if ((rc = pct_generate_mlp(ctx, &dev, d_hull, stream, &P)) != PCT_OK) { cleanup(); return rc; }
+    REC_CUDA(cudaEventRecord(ev[2], st));
+    if (!x0_host && (rc = launch_fill(ctx, d_x, n, 1.0f, st)) != PCT_OK) { cleanup(); return rc; }   // x0 = 1 (BASELINE.json configs)
+    if ((rc = pct_solve(ctx, P, d_b, d_x, iters, block_size, lambda, d_x, stream)) != PCT_OK) { cleanup(); return rc; }
+    REC_CUDA(cudaEventRecord(ev[3], st));
+    REC_CUDA(cudaMemcpyAsync(x_out_host, d_x, sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost, st));
+    REC_CUDA(cudaEventRecord(ev[4], st));
+    REC_CUDA(cudaStreamSynchronize(st));
+    if (stats) {
+        stats->m = m; stats->total_visits = P->total_visits; stats->n_rejected = P->n_rejected; stats->n_ties = P->n_ties;
+        float ms[4] = {0, 0, 0, 0};
+        for (int k = 0; k < 4; ++k) cudaEventElapsedTime(&ms[k], ev[k], ev[k + 1]);
+        stats->ms_h2d = ms[0]; stats->ms_mlp = ms[1]; stats->ms_solve = ms[2]; stats->ms_d2h = ms[3];
+    }
+#undef REC_CUDA
+    cleanup();
+    return PCT_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,112 @@
+// pct_internal.cuh -- shared declarations of libpct.so (CUDA path only; nothing here is used by oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "pct.h"
+
+namespace pct {
+
+// ---- encoding of one row of A (R9-R12) -------------------------------------------------------------------
+// A row is  start voxel (int32)  +  N-1 face-step codes of 3 bits:  0:+x 1:-x 2:+y 3:-y 4:+z 5:-z 7:pad.
+// Codes are packed 21 per uint64 (bits 3k..3k+2), two uint64 = one 16-byte chunk = 42 codes, so the stream is
+// read with 128-bit loads and every row starts on a 16-byte boundary.
+constexpr int CODES_PER_WORD = 21;
+constexpr int CODES_PER_CHUNK = 42;
+constexpr int MAX_VISITS_LIMIT = 8192;
+constexpr int GEN_BATCH = 1 << 20;   // histories per generation batch (bounds the worst-case staging buffer)
+
+// constants handed to kernels by value (__grid_constant__)
+struct DevCfg {
+    int nx, ny, nz;
+    int sx, sy, sz;            // linear strides 1, nx, nx*ny
+    double h, inv_h;
+    double lo[3], hi[3];
+    double a[6];               // f(w) = sum a_i w^i
+    double s1c[3][6];          // Sigma1 moments: I_q(w) = w^(q+1) * sum_i s1c[q][i] w^i,  s1c[q][i] = a_i q! i!/(i+q+1)!
+    double X0, log_coeff, step_frac, tie_eps, max_depth;
+    int max_visits;
+    int stage_chunks;          // chunks per history in the staging buffer
+    double u_in, u_out;
+};
+
+struct ProtonPtrs {
+    const double *phi, *t_in, *v_in, *dt_in, *dv_in, *t_out, *v_out, *dt_out, *dv_out;
+};
+
+struct GenStats { unsigned long long total_visits, n_rejected, n_ties; };
+
+}  // namespace pct
+
+struct pct_ctx {
+    pct_geometry geom;
+    pct_mlp_params params;
+    pct::DevCfg cfg;
+    int device;
+    int num_sms;
+    int64_t n_vox;
+    int64_t launches;
+    char err[512];
+    // scratch owned by the context (grown on demand)
+    float2* ds;          // {Delta_j, s_j} accumulator, n_vox
+    int64_t ds_cap;
+    void* scan_tmp;      // block sums for scans
+    int64_t scan_tmp_bytes;
+    pct::GenStats* d_stats;
+    unsigned long long* d_total;
+    // optional per-kernel event timing (pct_profile_enable)
+    bool profiling;
+    std::vector<cudaEvent_t>* prof_events[3];   // start/stop pairs per kind
+};
+
+struct pct_paths {
+    int device;
+    int64_t m, n_vox;
+    uint32_t* N;         // path entries per history
+    int32_t* start;      // start voxel
+    float* ell;          // mean chord l_i (R11)
+    uint8_t* flags;
+    uint64_t* code_off;  // first 16-byte chunk of the row in `codes`
+    ulonglong2* codes;
+    int64_t chunks_used, chunks_cap;
+    int64_t total_visits, n_rejected, n_ties;
+};
+
+namespace pct {
+
+int set_error(pct_ctx* ctx, int code, const char* fmt, ...);
+
+// RAII bracket around one kernel launch when profiling is on (kind: 0 MLP, 1 project+scatter, 2 update)
+struct ProfScope {
+    pct_ctx* ctx; int kind; cudaStream_t st; bool on;
+    ProfScope(pct_ctx* c, int k, cudaStream_t s);
+    ~ProfScope();
+};
+
+#define PCT_CUDA(ctx, call)                                                                              \
+    do {                                                                                                 \
+        cudaError_t e__ = (call);                                                                        \
+        if (e__ != cudaSuccess)                                                                          \
+            return pct::set_error((ctx), e__ == cudaErrorMemoryAllocation ? PCT_E_OOM : PCT_E_CUDA,      \
+                                  "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e__), __FILE__, __LINE__); \
+    } while (0)
+
+// launchers implemented in the .cu files (all enqueue on `st`, none synchronises unless stated)
+int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, int64_t i_base, int count, int stage_stride,
+                     ulonglong2* stage, uint32_t* nchunks, pct_paths* P, cudaStream_t st);
+int launch_scan_u32(pct_ctx* ctx, const uint32_t* in, uint64_t* out, int64_t n, uint64_t base,
+                    unsigned long long* d_total, cudaStream_t st);
+int launch_compact(pct_ctx* ctx, const ulonglong2* stage, const uint32_t* nchunks, const uint64_t* off, int count,
+                   int stage_stride, ulonglong2* codes, cudaStream_t st);
+int launch_decode(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, const uint64_t* row_ptr, int32_t* voxels,
+                  cudaStream_t st);
+int launch_forward_project(pct_ctx* ctx, const pct_paths* P, const float* x, float* b_out, cudaStream_t st);
+int launch_column_counts(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, uint32_t* counts, cudaStream_t st);
+int launch_block_project_scatter(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, const float* b,
+                                 const float* x, float2* ds, cudaStream_t st);
+int launch_block_update(pct_ctx* ctx, float* x, float2* ds, float lambda, cudaStream_t st);
+int launch_fill(pct_ctx* ctx, float* p, int64_t n, float value, cudaStream_t st);
+
+}  // namespace pct

@@ -1,0 +1,243 @@
+"""Parity of the CUDA path (through the C-ABI binding) against the CPU oracle, element by element.
+
+Acceptance (BASELINE.json north_star): voxel lists bit-exact except logged ties (< 1e-9 mm, fraction < 1e-6);
+image after k iterations within rel-L2 1e-4 and max-abs 1e-3 (FP32 atomics vs FP64 oracle).
+"""
+import dataclasses
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from paper_1802_01070_b200 import synth
+from helpers import oracle_setup, split_rows
+
+pytestmark = pytest.mark.gpu
+
+REL_L2_TOL, MAX_ABS_TOL = 1e-4, 1e-3      # north_star acceptance, FP32 solver vs FP64 oracle
+
+
+@pytest.fixture(scope="module")
+def binding():
+    from paper_1802_01070_b200 import binding as b
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    b.load_library()
+    return b
+
+
+def gpu_paths(binding, cfg, protons, hull, params_override=None):
+    kw = synth.mlp_params(cfg)
+    if params_override:
+        kw.update(params_override)
+    ctx = binding.Context(synth.geometry(cfg), kw, 0)
+    dev = {k: torch.as_tensor(np.asarray(v), dtype=torch.float64).cuda().contiguous() if not torch.is_tensor(v)
+           else v.to(torch.float64).cuda().contiguous() for k, v in protons.items() if k != "wepl"}
+    h = None if hull is None else torch.as_tensor(np.asarray(hull.cpu() if torch.is_tensor(hull) else hull)).to(torch.uint8).cuda().contiguous().reshape(-1)
+    return ctx, ctx.generate_mlp(dev, -cfg.u_tracker, cfg.u_tracker, h)
+
+
+def compare_lists(binding, oracle, ctx, paths, P, i0=0, i1=None):
+    """Returns (#mismatching rows, #rows).  Asserts every mismatch is a logged tie on at least one side."""
+    row_ptr_g, vox_g, ell_g, flags_g = [t.cpu().numpy() for t in ctx.paths_decode(paths, i0, i1)]
+    row_ptr_o, vox_o, ell_o, flags_o, _ = P.rows(i0, i1)
+    k = len(row_ptr_o) - 1
+    mism = np.zeros(k, bool)
+    if not (np.array_equal(row_ptr_g, row_ptr_o) and np.array_equal(vox_g, vox_o)):     # slow path: find the rows
+        for r in range(k):
+            a, b = vox_g[row_ptr_g[r]:row_ptr_g[r + 1]], vox_o[row_ptr_o[r]:row_ptr_o[r + 1]]
+            mism[r] = len(a) != len(b) or bool(np.any(a != b))
+    tie = ((flags_g | flags_o) & binding.TIE) != 0
+    assert not np.any(mism & ~tie), f"unlogged voxel-list mismatch in rows {np.nonzero(mism & ~tie)[0][:10] + i0}"
+    ok = ~mism
+    rej_g, rej_o = flags_g & binding.REJECT_MASK, flags_o & oracle.REJECT_MASK
+    assert np.array_equal(rej_g[ok], rej_o[ok])
+    assert np.array_equal(flags_g[ok] & binding.END_MISMATCH, flags_o[ok] & oracle.END_MISMATCH)
+    assert np.allclose(ell_g[ok], ell_o[ok], rtol=2e-7, atol=0)
+    return int(mism.sum()), k
+
+
+def test_tiny_full_parity(binding, oracle):
+    """BASELINE.json config 0 end to end: lists, l_i, flags, forward projection, counts and the solved image."""
+    cfg = synth.CONFIGS["tiny"]
+    x_true, hull, shadow = synth.make_phantom(cfg)
+    pr = synth.generate_protons(cfg, x_true, shadow)
+    g, p, pa, P = oracle_setup(oracle, cfg, pr, hull)
+    ctx, paths = gpu_paths(binding, cfg, pr, hull)
+    assert paths.m == P.m == cfg.m
+    n_mis, k = compare_lists(binding, oracle, ctx, paths, P)
+    assert n_mis <= max(1, int(1e-6 * k))
+    if n_mis == 0:
+        assert paths.total_visits == P.total_visits and paths.n_rejected == P.n_rejected
+    # forward projection and column counts
+    xt = x_true.reshape(-1).cuda()
+    b_g = ctx.forward_project(paths, xt).cpu().numpy()
+    b_o = P.forward_project(x_true.numpy())
+    assert np.allclose(b_g, b_o, rtol=2e-5, atol=1e-5)
+    for (i0, i1) in ((0, cfg.m), (5000, 10000), (49990, 50000), (7, 7)):
+        c_g = ctx.column_counts(paths, i0, i1).cpu().numpy().view(np.uint32)
+        if n_mis == 0:
+            assert np.array_equal(c_g, P.column_counts(i0, i1))
+    # solver at the configured settings (5 iterations, B = 5000, lambda = 0.1, x0 = 1)
+    b = pr["wepl"].cuda()
+    x0 = torch.ones(cfg.n, dtype=torch.float32, device="cuda")
+    x_g = ctx.solve(paths, b, x0, cfg.iters, cfg.block, cfg.lam).cpu().numpy()
+    x_o = P.solve(pr["wepl"].numpy(), np.ones(cfg.n, np.float32), cfg.iters, cfg.block, cfg.lam)
+    assert np.linalg.norm(x_g - x_o) / np.linalg.norm(x_o) <= REL_L2_TOL
+    assert np.max(np.abs(x_g - x_o)) <= MAX_ABS_TOL
+    assert np.abs(x_g - 1.0).max() > 0.05            # it did move
+    # in-place (x_out aliases x0) gives the same image up to atomic ordering
+    x_alias = x0.clone()
+    ctx.solve(paths, b, x_alias, cfg.iters, cfg.block, cfg.lam, out=x_alias)
+    assert np.max(np.abs(x_alias.cpu().numpy() - x_g)) <= 1e-4
+
+
+@pytest.mark.parametrize("B,lam,iters", [(1, 0.5, 1), (37, 0.2, 2), (1000, 0.05, 3), (4096, 0.1, 2), (10 ** 6, 0.2, 2)])
+def test_block_sizes_and_ragged_tails(binding, oracle, B, lam, iters):
+    """Config-4 style corners at a size the oracle finishes in seconds: B=1, ragged last block, B > m."""
+    cfg = synth.scaled(synth.CONFIGS["tiny"], 4500 if B > 1 else 300)
+    x_true, hull, shadow = synth.make_phantom(cfg)
+    pr = synth.generate_protons(cfg, x_true, shadow)
+    g, p, pa, P = oracle_setup(oracle, cfg, pr, hull)
+    ctx, paths = gpu_paths(binding, cfg, pr, hull)
+    compare_lists(binding, oracle, ctx, paths, P)
+    x0 = torch.ones(cfg.n, dtype=torch.float32, device="cuda")
+    x_g = ctx.solve(paths, pr["wepl"].cuda(), x0, iters, B, lam).cpu().numpy()
+    x_o = P.solve(pr["wepl"].numpy(), np.ones(cfg.n, np.float32), iters, B, lam)
+    assert np.linalg.norm(x_g - x_o) / np.linalg.norm(x_o) <= REL_L2_TOL
+    assert np.max(np.abs(x_g - x_o)) <= MAX_ABS_TOL
+
+
+def test_non_unit_voxels_no_hull(binding, oracle):
+    """h = 0.7 mm, off-centre origin, hull = NULL (every voxel), straight and kinked histories."""
+    cfg = dataclasses.replace(synth.CONFIGS["tiny"], name="tiny-h07", nx=24, ny=30, nz=10, h=0.7, u_tracker=30.0, m=3000)
+    rays = synth.random_rays(cfg.m, cfg, seed=9)
+    rng = np.random.default_rng(10)
+    kick = torch.from_numpy(rng.normal(0, 0.03, cfg.m))
+    rays["dt_out"] = rays["dt_out"] + kick
+    rays["t_out"] = rays["t_out"] + 0.5 * kick * 2 * cfg.u_tracker
+    geom = synth.geometry(cfg)
+    geom["origin_mm"] = (-8.3, -10.1, -3.3)
+    g = oracle.make_geometry(**geom)
+    p = oracle.make_params(**synth.mlp_params(cfg))
+    pa = oracle.ProtonArrays({k: v.numpy() for k, v in rays.items()}, -cfg.u_tracker, cfg.u_tracker)
+    P = oracle.Paths(g, p, pa, None)
+    ctx = binding.Context(geom, synth.mlp_params(cfg), 0)
+    dev = {k: v.cuda() for k, v in rays.items()}
+    paths = ctx.generate_mlp(dev, -cfg.u_tracker, cfg.u_tracker, None)
+    n_mis, k = compare_lists(binding, oracle, ctx, paths, P)
+    assert n_mis <= 1 and paths.total_visits > 20 * cfg.m * 0.5
+
+
+def test_rejections_and_degenerate_inputs(binding, oracle):
+    cfg = synth.scaled(synth.CONFIGS["tiny"], 6)
+    x_true, hull, shadow = synth.make_phantom(cfg)
+    z = np.zeros(6)
+    pr = dict(phi=z.copy(), t_in=z.copy(), v_in=z.copy(), dt_in=z.copy(), dv_in=z.copy(), t_out=z.copy(),
+              v_out=z.copy(), dt_out=z.copy(), dv_out=z.copy())
+    pr["t_in"][1] = pr["t_out"][1] = 15.5
+    pr["t_in"][2] = pr["t_out"][2] = 40.0
+    pr["t_in"][3] = np.nan
+    pr["dv_in"][4] = 0.5; pr["v_out"][4] = 22.0; pr["dv_out"][4] = 0.5
+    for override in (None, dict(max_visits=10), dict(poly_max_depth_mm=20.0)):
+        g, p, pa, P = oracle_setup(oracle, cfg, pr, hull, params_override=override)
+        ctx, paths = gpu_paths(binding, cfg, pr, hull, params_override=override)
+        _, _, _, flags_g = [t.cpu().numpy() for t in ctx.paths_decode(paths)]
+        assert np.array_equal(flags_g, P.rows()[3])
+        assert (paths.total_visits, paths.n_rejected) == (P.total_visits, P.n_rejected)
+        compare_lists(binding, oracle, ctx, paths, P)
+        # rejected histories contribute nothing: b_hat = 0 and the solve ignores them
+        b_hat = ctx.forward_project(paths, torch.ones(cfg.n, device="cuda")).cpu().numpy()
+        assert np.all(b_hat[np.diff(P.rows()[0]) == 0] == 0)
+    # m = 0
+    ctx = binding.Context(synth.geometry(cfg), synth.mlp_params(cfg), 0)
+    empty = {k: torch.empty(0, dtype=torch.float64, device="cuda") for k in binding.PROTON_KEYS}
+    paths = ctx.generate_mlp(empty, -22.0, 22.0, hull.cuda().reshape(-1))
+    assert paths.m == 0 and paths.total_visits == 0
+    x0 = torch.full((cfg.n,), 0.7, dtype=torch.float32, device="cuda")
+    x = ctx.solve(paths, torch.empty(0, dtype=torch.float32, device="cuda"), x0, 3, 100, 0.1)
+    assert torch.equal(x, x0)
+    # argument errors are reported, not fatal
+    with pytest.raises(binding.PctError):
+        ctx.solve(paths, torch.empty(0, dtype=torch.float32, device="cuda"), x0, 3, 0, 0.1)
+    with pytest.raises(binding.PctError):
+        binding.Context(dict(nx=0, ny=4, nz=4, h_mm=1.0, origin_mm=(0, 0, 0)), synth.mlp_params(cfg), 0)
+
+
+@pytest.mark.parametrize("name,m,B", [("head", 24000, 5000), ("paperA", 12000, 5000), ("paperB", 8000, 3000)])
+def test_big_phantom_samples(binding, oracle, name, m, B):
+    """Configs 1-3 geometry/beam/energy at an oracle-sized history count: several blocks and a ragged tail."""
+    cfg = synth.scaled(synth.CONFIGS[name], m, block=B, iters=2)
+    x_true, hull, shadow = synth.make_phantom(cfg, "cuda")
+    pr = synth.generate_protons(cfg, x_true, shadow, device="cuda")
+    pr_h = {k: v.cpu() for k, v in pr.items()}
+    g, p, pa, P = oracle_setup(oracle, cfg, pr_h, hull.cpu())
+    ctx, paths = gpu_paths(binding, cfg, pr, hull)
+    n_mis, k = compare_lists(binding, oracle, ctx, paths, P)
+    assert n_mis <= 1
+    assert paths.n_rejected < 0.1 * m
+    x0 = torch.ones(cfg.n, dtype=torch.float32, device="cuda")
+    x_g = ctx.solve(paths, pr["wepl"], x0, cfg.iters, cfg.block, cfg.lam).cpu().numpy()
+    x_o = P.solve(pr_h["wepl"].numpy(), np.ones(cfg.n, np.float32), cfg.iters, cfg.block, cfg.lam)
+    assert np.linalg.norm(x_g - x_o) / np.linalg.norm(x_o) <= REL_L2_TOL
+    assert np.max(np.abs(x_g - x_o)) <= MAX_ABS_TOL
+
+
+def test_reconstruct_host_matches_device_calls(binding, oracle):
+    cfg = synth.scaled(synth.CONFIGS["tiny"], 6000, block=2000, iters=2)
+    x_true, hull, shadow = synth.make_phantom(cfg)
+    pr = synth.generate_protons(cfg, x_true, shadow)
+    ctx, paths = gpu_paths(binding, cfg, pr, hull)
+    x_ref = ctx.solve(paths, pr["wepl"].cuda(), torch.ones(cfg.n, device="cuda"), cfg.iters, cfg.block, cfg.lam).cpu()
+    host = {k: pr[k].contiguous().pin_memory() for k in binding.PROTON_KEYS}
+    x_out = torch.empty(cfg.n, dtype=torch.float32).pin_memory()
+    st = ctx.reconstruct_host(host, -cfg.u_tracker, cfg.u_tracker, hull.reshape(-1).contiguous(), pr["wepl"].contiguous(),
+                              None, cfg.iters, cfg.block, cfg.lam, x_out)
+    assert st["total_visits"] == paths.total_visits and st["m"] == cfg.m
+    assert torch.max(torch.abs(x_out - x_ref)).item() <= 1e-4
+    g, p, pa, P = oracle_setup(oracle, cfg, pr, hull)
+    x_o = P.solve(pr["wepl"].numpy(), np.ones(cfg.n, np.float32), cfg.iters, cfg.block, cfg.lam)
+    assert np.max(np.abs(x_out.numpy() - x_o)) <= MAX_ABS_TOL
+
+
+def test_head_full_size_sampled(binding, oracle):
+    """BASELINE.json config 1 at FULL size (20 M histories, the launch configuration bench.py times): voxel lists of
+    sampled runs of histories vs the oracle one by one, plus size-independent properties of the full result."""
+    m = int(os.environ.get("PCT_TEST_FULL_M", 20_000_000))
+    cfg = synth.scaled(synth.CONFIGS["head"], m)
+    x_true, hull, shadow = synth.make_phantom(cfg, "cuda")
+    pr = synth.generate_protons(cfg, x_true, shadow, device="cuda")
+    ctx, paths = gpu_paths(binding, cfg, pr, hull)
+    assert paths.m == m and paths.n_rejected < 0.05 * m
+    rng = np.random.default_rng(0)
+    starts = np.sort(rng.integers(0, m - 400, 24))
+    total_mis = 0
+    for s in starts:
+        sub = {k: v[s:s + 400].cpu() for k, v in pr.items()}
+        g, p, pa, P = oracle_setup(oracle, cfg, sub, hull.cpu())
+        row_ptr_g, vox_g, ell_g, flags_g = [t.cpu().numpy() for t in ctx.paths_decode(paths, int(s), int(s) + 400)]
+        row_ptr_o, vox_o, ell_o, flags_o, _ = P.rows()
+        for r in range(400):
+            a, b = vox_g[row_ptr_g[r]:row_ptr_g[r + 1]], vox_o[row_ptr_o[r]:row_ptr_o[r + 1]]
+            if len(a) != len(b) or np.any(a != b):
+                assert (flags_g[r] | flags_o[r]) & binding.TIE
+                total_mis += 1
+    assert total_mis <= 1
+    # properties that hold at any size: forward_project(1) = L_i = N_i * l_i; sum of counts = sum of N
+    row_ptr, _, ell, flags = ctx.paths_decode(paths, 0, 200_000)
+    N = torch.diff(row_ptr).to(torch.float64)
+    ones = torch.ones(cfg.n, dtype=torch.float32, device="cuda")
+    L = ctx.forward_project(paths, ones)[:200_000].to(torch.float64)
+    assert torch.allclose(L, N * ell.to(torch.float64), rtol=1e-5)
+    counts = ctx.column_counts(paths, 0, m)
+    assert int(counts.to(torch.int64).sum().item()) == paths.total_visits
+    # two blocks of the configured solve (B = 200 k) against the oracle on the same histories
+    sub_m = min(m, 400_000)
+    if os.environ.get("PCT_TEST_SKIP_BLOCKS", "0") != "1":
+        sub = {k: v[:sub_m].contiguous() for k, v in pr.items()}
+        ctx2, paths2 = gpu_paths(binding, cfg, sub, hull)
+        x_g = ctx2.solve(paths2, sub["wepl"], ones, 1, cfg.block, cfg.lam).cpu().numpy()
+        g, p, pa, P = oracle_setup(oracle, cfg, {k: v.cpu() for k, v in sub.items()}, hull.cpu())
+        x_o = P.solve(sub["wepl"].cpu().numpy(), np.ones(cfg.n, np.float32), 1, cfg.block, cfg.lam)
+        assert np.linalg.norm(x_g - x_o) / np.linalg.norm(x_o) <= REL_L2_TOL
+        assert np.max(np.abs(x_g - x_o)) <= MAX_ABS_TOL
