@@ -105,7 +105,8 @@ int pct_create(const pct_geometry* geom, const pct_mlp_params* params, int devic
     c.sx = 1; c.sy = geom->nx; c.sz = geom->nx * geom->ny;
     c.h = geom->h_mm; c.inv_h = 1.0 / geom->h_mm;
     const int nn[3] = {geom->nx, geom->ny, geom->nz};
-    for (int a = 0; a < 3; ++a) { c.lo[a] = geom->origin_mm[a]; c.hi[a] = geom->origin_mm[a] + nn[a] * geom->h_mm; }
+    // hi must be bit-identical to the kernels' face_coord(a, n) = fma(n, h, lo): the exit point is snapped to it
+    for (int a = 0; a < 3; ++a) { c.lo[a] = geom->origin_mm[a]; c.hi[a] = std::fma((double)nn[a], geom->h_mm, geom->origin_mm[a]); }
     for (int i = 0; i < 6; ++i) {
         c.a[i] = params->poly[i];
         // int_0^W (W-w)^q w^i dw = W^(i+q+1) q! i! / (i+q+1)!
@@ -263,7 +264,7 @@ int pct_paths_decode(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, i
 
 int pct_forward_project(pct_ctx* ctx, const pct_paths* P, const float* x, float* b_out, void* stream) {
     if (!ctx) return PCT_E_INVALID_ARG;
-    if (!P || !x || !b_out || P->n_vox != ctx->n_vox) return set_error(ctx, PCT_E_INVALID_ARG, "bad forward_project arguments");
+    if (!P || !x || (!b_out && P->m > 0) || P->n_vox != ctx->n_vox) return set_error(ctx, PCT_E_INVALID_ARG, "bad forward_project arguments");
     DeviceGuard guard(ctx->device);
     return launch_forward_project(ctx, P, x, b_out, (cudaStream_t)stream);
 }
@@ -279,7 +280,7 @@ int pct_column_counts(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, 
 int pct_solve(pct_ctx* ctx, const pct_paths* P, const float* b, const float* x0, int iters, int64_t block_size, float lambda,
               float* x_out, void* stream) {
     if (!ctx) return PCT_E_INVALID_ARG;
-    if (!P || !b || !x0 || !x_out || iters < 0 || block_size < 1 || P->n_vox != ctx->n_vox || !std::isfinite(lambda))
+    if (!P || (!b && P->m > 0) || !x0 || !x_out || iters < 0 || block_size < 1 || P->n_vox != ctx->n_vox || !std::isfinite(lambda))
         return set_error(ctx, PCT_E_INVALID_ARG, "bad solve arguments");
     DeviceGuard guard(ctx->device);
     cudaStream_t st = (cudaStream_t)stream;
