@@ -134,6 +134,18 @@ typedef struct {
 int pct_profile_enable(pct_ctx* ctx, int on);
 int pct_profile_read(pct_ctx* ctx, pct_profile* out);
 
+/* Roofline denominators MEASURED_PEAKS.json lacks, measured on ctx's device with register /
+ * L2 / shared-memory resident microbenchmarks (best of three launches, CUDA events; ~0.3 s in total):
+ * plain FP64 FMA/s (K1), random 4-byte L2 gathers/s over a 64 MiB array, red.global.add.f32/s and .v2.f32/s
+ * (random and warp-contiguous addresses), shared-memory 32-bit atomic adds/s and loads/s (random slots).
+ * out: HOST.  Blocking; uses the legacy default stream. */
+typedef struct {
+    double fp64_fma_per_s, l2_gather_per_s, l2_red_f32_per_s, l2_red_v2_per_s, l2_red_v2_coalesced_per_s,
+        smem_atomic_per_s, smem_load_per_s;
+    int32_t num_sms;
+} pct_peaks;
+int pct_measure_peaks(pct_ctx* ctx, pct_peaks* out);
+
 #ifdef __cplusplus
 }
 #endif

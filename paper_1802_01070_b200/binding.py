@@ -20,7 +20,7 @@ REJECT_MASK = REJ_MISS | REJ_ORDER | REJ_DEPTH | REJ_LEFT_GRID | REJ_CAPACITY | 
 
 EXPORTS = ("pct_create", "pct_destroy", "pct_last_error", "pct_generate_mlp", "pct_paths_info", "pct_paths_free",
            "pct_paths_decode", "pct_forward_project", "pct_column_counts", "pct_solve", "pct_reconstruct_host",
-           "pct_launch_count", "pct_profile_enable", "pct_profile_read")
+           "pct_launch_count", "pct_profile_enable", "pct_profile_read", "pct_measure_peaks")
 
 
 class Geometry(C.Structure):
@@ -51,6 +51,12 @@ class ReconStats(C.Structure):
 
 class Profile(C.Structure):
     _fields_ = [("ms", C.c_double * 3), ("launches", C.c_int64 * 3)]
+
+
+class Peaks(C.Structure):
+    _fields_ = [(k, C.c_double) for k in ("fp64_fma_per_s", "l2_gather_per_s", "l2_red_f32_per_s", "l2_red_v2_per_s",
+                                          "l2_red_v2_coalesced_per_s", "smem_atomic_per_s", "smem_load_per_s")] + [
+        ("num_sms", C.c_int32)]
 
 
 PROTON_KEYS = ("phi", "t_in", "v_in", "dt_in", "dv_in", "t_out", "v_out", "dt_out", "dv_out")
@@ -90,6 +96,7 @@ def load_library(path: Optional[str] = None):
     L.pct_launch_count.restype = i64
     L.pct_profile_enable.argtypes = [vp, C.c_int]
     L.pct_profile_read.argtypes = [vp, C.POINTER(Profile)]
+    L.pct_measure_peaks.argtypes = [vp, C.POINTER(Peaks)]
     if path == _build.LIB:
         _lib = L
     return L
@@ -185,6 +192,11 @@ class Context:
         pr = Profile()
         self._check(self._L.pct_profile_read(self._h, C.byref(pr)))
         return {k: (pr.ms[i], pr.launches[i]) for i, k in enumerate(("mlp", "project_scatter", "update"))}
+
+    def measure_peaks(self) -> dict:
+        pk = Peaks()
+        self._check(self._L.pct_measure_peaks(self._h, C.byref(pk)))
+        return {k: getattr(pk, k) for k, _ in Peaks._fields_}
 
     # -- the C-ABI calls, same names --------------------------------------------------------------------------
     def generate_mlp(self, protons: Dict[str, torch.Tensor], u_in_mm: float, u_out_mm: float,
