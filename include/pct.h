@@ -123,13 +123,28 @@ int pct_reconstruct_host(pct_ctx* ctx, const pct_protons* protons, const uint8_t
 /* Number of kernel launches issued by this context so far (bench.py reports it as gpu_launches). */
 int64_t pct_launch_count(const pct_ctx* ctx);
 
-/* Per-kernel timing for the roofline report.  pct_profile_enable(ctx, 1) makes the launchers bracket every launch
- * of the three hot kernels with CUDA events on the launching stream; pct_profile_read synchronises the device,
- * ADDS the elapsed times since the last read to out (HOST) and clears the event list.  kind: 0 = MLP + walk (K1),
- * 1 = block project + scatter (K2), 2 = voxel update (K3). */
+/* How pct_solve runs a block's projection (A4-A6).  mode 0 (default) = automatic: blocks of at least
+ * `min_block` histories (<= 0: library default) use the solve plan -- the block's histories regrouped into spatially
+ * compact tubes whose x / {Delta, s} windows live in shared memory -- and smaller blocks the direct
+ * kernel (one warp per history, gathers and reductions in L2); mode 1 = direct kernel only; mode 2 = plan
+ * whenever it can be built.  The result is the same up to FP32 summation order (R18, R21). */
+int pct_solve_config(pct_ctx* ctx, int mode, int64_t min_block);
+
+/* Statistics of the solve plan cached in `paths` by the last pct_solve that used one (all zero if none). */
 typedef struct {
-    double ms[3];
-    int64_t launches[3];
+    int64_t block_size, n_blocks, n_groups, n_direct, plan_bytes;
+} pct_plan_stats;
+int pct_plan_info(const pct_paths* paths, pct_plan_stats* out /* HOST */);
+
+/* Per-kernel timing for the roofline report.  pct_profile_enable(ctx, 1) makes the launchers bracket every launch
+ * of the hot kernels with CUDA events on the launching stream; pct_profile_read synchronises the device,
+ * ADDS the elapsed times since the last read to out (HOST) and clears the event list.  kind: 0 = MLP + walk (K1),
+ * 1 = windowed block projection (K2w), 2 = voxel update (K3), 3 = direct block projection (K2d),
+ * 4 = solve-plan construction (sort, grouping, verification). */
+#define PCT_PROFILE_KINDS 5
+typedef struct {
+    double ms[PCT_PROFILE_KINDS];
+    int64_t launches[PCT_PROFILE_KINDS];
 } pct_profile;
 int pct_profile_enable(pct_ctx* ctx, int on);
 int pct_profile_read(pct_ctx* ctx, pct_profile* out);

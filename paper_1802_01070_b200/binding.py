@@ -20,7 +20,8 @@ REJECT_MASK = REJ_MISS | REJ_ORDER | REJ_DEPTH | REJ_LEFT_GRID | REJ_CAPACITY | 
 
 EXPORTS = ("pct_create", "pct_destroy", "pct_last_error", "pct_generate_mlp", "pct_paths_info", "pct_paths_free",
            "pct_paths_decode", "pct_forward_project", "pct_column_counts", "pct_solve", "pct_reconstruct_host",
-           "pct_launch_count", "pct_profile_enable", "pct_profile_read", "pct_measure_peaks")
+           "pct_launch_count", "pct_profile_enable", "pct_profile_read", "pct_measure_peaks", "pct_solve_config",
+           "pct_plan_info")
 
 
 class Geometry(C.Structure):
@@ -49,8 +50,15 @@ class ReconStats(C.Structure):
         (k, C.c_double) for k in ("ms_h2d", "ms_mlp", "ms_solve", "ms_d2h")]
 
 
+PROFILE_KINDS = ("mlp", "project_windowed", "update", "project_direct", "plan")
+
+
 class Profile(C.Structure):
-    _fields_ = [("ms", C.c_double * 3), ("launches", C.c_int64 * 3)]
+    _fields_ = [("ms", C.c_double * len(PROFILE_KINDS)), ("launches", C.c_int64 * len(PROFILE_KINDS))]
+
+
+class PlanStats(C.Structure):
+    _fields_ = [(k, C.c_int64) for k in ("block_size", "n_blocks", "n_groups", "n_direct", "plan_bytes")]
 
 
 class Peaks(C.Structure):
@@ -97,6 +105,8 @@ def load_library(path: Optional[str] = None):
     L.pct_profile_enable.argtypes = [vp, C.c_int]
     L.pct_profile_read.argtypes = [vp, C.POINTER(Profile)]
     L.pct_measure_peaks.argtypes = [vp, C.POINTER(Peaks)]
+    L.pct_solve_config.argtypes = [vp, C.c_int, i64]
+    L.pct_plan_info.argtypes = [vp, C.POINTER(PlanStats)]
     if path == _build.LIB:
         _lib = L
     return L
@@ -127,6 +137,12 @@ class Paths:
         ctx._check(ctx._L.pct_paths_info(handle, C.byref(st)))
         self.m, self.total_visits, self.n_rejected, self.n_ties = st.m, st.total_visits, st.n_rejected, st.n_ties
         self.code_bytes, self.header_bytes = st.code_bytes, st.header_bytes
+
+    def plan_info(self) -> dict:
+        """Statistics of the solve plan cached by the last pct_solve (zeros if it used the direct kernel)."""
+        st = PlanStats()
+        self.ctx._check(self.ctx._L.pct_plan_info(self._h, C.byref(st)))
+        return {k: getattr(st, k) for k, _ in PlanStats._fields_}
 
     def free(self):
         if self._h:
@@ -188,10 +204,14 @@ class Context:
         self._check(self._L.pct_profile_enable(self._h, 1 if on else 0))
 
     def profile_read(self) -> dict:
-        """{kind: (ms, launches)} for kind in mlp / project_scatter / update since the last read."""
+        """{kind: (ms, launches)} for kind in PROFILE_KINDS since the last read."""
         pr = Profile()
         self._check(self._L.pct_profile_read(self._h, C.byref(pr)))
-        return {k: (pr.ms[i], pr.launches[i]) for i, k in enumerate(("mlp", "project_scatter", "update"))}
+        return {k: (pr.ms[i], pr.launches[i]) for i, k in enumerate(PROFILE_KINDS)}
+
+    def solve_config(self, mode: int = 0, min_block: int = 0):
+        """pct_solve_config: 0 = automatic, 1 = direct kernel only, 2 = windowed plan whenever possible."""
+        self._check(self._L.pct_solve_config(self._h, int(mode), int(min_block)))
 
     def measure_peaks(self) -> dict:
         pk = Peaks()

@@ -130,8 +130,8 @@ struct CodeWriter {
 __global__ void __launch_bounds__(128)
 k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const uint8_t* __restrict__ hull, int64_t i_base,
            int count, int stage_stride, ulonglong2* __restrict__ stage, uint32_t* __restrict__ nchunks, uint32_t* __restrict__ Nout,
-           int32_t* __restrict__ start_out, float* __restrict__ ell_out, uint8_t* __restrict__ flags_out,
-           GenStats* __restrict__ stats) {
+           int32_t* __restrict__ start_out, int32_t* __restrict__ end_out, float* __restrict__ ell_out,
+           uint8_t* __restrict__ flags_out, GenStats* __restrict__ stats) {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     const bool active = p < count;
     unsigned flags = 0;
@@ -141,7 +141,7 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const uint8_t*
         const int64_t i = i_base + p;
         const double phi = pr.phi[i], t_in = pr.t_in[i], v_in = pr.v_in[i], dt_in = pr.dt_in[i], dv_in = pr.dv_in[i];
         const double t_out = pr.t_out[i], v_out = pr.v_out[i], dt_out = pr.dt_out[i], dv_out = pr.dv_out[i];
-        int32_t start_v = -1;
+        int32_t start_v = -1, end_v = -1;
         float ell = 0.f;
         do {
             if (!(isfinite(phi) && isfinite(t_in) && isfinite(v_in) && isfinite(dt_in) && isfinite(dv_in) &&
@@ -250,11 +250,13 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const uint8_t*
             if (tie) flags |= PCT_TIE;
             if (c[0] != h_out.c[0] || c[1] != h_out.c[1] || c[2] != h_out.c[2]) flags |= PCT_END_MISMATCH;   // R10
             ell = (float)(L / (double)N);                                                                    // R11
+            end_v = c[0] + g.nx * (c[1] + g.ny * c[2]);
         } while (false);
-        if (N == 0) { n_chunks = 0; start_v = -1; ell = 0.f; }
+        if (N == 0) { n_chunks = 0; start_v = -1; end_v = -1; ell = 0.f; }
         nchunks[p] = (uint32_t)n_chunks;
         Nout[i] = N;
         start_out[i] = start_v;
+        end_out[i] = end_v;
         ell_out[i] = ell;
         flags_out[i] = (uint8_t)flags;
     }
@@ -274,8 +276,8 @@ int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, in
     const int threads = 128;
     const int blocks = (count + threads - 1) / threads;
     ProfScope prof(ctx, 0, st);
-    k_mlp_walk<<<blocks, threads, 0, st>>>(ctx->cfg, pr, hull, i_base, count, stage_stride, stage, nchunks, P->N, P->start, P->ell,
-                                           P->flags, ctx->d_stats);
+    k_mlp_walk<<<blocks, threads, 0, st>>>(ctx->cfg, pr, hull, i_base, count, stage_stride, stage, nchunks, P->N, P->start, P->end,
+                                           P->ell, P->flags, ctx->d_stats);
     ++ctx->launches;
     PCT_CUDA(ctx, cudaGetLastError());
     return PCT_OK;

@@ -34,6 +34,8 @@ ProfScope::~ProfScope() {
     ctx->prof_events[kind]->push_back(e);
 }
 
+constexpr int64_t DEFAULT_MIN_PLAN_BLOCK = 32768;   // below this a block is too sparse for shared-memory windows
+
 static double factorial(int k) { double r = 1.0; for (int i = 2; i <= k; ++i) r *= i; return r; }
 
 struct DeviceGuard {
@@ -43,8 +45,9 @@ struct DeviceGuard {
 };
 
 static void free_paths_arrays(pct_paths* P) {
-    cudaFree(P->N); cudaFree(P->start); cudaFree(P->ell); cudaFree(P->flags); cudaFree(P->code_off); cudaFree(P->codes);
-    P->N = nullptr; P->start = nullptr; P->ell = nullptr; P->flags = nullptr; P->code_off = nullptr; P->codes = nullptr;
+    cudaFree(P->N); cudaFree(P->start); cudaFree(P->end); cudaFree(P->ell); cudaFree(P->flags); cudaFree(P->code_off); cudaFree(P->codes);
+    if (P->plan) { free_solve_plan(P->plan); P->plan = nullptr; }
+    P->N = nullptr; P->start = nullptr; P->end = nullptr; P->ell = nullptr; P->flags = nullptr; P->code_off = nullptr; P->codes = nullptr;
 }
 
 static int ensure_ds(pct_ctx* ctx, cudaStream_t st) {
@@ -100,6 +103,8 @@ int pct_create(const pct_geometry* geom, const pct_mlp_params* params, int devic
     ctx->params = *params;
     ctx->device = device;
     ctx->n_vox = (int64_t)geom->nx * geom->ny * geom->nz;
+    ctx->solve_mode = 0;
+    ctx->solve_min_block = DEFAULT_MIN_PLAN_BLOCK;
     DevCfg& c = ctx->cfg;
     c.nx = geom->nx; c.ny = geom->ny; c.nz = geom->nz;
     c.sx = 1; c.sy = geom->nx; c.sz = geom->nx * geom->ny;
@@ -145,7 +150,7 @@ int pct_profile_read(pct_ctx* ctx, pct_profile* out) {
     if (!ctx || !out) return PCT_E_INVALID_ARG;
     DeviceGuard guard(ctx->device);
     PCT_CUDA(ctx, cudaDeviceSynchronize());
-    for (int k = 0; k < 3; ++k) {
+    for (int k = 0; k < PCT_PROFILE_KINDS; ++k) {
         std::vector<cudaEvent_t>& v = *ctx->prof_events[k];
         for (size_t i = 0; i + 1 < v.size(); i += 2) {
             float ms = 0.f;
@@ -187,6 +192,7 @@ int pct_generate_mlp(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hull, v
         return fail(set_error(ctx, e__ == cudaErrorMemoryAllocation ? PCT_E_OOM : PCT_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e__))); } } while (0)
     GEN_CUDA(cudaMalloc(&P->N, sizeof(uint32_t) * mm));
     GEN_CUDA(cudaMalloc(&P->start, sizeof(int32_t) * mm));
+    GEN_CUDA(cudaMalloc(&P->end, sizeof(int32_t) * mm));
     GEN_CUDA(cudaMalloc(&P->ell, sizeof(float) * mm));
     GEN_CUDA(cudaMalloc(&P->flags, sizeof(uint8_t) * mm));
     GEN_CUDA(cudaMalloc(&P->code_off, sizeof(uint64_t) * mm));
@@ -224,11 +230,29 @@ int pct_generate_mlp(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hull, v
     return PCT_OK;
 }
 
+int pct_solve_config(pct_ctx* ctx, int mode, int64_t min_block) {
+    if (!ctx) return PCT_E_INVALID_ARG;
+    if (mode < 0 || mode > 2) return set_error(ctx, PCT_E_INVALID_ARG, "solve mode must be 0, 1 or 2");
+    ctx->solve_mode = mode;
+    ctx->solve_min_block = min_block > 0 ? min_block : DEFAULT_MIN_PLAN_BLOCK;
+    return PCT_OK;
+}
+
+int pct_plan_info(const pct_paths* P, pct_plan_stats* out) {
+    if (!P || !out) return PCT_E_INVALID_ARG;
+    std::memset(out, 0, sizeof(*out));
+    const SolvePlan* pl = P->plan;
+    if (!pl) return PCT_OK;
+    out->block_size = pl->block_size; out->n_blocks = pl->n_blocks; out->n_groups = pl->n_groups; out->n_direct = pl->n_direct;
+    out->plan_bytes = pl->cnt_bytes + P->m * 13 + (pl->n_groups + 1) * (int64_t)sizeof(PlanGroup) + pl->n_blocks * 4;
+    return PCT_OK;
+}
+
 int pct_paths_info(const pct_paths* P, pct_paths_stats* out) {
     if (!P || !out) return PCT_E_INVALID_ARG;
     out->m = P->m; out->total_visits = P->total_visits; out->n_rejected = P->n_rejected; out->n_ties = P->n_ties;
     out->code_bytes = P->chunks_used * (int64_t)sizeof(ulonglong2);
-    out->header_bytes = P->m * (int64_t)(sizeof(uint32_t) + sizeof(int32_t) + sizeof(float) + sizeof(uint8_t) + sizeof(uint64_t));
+    out->header_bytes = P->m * (int64_t)(sizeof(uint32_t) + 2 * sizeof(int32_t) + sizeof(float) + sizeof(uint8_t) + sizeof(uint64_t));
     return PCT_OK;
 }
 
@@ -287,10 +311,30 @@ int pct_solve(pct_ctx* ctx, const pct_paths* P, const float* b, const float* x0,
     int rc;
     if ((rc = ensure_ds(ctx, st)) != PCT_OK) return rc;
     if (x_out != x0) PCT_CUDA(ctx, cudaMemcpyAsync(x_out, x0, sizeof(float) * (size_t)ctx->n_vox, cudaMemcpyDeviceToDevice, st));
+    // the plan is built once per (paths, block_size) and cached in the paths object
+    const SolvePlan* plan = nullptr;
+    const int64_t n_blocks = P->m > 0 ? (P->m + block_size - 1) / block_size : 0;
+    const bool plan_possible = iters > 0 && P->m > 0 && P->m < 0xffffffffLL && n_blocks < (1LL << 24);
+    const bool want_plan = ctx->solve_mode == 2 || (ctx->solve_mode == 0 && (P->m < block_size ? P->m : block_size) >= ctx->solve_min_block);
+    if (plan_possible && want_plan) {
+        pct_paths* Pm = const_cast<pct_paths*>(P);
+        if (Pm->plan && Pm->plan->block_size != block_size) { free_solve_plan(Pm->plan); Pm->plan = nullptr; }
+        if (!Pm->plan) {
+            ProfScope prof(ctx, 4, st);
+            if ((rc = build_solve_plan(ctx, P, block_size, st, &Pm->plan)) != PCT_OK) return rc;
+        }
+        plan = Pm->plan;
+    }
     for (int it = 0; it < iters; ++it) {
-        for (int64_t i0 = 0; i0 < P->m; i0 += block_size) {
+        for (int64_t t = 0, i0 = 0; i0 < P->m; i0 += block_size, ++t) {
             const int64_t i1 = (P->m - i0) < block_size ? P->m : i0 + block_size;
-            if ((rc = launch_block_project_scatter(ctx, P, i0, i1, b, x_out, ctx->ds, st)) != PCT_OK) return rc;
+            if (plan) {
+                if ((rc = launch_block_windowed(ctx, P, plan, t, b, x_out, ctx->ds, st)) != PCT_OK) return rc;
+                const int64_t nd = plan->direct_count[(size_t)t];
+                if (nd > 0 && (rc = launch_block_project_scatter(ctx, P, i0, i0 + nd, plan->direct_list, b, x_out, ctx->ds, st)) != PCT_OK) return rc;
+            } else {
+                if ((rc = launch_block_project_scatter(ctx, P, i0, i1, nullptr, b, x_out, ctx->ds, st)) != PCT_OK) return rc;
+            }
             if ((rc = launch_block_update(ctx, x_out, ctx->ds, lambda, st)) != PCT_OK) return rc;
         }
     }

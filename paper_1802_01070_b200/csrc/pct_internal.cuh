@@ -38,6 +38,53 @@ struct ProtonPtrs {
 
 struct GenStats { unsigned long long total_visits, n_rejected, n_ties; };
 
+// ---- solve plan: a block's histories regrouped into spatially compact tubes ----------------------
+// A group = up to GROUP histories of one block that travel the same way (class = major axis and direction) and lie
+// next to each other.  Row r of a group is the grid plane  major index = m_first + dir*r ; in that row the group's
+// window covers WIN_N voxels of the minor in-plane axis from nbase(r) and WIN_Z slices from zbase(r), where the bases
+// drift linearly with r (16.16 fixed point).  Window slots are addressed circularly (coordinate mod window size), so a
+// history walking its codes needs no knowledge of the bases.  SLAB rows are resident in shared memory at a time.
+constexpr int WIN_N = 32, WIN_Z = 16, SLAB = 16;
+constexpr int WIN_SLOTS = WIN_N * WIN_Z * SLAB;            // 8192
+constexpr int GROUP = 1024;                                // histories per group = threads per CTA
+constexpr int MAX_ROW_VISITS = 6;                          // verified per history and row; bounds the fixed-point sums
+constexpr int ZROW = 4;                                    // sort rows: slices per z-row of the reference plane
+
+struct PlanGroup {
+    uint32_t start;      // first position in perm
+    uint32_t size;       // histories in the group (<= GROUP)
+    int32_t cls;         // travel code of the group: 0:+x 1:-x 2:+y 3:-y
+    int32_t nslab;       // slabs of SLAB rows
+    int32_t m_first;     // major-axis index of row 0
+    int32_t nb0, zb0;    // window base at row 0 (minor in-plane axis, z), 16.16 fixed point
+    int32_t sn, sz;      // base drift per row, 16.16 fixed point
+    int32_t pad_;
+    uint64_t cnt_off;    // first byte of this group's visits-per-slab table: cnt[cnt_off + slab*GROUP + thread]
+};
+
+__host__ __device__ __forceinline__ int plan_nbase(const PlanGroup& g, int r) { return (int)(((long long)g.nb0 + (long long)r * g.sn) >> 16); }
+__host__ __device__ __forceinline__ int plan_zbase(const PlanGroup& g, int r) { return (int)(((long long)g.zb0 + (long long)r * g.sz) >> 16); }
+
+// Packed window coordinate of a visit = byte offset of its 4-byte slot: (n mod 32) << 2 | (row mod 16) << 7 |
+// (z mod 16) << 11.  The shared-memory address XORs the row into the n field (bank swizzle, see k_block_windowed).
+__host__ __device__ __forceinline__ unsigned win_pack(int n, int r, int z) {
+    return ((unsigned)(n & (WIN_N - 1)) << 2) | ((unsigned)(r & (SLAB - 1)) << 7) | ((unsigned)(z & (WIN_Z - 1)) << 11);
+}
+__host__ __device__ __forceinline__ unsigned win_addr(unsigned p) { return p ^ ((p >> 5) & 0x3Cu); }
+
+struct SolvePlan {
+    int64_t block_size, n_blocks, n_groups, n_direct, cnt_bytes;
+    uint32_t* perm;          // sorted position -> history index (m)
+    uint32_t* p0;            // packed window coordinate of the first visit, per sorted position
+    uint8_t* pflag;          // per sorted position: 1 = windowed, 0 = not (rejected, or listed in direct_list)
+    uint8_t* cnt;            // visits per (group, slab, thread)
+    PlanGroup* groups;
+    uint32_t* direct_list;   // histories that take the direct path; block t owns [t*block_size, t*block_size + direct_count[t])
+    uint32_t* d_direct_count;
+    std::vector<int64_t> group_begin;    // per block, + sentinel (host)
+    std::vector<uint32_t> direct_count;  // per block (host)
+};
+
 }  // namespace pct
 
 struct pct_ctx {
@@ -50,6 +97,8 @@ struct pct_ctx {
     int64_t launches;
     char err[512];
     // scratch owned by the context (grown on demand)
+    int solve_mode;      // 0 auto, 1 direct kernel only, 2 windowed plan whenever possible (pct_solve_config)
+    int64_t solve_min_block;  // auto: blocks smaller than this take the direct kernel
     float2* ds;          // {Delta_j, s_j} accumulator, n_vox
     int64_t ds_cap;
     void* scan_tmp;      // block sums for scans
@@ -58,7 +107,8 @@ struct pct_ctx {
     unsigned long long* d_total;
     // optional per-kernel event timing (pct_profile_enable)
     bool profiling;
-    std::vector<cudaEvent_t>* prof_events[3];   // start/stop pairs per kind
+    std::vector<cudaEvent_t>* prof_events[PCT_PROFILE_KINDS];   // start/stop pairs per kind
+    bool k2w_ready;      // dynamic shared memory attribute of k_block_windowed set on this device
 };
 
 struct pct_paths {
@@ -68,17 +118,19 @@ struct pct_paths {
     int32_t* start;      // start voxel
     float* ell;          // mean chord l_i (R11)
     uint8_t* flags;
+    int32_t* end;        // voxel the walk ended in (R10); used by the solve plan only
     uint64_t* code_off;  // first 16-byte chunk of the row in `codes`
     ulonglong2* codes;
     int64_t chunks_used, chunks_cap;
     int64_t total_visits, n_rejected, n_ties;
+    pct::SolvePlan* plan; // cached by pct_solve for (this, block_size); owned by the paths object
 };
 
 namespace pct {
 
 int set_error(pct_ctx* ctx, int code, const char* fmt, ...);
 
-// RAII bracket around one kernel launch when profiling is on (kind: 0 MLP, 1 project+scatter, 2 update)
+// RAII bracket around one kernel launch when profiling is on (kinds: pct.h, pct_profile)
 struct ProfScope {
     pct_ctx* ctx; int kind; cudaStream_t st; bool on;
     ProfScope(pct_ctx* c, int k, cudaStream_t s);
@@ -104,8 +156,12 @@ int launch_decode(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, cons
                   cudaStream_t st);
 int launch_forward_project(pct_ctx* ctx, const pct_paths* P, const float* x, float* b_out, cudaStream_t st);
 int launch_column_counts(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, uint32_t* counts, cudaStream_t st);
-int launch_block_project_scatter(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, const float* b,
-                                 const float* x, float2* ds, cudaStream_t st);
+int launch_block_project_scatter(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, const uint32_t* list,
+                                 const float* b, const float* x, float2* ds, cudaStream_t st);
+int launch_block_windowed(pct_ctx* ctx, const pct_paths* P, const SolvePlan* plan, int64_t block, const float* b,
+                          const float* x, float2* ds, cudaStream_t st);
+int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaStream_t st, SolvePlan** out);
+void free_solve_plan(SolvePlan* plan);
 int launch_block_update(pct_ctx* ctx, float* x, float2* ds, float lambda, cudaStream_t st);
 int launch_fill(pct_ctx* ctx, float* p, int64_t n, float value, cudaStream_t st);
 

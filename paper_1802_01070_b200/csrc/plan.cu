@@ -1,0 +1,334 @@
+// plan.cu -- the solve plan: regroups every block's histories into spatially compact "tubes" so that
+// the block projection (A5/A6, "the block size is the number of protons to be processed in parallel")
+// can gather x and accumulate {Delta, s} in shared memory instead of L2.
+//
+// Reading R18/R22: inside a block the update is simultaneous, so the order in which a block's histories are
+// processed is free; block membership (R13, consecutive input ranges) is never changed.
+//
+// Steps (all on the device, one host synchronisation at the end to read the per-block group ranges):
+//   1. k_plan_keys      key_i = (block, travel class, z-row, lateral position at the grid's mid plane) from the start
+//                       and end voxel of the row; rejected histories get class 7 (sorted last in their block).
+//   2. radix sort       (key, i) pairs -- cub::DeviceRadixSort, the one library primitive used (a plain sort).
+//   3. k_plan_heads     group heads: every change of (block, class, z-row) and every GROUP-th sorted position.
+//   4. k_plan_params    per group: travel class, first row, window centre line (weighted mean of its members).
+//   5. k_plan_verify    WALKS THE CODES of every member and checks that each visit lies inside the group's window,
+//                       that the history never steps against the travel direction and never has more than
+//                       MAX_ROW_VISITS visits in one row; records visits per slab and the packed start coordinate.
+//                       A history that fails is appended to its block's direct list.
+// Correctness of the solver never depends on the sort or the centre-line fit: a history is either verified to stay
+// in its group's window or it takes the direct kernel.
+#include <cub/device/device_radix_sort.cuh>
+
+#include "pct_internal.cuh"
+
+namespace pct {
+
+constexpr int KEY_NREF_BITS = 24, KEY_ZROW_BITS = 13, KEY_CLS_BITS = 3;
+constexpr int KEY_RUN_SHIFT = KEY_NREF_BITS;                                   // bits above = (block, class, z-row)
+constexpr int KEY_BLOCK_SHIFT = KEY_NREF_BITS + KEY_ZROW_BITS + KEY_CLS_BITS;   // 40
+
+struct ChordInfo { int cls; int m_s, m_e, n_s, n_e, z_s, z_e; };
+
+// start/end voxel -> travel class and (major, minor, z) coordinates of both ends
+__device__ __forceinline__ ChordInfo chord_info(const DevCfg& g, int start, int end) {
+    ChordInfo c;
+    const int sx = start % g.nx, sy = (start / g.nx) % g.ny, sz = start / (g.nx * g.ny);
+    const int ex = end % g.nx, ey = (end / g.nx) % g.ny, ez = end / (g.nx * g.ny);
+    const int dx = ex - sx, dy = ey - sy;
+    if (abs(dx) >= abs(dy)) { c.cls = dx >= 0 ? 0 : 1; c.m_s = sx; c.m_e = ex; c.n_s = sy; c.n_e = ey; }
+    else { c.cls = dy >= 0 ? 2 : 3; c.m_s = sy; c.m_e = ey; c.n_s = sx; c.n_e = ex; }
+    c.z_s = sz; c.z_e = ez;
+    return c;
+}
+
+// lateral position of the chord where it crosses the mid plane of the major axis (extrapolated if it does not)
+__device__ __forceinline__ void chord_ref(const DevCfg& g, const ChordInfo& c, float& n_ref, float& z_ref, float& sl_n, float& sl_z) {
+    const int n_major = (c.cls < 2) ? g.nx : g.ny, n_minor = (c.cls < 2) ? g.ny : g.nx;
+    const float m_ref = 0.5f * (float)n_major;
+    const int dm = c.m_e - c.m_s;
+    sl_n = 0.f; sl_z = 0.f;
+    if (dm != 0) { sl_n = (float)(c.n_e - c.n_s) / (float)dm; sl_z = (float)(c.z_e - c.z_s) / (float)dm; }
+    const float mid_m = 0.5f * (float)(c.m_s + c.m_e);
+    n_ref = 0.5f * (float)(c.n_s + c.n_e) + sl_n * (m_ref - mid_m);
+    z_ref = 0.5f * (float)(c.z_s + c.z_e) + sl_z * (m_ref - mid_m);
+    n_ref = fminf(fmaxf(n_ref, -(float)n_minor), 2.f * (float)n_minor);
+    z_ref = fminf(fmaxf(z_ref, 0.f), (float)(g.nz - 1));
+}
+
+__global__ void __launch_bounds__(256)
+k_plan_keys(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, const int32_t* __restrict__ start,
+            const int32_t* __restrict__ end, int64_t m, int64_t block_size, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= m) return;
+    const uint64_t t = (uint64_t)(i / block_size);
+    uint64_t key;
+    if (N[i] == 0) {
+        key = (t << KEY_BLOCK_SHIFT) | (7ull << (KEY_NREF_BITS + KEY_ZROW_BITS));
+    } else {
+        const ChordInfo c = chord_info(g, start[i], end[i]);
+        float n_ref, z_ref, sl_n, sl_z;
+        chord_ref(g, c, n_ref, z_ref, sl_n, sl_z);
+        const int n_minor = (c.cls < 2) ? g.ny : g.nx;
+        const uint64_t nq = (uint64_t)min((1 << KEY_NREF_BITS) - 1, max(0, (int)((n_ref + (float)n_minor) * 4.f)));
+        const uint64_t zr = (uint64_t)min((1 << KEY_ZROW_BITS) - 1, (int)z_ref / ZROW);
+        key = (t << KEY_BLOCK_SHIFT) | ((uint64_t)c.cls << (KEY_NREF_BITS + KEY_ZROW_BITS)) | (zr << KEY_NREF_BITS) | nq;
+    }
+    keys[i] = key;
+    vals[i] = (uint32_t)i;
+}
+
+__global__ void __launch_bounds__(256) k_plan_heads(const uint64_t* __restrict__ keys, int64_t m, uint32_t* __restrict__ head) {
+    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= m) return;
+    head[j] = (j % GROUP == 0 || (keys[j] >> KEY_RUN_SHIFT) != (keys[j - 1] >> KEY_RUN_SHIFT)) ? 1u : 0u;
+}
+
+// heads write their group's start; the first head of every block writes group_begin[block]
+__global__ void __launch_bounds__(256)
+k_plan_starts(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ head, const uint64_t* __restrict__ gid, int64_t m,
+              PlanGroup* __restrict__ groups, int64_t* __restrict__ group_begin) {
+    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= m || !head[j]) return;
+    const uint64_t g = gid[j];
+    groups[g].start = (uint32_t)j;
+    groups[g].cls = (int)((keys[j] >> (KEY_NREF_BITS + KEY_ZROW_BITS)) & 7ull);
+    const uint64_t t = keys[j] >> KEY_BLOCK_SHIFT;
+    if (j == 0 || (keys[j - 1] >> KEY_BLOCK_SHIFT) != t) group_begin[t] = (int64_t)g;
+}
+
+template <typename T, typename Op>
+__device__ __forceinline__ T block_reduce_256(T v, Op op, T* scratch /* 8 */) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = op(v, __shfl_xor_sync(0xffffffffu, v, o));
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) scratch[threadIdx.x >> 5] = v;
+    __syncthreads();
+    T r = scratch[0];
+#pragma unroll
+    for (int k = 1; k < 8; ++k) r = op(r, scratch[k]);
+    return r;
+}
+
+// one CTA of 256 threads per group: first row, number of slabs, window centre line
+__global__ void __launch_bounds__(256)
+k_plan_params(const __grid_constant__ DevCfg g, const int32_t* __restrict__ start, const int32_t* __restrict__ end,
+              const uint32_t* __restrict__ perm, int64_t m, int64_t n_groups, PlanGroup* __restrict__ groups,
+              uint32_t* __restrict__ cnt_len) {
+    __shared__ float sf[8];
+    __shared__ int si[8];
+    const int64_t gi = blockIdx.x;
+    PlanGroup G = groups[gi];
+    const uint32_t size = (uint32_t)(((gi + 1 < n_groups) ? (int64_t)groups[gi + 1].start : m) - (int64_t)G.start);
+    if (G.cls == 7) {
+        if (threadIdx.x == 0) { G.size = size; G.nslab = 0; G.m_first = 0; G.nb0 = G.zb0 = G.sn = G.sz = 0; G.pad_ = 0; groups[gi] = G; cnt_len[gi] = 0; }
+        return;
+    }
+    const int dir = (G.cls & 1) ? -1 : 1;
+    float w_sum = 0.f, wn = 0.f, wz = 0.f, wsn = 0.f, wsz = 0.f;
+    int r_lo = INT_MAX, r_hi = INT_MIN;      // dir * m of starts / ends
+    for (uint32_t j = threadIdx.x; j < size; j += 256) {
+        const uint32_t i = perm[G.start + j];
+        const ChordInfo c = chord_info(g, start[i], end[i]);
+        float n_ref, z_ref, sl_n, sl_z;
+        chord_ref(g, c, n_ref, z_ref, sl_n, sl_z);
+        const float w = (float)abs(c.m_e - c.m_s) + 0.25f;
+        w_sum += w; wn += w * n_ref; wz += w * z_ref; wsn += w * sl_n; wsz += w * sl_z;
+        r_lo = min(r_lo, dir * c.m_s);
+        r_hi = max(r_hi, dir * c.m_e);
+    }
+    auto fadd = [](float a, float b) { return a + b; };
+    w_sum = block_reduce_256(w_sum, fadd, sf);
+    wn = block_reduce_256(wn, fadd, sf);
+    wz = block_reduce_256(wz, fadd, sf);
+    wsn = block_reduce_256(wsn, fadd, sf);
+    wsz = block_reduce_256(wsz, fadd, sf);
+    r_lo = block_reduce_256(r_lo, [](int a, int b) { return min(a, b); }, si);
+    r_hi = block_reduce_256(r_hi, [](int a, int b) { return max(a, b); }, si);
+    if (threadIdx.x != 0) return;
+    const int n_major = (G.cls < 2) ? g.nx : g.ny;
+    const float m_ref = 0.5f * (float)n_major;
+    const float n_c = wn / w_sum, z_c = wz / w_sum, s_n = wsn / w_sum, s_z = wsz / w_sum;
+    const int m_first = dir * r_lo;
+    // centre of the tube in row r (major index m_first + dir r): n_c + s_n (m - m_ref); window = 32 (16) voxels around it
+    const double n0 = (double)n_c + (double)s_n * ((double)m_first - (double)m_ref) - 0.5 * (WIN_N - 1);
+    const double z0 = (double)z_c + (double)s_z * ((double)m_first - (double)m_ref) - 0.5 * (WIN_Z - 1);
+    G.size = size;
+    G.m_first = m_first;
+    G.nslab = (r_hi - r_lo) / SLAB + 1;
+    G.nb0 = (int)llrint(fmin(fmax(n0 + 0.5, -16000.0), 16000.0) * 65536.0);
+    G.zb0 = (int)llrint(fmin(fmax(z0 + 0.5, -16000.0), 16000.0) * 65536.0);
+    G.sn = (int)llrint((double)s_n * dir * 65536.0);
+    G.sz = (int)llrint((double)s_z * dir * 65536.0);
+    G.pad_ = 0;
+    groups[gi] = G;
+    cnt_len[gi] = (uint32_t)G.nslab * GROUP;
+}
+
+__global__ void k_plan_cnt_off(const uint64_t* __restrict__ off, int64_t n_groups, PlanGroup* __restrict__ groups) {
+    const int64_t gi = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gi < n_groups) groups[gi].cnt_off = off[gi];
+}
+
+// one CTA per group, one thread per member: walk the codes, verify the window, record visits per slab
+__global__ void __launch_bounds__(GROUP)
+k_plan_verify(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, const int32_t* __restrict__ start,
+              const uint64_t* __restrict__ code_off, const ulonglong2* __restrict__ codes, const uint32_t* __restrict__ perm,
+              const PlanGroup* __restrict__ groups, int64_t block_size, uint32_t* __restrict__ p0_out,
+              uint8_t* __restrict__ pflag, uint8_t* __restrict__ cnt, uint32_t* __restrict__ direct_list,
+              uint32_t* __restrict__ direct_count) {
+    const PlanGroup G = groups[blockIdx.x];
+    const uint32_t j = threadIdx.x;
+    if (j >= G.size) return;
+    const uint32_t pos = G.start + j;
+    if (G.cls == 7) { pflag[pos] = 0; return; }
+    const uint32_t i = perm[pos];
+    const uint32_t n_vis = N[i];
+    const int sv = start[i];
+    const int vx = sv % g.nx, vy = (sv / g.nx) % g.ny;
+    int z = sv / (g.nx * g.ny);
+    int mj = (G.cls < 2) ? vx : vy, n = (G.cls < 2) ? vy : vx;
+    const int dir = (G.cls & 1) ? -1 : 1;
+    const int n_plus = (G.cls < 2) ? 2 : 0;             // code of a +1 step along the minor in-plane axis
+    int r = (mj - G.m_first) * dir;
+    const int r_end = G.nslab * SLAB;
+    bool ok = r >= 0 && r < r_end;
+    uint8_t* my_cnt = cnt + G.cnt_off + j;
+    const unsigned long long* cp = reinterpret_cast<const unsigned long long*>(codes + code_off[i]);
+    unsigned long long w = 0;
+    int nrem = 0, row_cnt = 0, slab_cnt = 0, cur_slab = ok ? r / SLAB : 0;
+    int nb = ok ? plan_nbase(G, r) : 0, zb = ok ? plan_zbase(G, r) : 0;
+    const uint32_t p0 = win_pack(n, r, z);
+    for (uint32_t v = 0; v < n_vis && ok; ++v) {
+        if (v > 0) {
+            if (nrem == 0) { w = __ldg(cp++); nrem = CODES_PER_WORD; }
+            const int code = (int)(w & 7ull);
+            w >>= 3; --nrem;
+            if (code == G.cls) {
+                ++r; row_cnt = 0;
+                if (r >= r_end) { ok = false; break; }
+                nb = plan_nbase(G, r); zb = plan_zbase(G, r);
+                if ((r / SLAB) != cur_slab) { my_cnt[(size_t)cur_slab * GROUP] = (uint8_t)slab_cnt; cur_slab = r / SLAB; slab_cnt = 0; }
+            } else if (code == (G.cls ^ 1) || code >= 6) { ok = false; break; }
+            else if (code >= 4) z += (code & 1) ? -1 : 1;
+            else n += (code == n_plus) ? 1 : -1;
+        }
+        if ((unsigned)(n - nb) >= (unsigned)WIN_N || (unsigned)(z - zb) >= (unsigned)WIN_Z || ++row_cnt > MAX_ROW_VISITS) { ok = false; break; }
+        ++slab_cnt;
+    }
+    if (ok) {
+        my_cnt[(size_t)cur_slab * GROUP] = (uint8_t)slab_cnt;
+        p0_out[pos] = p0;
+        pflag[pos] = 1;
+    } else {
+        for (int s = 0; s < G.nslab; ++s) my_cnt[(size_t)s * GROUP] = 0;
+        pflag[pos] = 0;
+        const uint64_t t = (uint64_t)i / (uint64_t)block_size;
+        const uint32_t slot = atomicAdd(direct_count + t, 1u);
+        direct_list[t * (uint64_t)block_size + slot] = i;
+    }
+}
+
+void free_solve_plan(SolvePlan* plan) {
+    if (!plan) return;
+    cudaFree(plan->perm); cudaFree(plan->p0); cudaFree(plan->pflag); cudaFree(plan->cnt); cudaFree(plan->groups);
+    cudaFree(plan->direct_list); cudaFree(plan->d_direct_count);
+    delete plan;
+}
+
+int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaStream_t st, SolvePlan** out) {
+    *out = nullptr;
+    const int64_t m = P->m;
+    const int64_t n_blocks = (m + block_size - 1) / block_size;
+    if (m <= 0 || m >= 0xffffffffLL || n_blocks >= (1LL << 24)) return set_error(ctx, PCT_E_INVALID_ARG, "solve plan: size out of range");
+    SolvePlan* plan = new (std::nothrow) SolvePlan();
+    if (!plan) return set_error(ctx, PCT_E_OOM, "host allocation");
+    plan->block_size = block_size; plan->n_blocks = n_blocks; plan->n_groups = 0; plan->n_direct = 0; plan->cnt_bytes = 0;
+    plan->perm = nullptr; plan->p0 = nullptr; plan->pflag = nullptr; plan->cnt = nullptr; plan->groups = nullptr;
+    plan->direct_list = nullptr; plan->d_direct_count = nullptr;
+    uint64_t *keysA = nullptr, *keysB = nullptr, *cnt_off = nullptr;
+    uint32_t *valsA = nullptr, *valsB = nullptr, *cnt_len = nullptr;
+    void* tmp = nullptr;
+    int64_t* d_group_begin = nullptr;
+    auto fail = [&](int code) {
+        cudaFree(keysA); cudaFree(keysB); cudaFree(valsA); cudaFree(valsB); cudaFree(tmp); cudaFree(cnt_off); cudaFree(cnt_len);
+        cudaFree(d_group_begin);
+        free_solve_plan(plan);
+        return code;
+    };
+#define PLAN_CUDA(call)                                                                                         \
+    do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { cudaGetLastError();                               \
+        return fail(set_error(ctx, e__ == cudaErrorMemoryAllocation ? PCT_E_OOM : PCT_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e__))); } } while (0)
+    const size_t mm = (size_t)m;
+    PLAN_CUDA(cudaMalloc(&keysA, 8 * mm)); PLAN_CUDA(cudaMalloc(&keysB, 8 * mm));
+    PLAN_CUDA(cudaMalloc(&valsA, 4 * mm)); PLAN_CUDA(cudaMalloc(&valsB, 4 * mm));
+    const unsigned nb256 = (unsigned)((m + 255) / 256);
+    k_plan_keys<<<nb256, 256, 0, st>>>(ctx->cfg, P->N, P->start, P->end, m, block_size, keysA, valsA);
+    ++ctx->launches;
+    PLAN_CUDA(cudaGetLastError());
+    int block_bits = 1;
+    while ((1LL << block_bits) < n_blocks) ++block_bits;
+    cub::DoubleBuffer<uint64_t> dk(keysA, keysB);
+    cub::DoubleBuffer<uint32_t> dv(valsA, valsB);
+    size_t tmp_bytes = 0;
+    PLAN_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, dk, dv, m, 0, KEY_BLOCK_SHIFT + block_bits, st));
+    PLAN_CUDA(cudaMalloc(&tmp, tmp_bytes > 0 ? tmp_bytes : 16));
+    PLAN_CUDA(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, dk, dv, m, 0, KEY_BLOCK_SHIFT + block_bits, st));
+    const uint64_t* keys = dk.Current();
+    uint64_t* gid = dk.Alternate();            // reused: group id per sorted position
+    uint32_t* head = dv.Alternate();           // reused: head flags
+    plan->perm = dv.Current();
+    if (plan->perm == valsA) valsA = nullptr; else valsB = nullptr;   // ownership moved to the plan
+    k_plan_heads<<<nb256, 256, 0, st>>>(keys, m, head);
+    ++ctx->launches;
+    PLAN_CUDA(cudaGetLastError());
+    int rc;
+    if ((rc = launch_scan_u32(ctx, head, gid, m, 0, ctx->d_total, st)) != PCT_OK) return fail(rc);
+    unsigned long long n_groups = 0;
+    PLAN_CUDA(cudaMemcpyAsync(&n_groups, ctx->d_total, sizeof(n_groups), cudaMemcpyDeviceToHost, st));
+    PLAN_CUDA(cudaStreamSynchronize(st));
+    plan->n_groups = (int64_t)n_groups;
+    PLAN_CUDA(cudaMalloc(&plan->groups, sizeof(PlanGroup) * (size_t)(n_groups + 1)));
+    PLAN_CUDA(cudaMalloc(&d_group_begin, sizeof(int64_t) * (size_t)(n_blocks + 1)));
+    PLAN_CUDA(cudaMalloc(&cnt_len, sizeof(uint32_t) * (size_t)n_groups));
+    PLAN_CUDA(cudaMalloc(&cnt_off, sizeof(uint64_t) * (size_t)n_groups));
+    k_plan_starts<<<nb256, 256, 0, st>>>(keys, head, gid, m, plan->groups, d_group_begin);
+    k_plan_params<<<(unsigned)n_groups, 256, 0, st>>>(ctx->cfg, P->start, P->end, plan->perm, m, (int64_t)n_groups, plan->groups, cnt_len);
+    ctx->launches += 2;
+    PLAN_CUDA(cudaGetLastError());
+    if ((rc = launch_scan_u32(ctx, cnt_len, cnt_off, (int64_t)n_groups, 0, ctx->d_total, st)) != PCT_OK) return fail(rc);
+    unsigned long long cnt_bytes = 0;
+    PLAN_CUDA(cudaMemcpyAsync(&cnt_bytes, ctx->d_total, sizeof(cnt_bytes), cudaMemcpyDeviceToHost, st));
+    PLAN_CUDA(cudaStreamSynchronize(st));
+    plan->cnt_bytes = (int64_t)cnt_bytes;
+    k_plan_cnt_off<<<(unsigned)((n_groups + 255) / 256), 256, 0, st>>>(cnt_off, (int64_t)n_groups, plan->groups);
+    ++ctx->launches;
+    // the sort buffers are no longer needed once the group table is complete
+    PLAN_CUDA(cudaStreamSynchronize(st));
+    cudaFree(keysA); cudaFree(keysB); cudaFree(valsA); cudaFree(valsB); cudaFree(tmp);
+    keysA = keysB = nullptr; valsA = valsB = nullptr; tmp = nullptr;
+    PLAN_CUDA(cudaMalloc(&plan->cnt, cnt_bytes > 0 ? (size_t)cnt_bytes : 16));
+    PLAN_CUDA(cudaMemsetAsync(plan->cnt, 0, cnt_bytes > 0 ? (size_t)cnt_bytes : 16, st));
+    PLAN_CUDA(cudaMalloc(&plan->p0, 4 * mm));
+    PLAN_CUDA(cudaMalloc(&plan->pflag, mm));
+    PLAN_CUDA(cudaMalloc(&plan->direct_list, 4 * mm));
+    PLAN_CUDA(cudaMalloc(&plan->d_direct_count, sizeof(uint32_t) * (size_t)n_blocks));
+    PLAN_CUDA(cudaMemsetAsync(plan->d_direct_count, 0, sizeof(uint32_t) * (size_t)n_blocks, st));
+    k_plan_verify<<<(unsigned)n_groups, GROUP, 0, st>>>(ctx->cfg, P->N, P->start, P->code_off, P->codes, plan->perm, plan->groups,
+                                                       block_size, plan->p0, plan->pflag, plan->cnt, plan->direct_list,
+                                                       plan->d_direct_count);
+    ++ctx->launches;
+    PLAN_CUDA(cudaGetLastError());
+    plan->group_begin.resize((size_t)n_blocks + 1);
+    plan->direct_count.resize((size_t)n_blocks);
+    PLAN_CUDA(cudaMemcpyAsync(plan->group_begin.data(), d_group_begin, sizeof(int64_t) * (size_t)n_blocks, cudaMemcpyDeviceToHost, st));
+    PLAN_CUDA(cudaMemcpyAsync(plan->direct_count.data(), plan->d_direct_count, sizeof(uint32_t) * (size_t)n_blocks, cudaMemcpyDeviceToHost, st));
+    PLAN_CUDA(cudaStreamSynchronize(st));
+    plan->group_begin[(size_t)n_blocks] = (int64_t)n_groups;
+    for (uint32_t c : plan->direct_count) plan->n_direct += c;
+    cudaFree(cnt_off); cudaFree(cnt_len); cudaFree(d_group_begin);
+#undef PLAN_CUDA
+    *out = plan;
+    return PCT_OK;
+}
+
+}  // namespace pct

@@ -95,11 +95,13 @@ __device__ __forceinline__ void red_add_v2(float2* p, float a, float b) {
 __global__ void __launch_bounds__(PROJ_THREADS)
 k_block_project_scatter(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, const int32_t* __restrict__ start,
                         const float* __restrict__ ell, const uint64_t* __restrict__ code_off,
-                        const ulonglong2* __restrict__ codes, int64_t i0, int64_t i1, const float* __restrict__ b,
-                        const float* __restrict__ x, float2* __restrict__ ds) {
+                        const ulonglong2* __restrict__ codes, int64_t i0, int64_t i1, const uint32_t* __restrict__ list,
+                        const float* __restrict__ b, const float* __restrict__ x, float2* __restrict__ ds) {
+    // list == nullptr: histories [i0, i1); else the histories list[i0 .. i1) (a block's direct list, plan.cu)
     const int lane = threadIdx.x & 31;
     const int64_t warps = (int64_t)gridDim.x * PROJ_WARPS;
-    for (int64_t i = i0 + (int64_t)blockIdx.x * PROJ_WARPS + (threadIdx.x >> 5); i < i1; i += warps) {
+    for (int64_t k = i0 + (int64_t)blockIdx.x * PROJ_WARPS + (threadIdx.x >> 5); k < i1; k += warps) {
+        const int64_t i = list ? (int64_t)list[k] : k;
         const unsigned n = N[i];
         if (n == 0) continue;
         const uint64_t off = code_off[i];
@@ -155,12 +157,12 @@ int launch_column_counts(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i
     return PCT_OK;
 }
 
-int launch_block_project_scatter(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, const float* b, const float* x,
-                                 float2* ds, cudaStream_t st) {
+int launch_block_project_scatter(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, const uint32_t* list,
+                                 const float* b, const float* x, float2* ds, cudaStream_t st) {
     if (i1 <= i0) return PCT_OK;
-    ProfScope prof(ctx, 1, st);
+    ProfScope prof(ctx, 3, st);
     k_block_project_scatter<<<proj_grid(ctx, i1 - i0), PROJ_THREADS, 0, st>>>(ctx->cfg, P->N, P->start, P->ell,
-                                                                              P->code_off, P->codes, i0, i1, b, x, ds);
+                                                                              P->code_off, P->codes, i0, i1, list, b, x, ds);
     ++ctx->launches;
     PCT_CUDA(ctx, cudaGetLastError());
     return PCT_OK;

@@ -241,3 +241,83 @@ def test_head_full_size_sampled(binding, oracle):
         x_o = P.solve(sub["wepl"].cpu().numpy(), np.ones(cfg.n, np.float32), 1, cfg.block, cfg.lam)
         assert np.linalg.norm(x_g - x_o) / np.linalg.norm(x_o) <= REL_L2_TOL
         assert np.max(np.abs(x_g - x_o)) <= MAX_ABS_TOL
+
+
+# ---- the windowed solve plan: same image as the oracle whichever path a history takes ----------------
+@pytest.mark.parametrize("B,iters", [(5000, 3), (1234, 2), (50000, 2)])
+def test_windowed_plan_tiny(binding, oracle, B, iters):
+    """Config 0 with the plan forced on (mode 2): every block regrouped into tubes, shared-memory windows, fixed-point
+    Delta (R21).  Must match the oracle within the north_star tolerance and the direct kernel (mode 1) closely."""
+    cfg = synth.scaled(synth.CONFIGS["tiny"], 20000)
+    x_true, hull, shadow = synth.make_phantom(cfg)
+    pr = synth.generate_protons(cfg, x_true, shadow)
+    g, p, pa, P = oracle_setup(oracle, cfg, pr, hull)
+    ctx, paths = gpu_paths(binding, cfg, pr, hull)
+    b = pr["wepl"].cuda()
+    x0 = torch.ones(cfg.n, dtype=torch.float32, device="cuda")
+    ctx.solve_config(2)
+    x_w = ctx.solve(paths, b, x0, iters, B, 0.1).cpu().numpy()
+    info = paths.plan_info()
+    assert info["block_size"] == B and info["n_groups"] >= info["n_blocks"] == -(-cfg.m // B)
+    assert info["n_direct"] <= 0.05 * cfg.m, info           # the 32 x 16 window covers this whole grid
+    ctx.solve_config(1)
+    x_d = ctx.solve(paths, b, x0, iters, B, 0.1).cpu().numpy()
+    x_o = P.solve(pr["wepl"].numpy(), np.ones(cfg.n, np.float32), iters, B, 0.1)
+    for x_g in (x_w, x_d):
+        assert np.linalg.norm(x_g - x_o) / np.linalg.norm(x_o) <= REL_L2_TOL
+        assert np.max(np.abs(x_g - x_o)) <= MAX_ABS_TOL
+    assert np.max(np.abs(x_w - x_d)) <= 2e-4
+    assert np.abs(x_w - 1.0).max() > 0.02
+
+
+def test_windowed_plan_all_directions_and_fallback(binding, oracle):
+    """Random directions on a flat, wide grid (all four travel classes, windows that miss, steep and short rows):
+    whatever the plan decides per history, the image equals the oracle's."""
+    cfg = dataclasses.replace(synth.CONFIGS["tiny"], name="tiny-wide", nx=96, ny=80, nz=24, h=1.0, u_tracker=70.0, m=30000)
+    rays = synth.random_rays(cfg.m, cfg, seed=3)
+    rng = np.random.default_rng(4)
+    kick = torch.from_numpy(rng.normal(0, 0.05, cfg.m))
+    rays["dt_out"] = rays["dt_out"] + kick
+    rays["t_out"] = rays["t_out"] + 0.5 * kick * 2 * cfg.u_tracker
+    # half of the histories: a dense parallel bundle (the plan's good case), the rest stay random
+    half = cfg.m // 2
+    rays["phi"][:half] = 0.3
+    rays["dt_in"][:half] = 0.0; rays["dv_in"][:half] = 0.0
+    rays["t_out"][:half] = rays["t_in"][:half] + 0.5 * kick[:half] * 2 * cfg.u_tracker
+    rays["v_out"][:half] = rays["v_in"][:half]
+    rays["dt_out"][:half] = kick[:half]; rays["dv_out"][:half] = 0.0
+    wepl = torch.from_numpy(rng.uniform(20.0, 90.0, cfg.m).astype(np.float32))
+    g = oracle.make_geometry(**synth.geometry(cfg))
+    p = oracle.make_params(**synth.mlp_params(cfg))
+    pa = oracle.ProtonArrays({k: v.numpy() for k, v in rays.items()}, -cfg.u_tracker, cfg.u_tracker)
+    P = oracle.Paths(g, p, pa, None)
+    ctx = binding.Context(synth.geometry(cfg), synth.mlp_params(cfg), 0)
+    paths = ctx.generate_mlp({k: v.cuda() for k, v in rays.items()}, -cfg.u_tracker, cfg.u_tracker, None)
+    compare_lists(binding, oracle, ctx, paths, P)
+    ctx.solve_config(2)
+    x0 = torch.ones(cfg.n, dtype=torch.float32, device="cuda")
+    for B in (15000, 7001):
+        x_g = ctx.solve(paths, wepl.cuda(), x0, 2, B, 0.2).cpu().numpy()
+        info = paths.plan_info()
+        assert 0 < info["n_direct"] < cfg.m and info["n_groups"] > 4, info      # both paths are exercised
+        x_o = P.solve(wepl.numpy(), np.ones(cfg.n, np.float32), 2, B, 0.2)
+        assert np.linalg.norm(x_g - x_o) / np.linalg.norm(x_o) <= REL_L2_TOL
+        assert np.max(np.abs(x_g - x_o)) <= MAX_ABS_TOL
+
+
+def test_windowed_plan_head_blocks(binding, oracle):
+    """The first two blocks of config 1 exactly as bench.py runs them (B = 200 k, one gantry angle per block, automatic
+    mode): most histories must take the windowed kernel, and the image must match the oracle."""
+    cfg = synth.CONFIGS["head"]
+    m = 400_000
+    x_true, hull, shadow = synth.make_phantom(cfg, "cuda")
+    pr = synth.generate_protons(cfg, x_true, shadow, device="cuda", i0=0, i1=m)
+    ctx, paths = gpu_paths(binding, cfg, pr, hull)
+    x0 = torch.ones(cfg.n, dtype=torch.float32, device="cuda")
+    x_g = ctx.solve(paths, pr["wepl"], x0, 2, cfg.block, cfg.lam).cpu().numpy()
+    info = paths.plan_info()
+    assert info["n_blocks"] == 2 and info["n_direct"] < 0.25 * m, info
+    g, p, pa, P = oracle_setup(oracle, cfg, {k: v.cpu() for k, v in pr.items()}, hull.cpu())
+    x_o = P.solve(pr["wepl"].cpu().numpy(), np.ones(cfg.n, np.float32), 2, cfg.block, cfg.lam)
+    assert np.linalg.norm(x_g - x_o) / np.linalg.norm(x_o) <= REL_L2_TOL
+    assert np.max(np.abs(x_g - x_o)) <= MAX_ABS_TOL
