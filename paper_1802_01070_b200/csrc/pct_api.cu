@@ -244,7 +244,7 @@ int pct_plan_info(const pct_paths* P, pct_plan_stats* out) {
     const SolvePlan* pl = P->plan;
     if (!pl) return PCT_OK;
     out->block_size = pl->block_size; out->n_blocks = pl->n_blocks; out->n_groups = pl->n_groups; out->n_direct = pl->n_direct;
-    out->plan_bytes = pl->cnt_bytes + P->m * 13 + (pl->n_groups + 1) * (int64_t)sizeof(PlanGroup) + pl->n_blocks * 4;
+    out->plan_bytes = pl->cnt_bytes + 8 * pl->stream_words + P->m * 13 + (pl->n_groups + 1) * (int64_t)sizeof(PlanGroup) + pl->n_blocks * 4;
     return PCT_OK;
 }
 

@@ -58,9 +58,21 @@ struct PlanGroup {
     int32_t m_first;     // major-axis index of row 0
     int32_t nb0, zb0;    // window base at row 0 (minor in-plane axis, z), 16.16 fixed point
     int32_t sn, sz;      // base drift per row, 16.16 fixed point
-    int32_t pad_;
+    int32_t wps;         // 64-bit code words per (slab, thread) in the group's slab-aligned code stream
     uint64_t cnt_off;    // first byte of this group's visits-per-slab table: cnt[cnt_off + slab*GROUP + thread]
+    uint64_t stream_off; // first word of the group's code stream: stream[stream_off + (slab*wps + w)*GROUP + thread]
 };
+
+// thread -> rank of its history in the group's sorted order.  Transposed on purpose: the lanes of a warp take
+// histories spread over the whole cross-section of the tube, so that they rarely hit the same window slot at once.
+__host__ __device__ __forceinline__ int plan_rank(int tid, int size) {
+    const int warps = (size + 31) >> 5;
+    const int w = tid >> 5;
+    if (w >= warps) return -1;
+    const int rk = (tid & 31) * warps + w;
+    return rk < size ? rk : -1;
+}
+constexpr int PLAN_CODE_FIRST = 6;   // slab stream: "visit here, no step" (the first visit of a history); 7 = pad
 
 __host__ __device__ __forceinline__ int plan_nbase(const PlanGroup& g, int r) { return (int)(((long long)g.nb0 + (long long)r * g.sn) >> 16); }
 __host__ __device__ __forceinline__ int plan_zbase(const PlanGroup& g, int r) { return (int)(((long long)g.zb0 + (long long)r * g.sz) >> 16); }
@@ -78,6 +90,8 @@ struct SolvePlan {
     uint32_t* p0;            // packed window coordinate of the first visit, per sorted position
     uint8_t* pflag;          // per sorted position: 1 = windowed, 0 = not (rejected, or listed in direct_list)
     uint8_t* cnt;            // visits per (group, slab, thread)
+    unsigned long long* stream;   // slab-aligned copy of the windowed histories' codes (21 codes per word)
+    int64_t stream_words;
     PlanGroup* groups;
     uint32_t* direct_list;   // histories that take the direct path; block t owns [t*block_size, t*block_size + direct_count[t])
     uint32_t* d_direct_count;

@@ -120,7 +120,7 @@ k_plan_params(const __grid_constant__ DevCfg g, const int32_t* __restrict__ star
     PlanGroup G = groups[gi];
     const uint32_t size = (uint32_t)(((gi + 1 < n_groups) ? (int64_t)groups[gi + 1].start : m) - (int64_t)G.start);
     if (G.cls == 7) {
-        if (threadIdx.x == 0) { G.size = size; G.nslab = 0; G.m_first = 0; G.nb0 = G.zb0 = G.sn = G.sz = 0; G.pad_ = 0; groups[gi] = G; cnt_len[gi] = 0; }
+        if (threadIdx.x == 0) { G.size = size; G.nslab = 0; G.m_first = 0; G.nb0 = G.zb0 = G.sn = G.sz = 0; G.wps = 0; G.cnt_off = G.stream_off = 0; groups[gi] = G; cnt_len[gi] = 0; }
         return;
     }
     const int dir = (G.cls & 1) ? -1 : 1;
@@ -159,7 +159,8 @@ k_plan_params(const __grid_constant__ DevCfg g, const int32_t* __restrict__ star
     G.zb0 = (int)llrint(fmin(fmax(z0 + 0.5, -16000.0), 16000.0) * 65536.0);
     G.sn = (int)llrint((double)s_n * dir * 65536.0);
     G.sz = (int)llrint((double)s_z * dir * 65536.0);
-    G.pad_ = 0;
+    G.wps = 0;               // k_plan_verify collects the largest visits-per-slab here
+    G.cnt_off = G.stream_off = 0;
     groups[gi] = G;
     cnt_len[gi] = (uint32_t)G.nslab * GROUP;
 }
@@ -169,68 +170,144 @@ __global__ void k_plan_cnt_off(const uint64_t* __restrict__ off, int64_t n_group
     if (gi < n_groups) groups[gi].cnt_off = off[gi];
 }
 
+// Shared walk of k_plan_verify / k_plan_emit: thread tid of a group's CTA walks the codes of its history (plan_rank) and
+// reports every visit as f(row r, code that led to it or PLAN_CODE_FIRST, in-window?) until f returns false.
+struct MemberWalk {
+    uint32_t pos, i, n_vis;
+    int mj, n, z, r, dir, n_plus;
+    const unsigned long long* cp;
+};
+
+__device__ __forceinline__ bool member_init(const DevCfg& g, const PlanGroup& G, const uint32_t* __restrict__ N,
+                                            const int32_t* __restrict__ start, const uint64_t* __restrict__ code_off,
+                                            const ulonglong2* __restrict__ codes, const uint32_t* __restrict__ perm, MemberWalk& mw) {
+    const int rk = plan_rank((int)threadIdx.x, (int)G.size);
+    if (rk < 0) return false;
+    mw.pos = G.start + (uint32_t)rk;
+    mw.i = perm[mw.pos];
+    mw.n_vis = N[mw.i];
+    const int sv = start[mw.i];
+    const int vx = sv % g.nx, vy = (sv / g.nx) % g.ny;
+    mw.z = sv / (g.nx * g.ny);
+    mw.mj = (G.cls < 2) ? vx : vy;
+    mw.n = (G.cls < 2) ? vy : vx;
+    mw.dir = (G.cls & 1) ? -1 : 1;
+    mw.n_plus = (G.cls < 2) ? 2 : 0;             // code of a +1 step along the minor in-plane axis
+    mw.r = (mw.mj - G.m_first) * mw.dir;
+    mw.cp = reinterpret_cast<const unsigned long long*>(codes + code_off[mw.i]);
+    return true;
+}
+
 // one CTA per group, one thread per member: walk the codes, verify the window, record visits per slab
 __global__ void __launch_bounds__(GROUP)
 k_plan_verify(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, const int32_t* __restrict__ start,
               const uint64_t* __restrict__ code_off, const ulonglong2* __restrict__ codes, const uint32_t* __restrict__ perm,
-              const PlanGroup* __restrict__ groups, int64_t block_size, uint32_t* __restrict__ p0_out,
+              PlanGroup* __restrict__ groups, int64_t block_size, uint32_t* __restrict__ p0_out,
               uint8_t* __restrict__ pflag, uint8_t* __restrict__ cnt, uint32_t* __restrict__ direct_list,
               uint32_t* __restrict__ direct_count) {
     const PlanGroup G = groups[blockIdx.x];
-    const uint32_t j = threadIdx.x;
-    if (j >= G.size) return;
-    const uint32_t pos = G.start + j;
-    if (G.cls == 7) { pflag[pos] = 0; return; }
-    const uint32_t i = perm[pos];
-    const uint32_t n_vis = N[i];
-    const int sv = start[i];
-    const int vx = sv % g.nx, vy = (sv / g.nx) % g.ny;
-    int z = sv / (g.nx * g.ny);
-    int mj = (G.cls < 2) ? vx : vy, n = (G.cls < 2) ? vy : vx;
-    const int dir = (G.cls & 1) ? -1 : 1;
-    const int n_plus = (G.cls < 2) ? 2 : 0;             // code of a +1 step along the minor in-plane axis
-    int r = (mj - G.m_first) * dir;
+    MemberWalk mw;
+    if (G.cls == 7) {
+        if (threadIdx.x < G.size) pflag[G.start + threadIdx.x] = 0;
+        return;
+    }
+    if (!member_init(g, G, N, start, code_off, codes, perm, mw)) return;
+    int r = mw.r, n = mw.n, z = mw.z;
     const int r_end = G.nslab * SLAB;
     bool ok = r >= 0 && r < r_end;
-    uint8_t* my_cnt = cnt + G.cnt_off + j;
-    const unsigned long long* cp = reinterpret_cast<const unsigned long long*>(codes + code_off[i]);
+    uint8_t* my_cnt = cnt + G.cnt_off + threadIdx.x;
     unsigned long long w = 0;
-    int nrem = 0, row_cnt = 0, slab_cnt = 0, cur_slab = ok ? r / SLAB : 0;
+    int nrem = 0, row_cnt = 0, slab_cnt = 0, max_cnt = 0, cur_slab = ok ? r / SLAB : 0;
     int nb = ok ? plan_nbase(G, r) : 0, zb = ok ? plan_zbase(G, r) : 0;
     const uint32_t p0 = win_pack(n, r, z);
-    for (uint32_t v = 0; v < n_vis && ok; ++v) {
+    for (uint32_t v = 0; v < mw.n_vis && ok; ++v) {
         if (v > 0) {
-            if (nrem == 0) { w = __ldg(cp++); nrem = CODES_PER_WORD; }
+            if (nrem == 0) { w = __ldg(mw.cp++); nrem = CODES_PER_WORD; }
             const int code = (int)(w & 7ull);
             w >>= 3; --nrem;
             if (code == G.cls) {
                 ++r; row_cnt = 0;
                 if (r >= r_end) { ok = false; break; }
                 nb = plan_nbase(G, r); zb = plan_zbase(G, r);
-                if ((r / SLAB) != cur_slab) { my_cnt[(size_t)cur_slab * GROUP] = (uint8_t)slab_cnt; cur_slab = r / SLAB; slab_cnt = 0; }
+                if ((r / SLAB) != cur_slab) {
+                    my_cnt[(size_t)cur_slab * GROUP] = (uint8_t)slab_cnt;
+                    max_cnt = max(max_cnt, slab_cnt);
+                    cur_slab = r / SLAB; slab_cnt = 0;
+                }
             } else if (code == (G.cls ^ 1) || code >= 6) { ok = false; break; }
             else if (code >= 4) z += (code & 1) ? -1 : 1;
-            else n += (code == n_plus) ? 1 : -1;
+            else n += (code == mw.n_plus) ? 1 : -1;
         }
         if ((unsigned)(n - nb) >= (unsigned)WIN_N || (unsigned)(z - zb) >= (unsigned)WIN_Z || ++row_cnt > MAX_ROW_VISITS) { ok = false; break; }
         ++slab_cnt;
     }
     if (ok) {
         my_cnt[(size_t)cur_slab * GROUP] = (uint8_t)slab_cnt;
-        p0_out[pos] = p0;
-        pflag[pos] = 1;
+        max_cnt = max(max_cnt, slab_cnt);
+        p0_out[mw.pos] = p0;
+        pflag[mw.pos] = 1;
+        atomicMax(&groups[blockIdx.x].wps, max_cnt);      // visits; turned into words per slab by k_plan_stream_len
     } else {
         for (int s = 0; s < G.nslab; ++s) my_cnt[(size_t)s * GROUP] = 0;
-        pflag[pos] = 0;
-        const uint64_t t = (uint64_t)i / (uint64_t)block_size;
+        pflag[mw.pos] = 0;
+        const uint64_t t = (uint64_t)mw.i / (uint64_t)block_size;
         const uint32_t slot = atomicAdd(direct_count + t, 1u);
-        direct_list[t * (uint64_t)block_size + slot] = i;
+        direct_list[t * (uint64_t)block_size + slot] = mw.i;
     }
+}
+
+__global__ void k_plan_stream_len(int64_t n_groups, PlanGroup* __restrict__ groups, uint32_t* __restrict__ len) {
+    const int64_t gi = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gi >= n_groups) return;
+    const int max_cnt = groups[gi].wps;
+    const int wps = max_cnt > 0 ? (max_cnt + CODES_PER_WORD - 1) / CODES_PER_WORD : 0;
+    groups[gi].wps = wps;
+    len[gi] = (uint32_t)(groups[gi].nslab * wps * GROUP);
+}
+
+__global__ void k_plan_stream_off(const uint64_t* __restrict__ off, int64_t n_groups, PlanGroup* __restrict__ groups) {
+    const int64_t gi = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gi < n_groups) groups[gi].stream_off = off[gi];
+}
+
+// second walk of the verified members: re-emit the codes slab by slab, 21 per word, words [slab][w][thread] (the
+// stream is pre-filled with pad codes).  The first visit becomes PLAN_CODE_FIRST.
+__global__ void __launch_bounds__(GROUP)
+k_plan_emit(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, const int32_t* __restrict__ start,
+            const uint64_t* __restrict__ code_off, const ulonglong2* __restrict__ codes, const uint32_t* __restrict__ perm,
+            const PlanGroup* __restrict__ groups, const uint8_t* __restrict__ pflag, unsigned long long* __restrict__ stream) {
+    const PlanGroup G = groups[blockIdx.x];
+    MemberWalk mw;
+    if (G.cls == 7 || G.wps == 0) return;
+    if (!member_init(g, G, N, start, code_off, codes, perm, mw)) return;
+    if (!pflag[mw.pos]) return;
+    unsigned long long* out = stream + G.stream_off + threadIdx.x;
+    int r = mw.r, cur_slab = r / SLAB, k = 0;                 // k = codes emitted in the current slab
+    unsigned long long w = 0, acc = ~0ull;
+    int nrem = 0;
+    for (uint32_t v = 0; v < mw.n_vis; ++v) {
+        int code = PLAN_CODE_FIRST;
+        if (v > 0) {
+            if (nrem == 0) { w = __ldg(mw.cp++); nrem = CODES_PER_WORD; }
+            code = (int)(w & 7ull);
+            w >>= 3; --nrem;
+            if (code == G.cls) {
+                ++r;
+                if ((r / SLAB) != cur_slab) {
+                    if (k % CODES_PER_WORD != 0) out[((size_t)cur_slab * G.wps + k / CODES_PER_WORD) * GROUP] = acc;
+                    cur_slab = r / SLAB; k = 0; acc = ~0ull;
+                }
+            }
+        }
+        acc ^= (unsigned long long)(7 ^ code) << (3 * (k % CODES_PER_WORD));
+        if (++k % CODES_PER_WORD == 0) { out[((size_t)cur_slab * G.wps + k / CODES_PER_WORD - 1) * GROUP] = acc; acc = ~0ull; }
+    }
+    if (k % CODES_PER_WORD != 0) out[((size_t)cur_slab * G.wps + k / CODES_PER_WORD) * GROUP] = acc;
 }
 
 void free_solve_plan(SolvePlan* plan) {
     if (!plan) return;
-    cudaFree(plan->perm); cudaFree(plan->p0); cudaFree(plan->pflag); cudaFree(plan->cnt); cudaFree(plan->groups);
+    cudaFree(plan->perm); cudaFree(plan->p0); cudaFree(plan->pflag); cudaFree(plan->cnt); cudaFree(plan->groups); cudaFree(plan->stream);
     cudaFree(plan->direct_list); cudaFree(plan->d_direct_count);
     delete plan;
 }
@@ -244,7 +321,7 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     if (!plan) return set_error(ctx, PCT_E_OOM, "host allocation");
     plan->block_size = block_size; plan->n_blocks = n_blocks; plan->n_groups = 0; plan->n_direct = 0; plan->cnt_bytes = 0;
     plan->perm = nullptr; plan->p0 = nullptr; plan->pflag = nullptr; plan->cnt = nullptr; plan->groups = nullptr;
-    plan->direct_list = nullptr; plan->d_direct_count = nullptr;
+    plan->direct_list = nullptr; plan->d_direct_count = nullptr; plan->stream = nullptr; plan->stream_words = 0;
     uint64_t *keysA = nullptr, *keysB = nullptr, *cnt_off = nullptr;
     uint32_t *valsA = nullptr, *valsB = nullptr, *cnt_len = nullptr;
     void* tmp = nullptr;
@@ -317,6 +394,20 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
                                                        block_size, plan->p0, plan->pflag, plan->cnt, plan->direct_list,
                                                        plan->d_direct_count);
     ++ctx->launches;
+    PLAN_CUDA(cudaGetLastError());
+    // slab-aligned code stream of the verified members
+    k_plan_stream_len<<<(unsigned)((n_groups + 255) / 256), 256, 0, st>>>((int64_t)n_groups, plan->groups, cnt_len);
+    if ((rc = launch_scan_u32(ctx, cnt_len, cnt_off, (int64_t)n_groups, 0, ctx->d_total, st)) != PCT_OK) return fail(rc);
+    unsigned long long stream_words = 0;
+    PLAN_CUDA(cudaMemcpyAsync(&stream_words, ctx->d_total, sizeof(stream_words), cudaMemcpyDeviceToHost, st));
+    PLAN_CUDA(cudaStreamSynchronize(st));
+    plan->stream_words = (int64_t)stream_words;
+    PLAN_CUDA(cudaMalloc(&plan->stream, stream_words > 0 ? 8 * (size_t)stream_words : 16));
+    PLAN_CUDA(cudaMemsetAsync(plan->stream, 0xFF, stream_words > 0 ? 8 * (size_t)stream_words : 16, st));
+    k_plan_stream_off<<<(unsigned)((n_groups + 255) / 256), 256, 0, st>>>(cnt_off, (int64_t)n_groups, plan->groups);
+    k_plan_emit<<<(unsigned)n_groups, GROUP, 0, st>>>(ctx->cfg, P->N, P->start, P->code_off, P->codes, plan->perm, plan->groups,
+                                                     plan->pflag, plan->stream);
+    ctx->launches += 3;
     PLAN_CUDA(cudaGetLastError());
     plan->group_begin.resize((size_t)n_blocks + 1);
     plan->direct_count.resize((size_t)n_blocks);

@@ -27,38 +27,65 @@ struct WinGeom {
     bool x_major;
 };
 
-// slot k of thread tid in a slab -> (nq, ml, zq).  The lane index runs along the grid's x axis (the contiguous one):
-// the minor axis for y-major groups, the row (major) axis for x-major groups.
-__device__ __forceinline__ void slot_coords(const WinGeom& w, int lin, int& nq, int& ml, int& zq) {
-    if (w.x_major) { ml = lin & (SLAB - 1); nq = (lin >> 4) & (WIN_N - 1); }
-    else { nq = lin & (WIN_N - 1); ml = (lin >> 5) & (SLAB - 1); }
-    zq = lin >> 9;
-}
+// Staging and flushing: thread tid owns the window column (nq, ml) = f(tid) and the STAGE_Z slots zq = zq0 + 2k of
+// it.  The lane index runs along the grid's x axis (the contiguous one): the minor axis for y-major groups, the row
+// (major) axis for x-major groups, so that global loads and reductions coalesce.
+constexpr int STAGE_Z = WIN_SLOTS / GROUP;   // 8
 
-// voxel index of window slot (nq, ml, zq) of slab s, or -1 if it lies outside the grid
-__device__ __forceinline__ int slot_voxel(const PlanGroup& G, const WinGeom& w, int s, int nq, int ml, int zq) {
-    const int r = s * SLAB + ml;
-    const int nb = plan_nbase(G, r), zb = plan_zbase(G, r);
-    const int n = nb + ((nq - nb) & (WIN_N - 1));
-    const int z = zb + ((zq - zb) & (WIN_Z - 1));
-    const int mj = G.m_first + w.dir * r;
-    if ((unsigned)n >= (unsigned)w.dim_n || (unsigned)z >= (unsigned)w.dim_z || (unsigned)mj >= (unsigned)w.dim_m) return -1;
-    return mj * w.stride_m + n * w.stride_n + z * w.stride_z;
-}
-
-struct Walker {
-    const unsigned long long* cp;
-    unsigned long long w;
-    unsigned p;
-    int nrem;
-    // the first visit has no code: it is presented as one pad code (table entry 7 = no move)
-    __device__ __forceinline__ void init(const unsigned long long* codes, unsigned p0) { cp = codes; w = 7ull; nrem = 1; p = p0; }
+struct Column {
+    int base;        // voxel index of (row, n, z = 0), or -1 if the column lies outside the grid in n or in the row
+    int zb;          // first slice of the window in this row
 };
+
+__device__ __forceinline__ Column slab_column(const PlanGroup& G, const WinGeom& w, int s, int nq, int ml) {
+    const int r = s * SLAB + ml;
+    const int nb = plan_nbase(G, r);
+    const int n = nb + ((nq - nb) & (WIN_N - 1));
+    const int mj = G.m_first + w.dir * r;
+    Column c;
+    c.zb = plan_zbase(G, r);
+    c.base = ((unsigned)n < (unsigned)w.dim_n && (unsigned)mj < (unsigned)w.dim_m) ? mj * w.stride_m + n * w.stride_n : -1;
+    return c;
+}
+
+__device__ __forceinline__ float lds_f32(unsigned a) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a)); return v; }
+__device__ __forceinline__ int2 lds_v2(unsigned a) { int2 v; asm volatile("ld.shared.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a)); return v; }
+__device__ __forceinline__ void atoms_add(unsigned a, int v) { asm volatile("red.shared.add.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
+// 4-byte asynchronous global -> shared copy; valid == false writes a zero instead (src-size 0)
+__device__ __forceinline__ void cp_async_f32(unsigned dst, const float* src, bool valid) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(dst), "l"(src), "r"(valid ? 4 : 0) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+__device__ __forceinline__ void atoms_inc(unsigned a) { asm volatile("red.shared.add.u32 [%0], 1;" ::"r"(a) : "memory"); }
+
+// One slab of one thread's walk.  The slab's codes sit in G.wps words [slab][w][thread] (21 codes each, pad = 7); the
+// loop runs to the warp's largest visit count (rounded up to 3) so that all lanes stay converged.  visit(p) is called
+// on every real visit.  tbl_s = shared address of the step table; entry = {delta, field mask}; a zero mask marks a pad.
+// w0 = the slab's first word (loaded by the caller ahead of time).
+template <typename F>
+__device__ __forceinline__ void walk_slab(const unsigned long long* __restrict__ sp, unsigned long long w0, int cmax,
+                                          unsigned tbl_s, unsigned& p, F&& visit) {
+    for (int wi = 0; wi * CODES_PER_WORD < cmax; ++wi) {
+        const unsigned long long w = wi == 0 ? w0 : __ldg(sp + (size_t)wi * GROUP);
+        const int lim = cmax - wi * CODES_PER_WORD;          // warp-uniform
+#pragma unroll
+        for (int k3 = 0; k3 < CODES_PER_WORD; k3 += 3) {
+            if (k3 >= lim) break;
+#pragma unroll
+            for (int k = k3; k < k3 + 3; ++k) {
+                const unsigned code8 = (unsigned)(w >> (3 * k)) << 3 & 0x38u;
+                const int2 t = lds_v2(tbl_s + code8);
+                p = ((p + (unsigned)t.x) & (unsigned)t.y) | (p & ~(unsigned)t.y);
+                if (t.y != 0) visit(p);
+            }
+        }
+    }
+}
 
 __global__ void __launch_bounds__(GROUP, 2)
 k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, const float* __restrict__ ell,
-                 const uint64_t* __restrict__ code_off, const ulonglong2* __restrict__ codes, const uint32_t* __restrict__ perm,
-                 const uint32_t* __restrict__ p0, const uint8_t* __restrict__ pflag, const uint8_t* __restrict__ cnt,
+                 const uint32_t* __restrict__ perm, const uint32_t* __restrict__ p0, const uint8_t* __restrict__ pflag,
+                 const uint8_t* __restrict__ cnt, const unsigned long long* __restrict__ stream,
                  const PlanGroup* __restrict__ groups, int64_t group0, const float* __restrict__ b, const float* __restrict__ x,
                  float2* __restrict__ ds) {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -68,7 +95,7 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
     if (threadIdx.x == 0) Gs = groups[group0 + blockIdx.x];
     __syncthreads();
     const PlanGroup& G = Gs;
-    if (G.cls == 7 || G.nslab == 0) return;
+    if (G.cls == 7 || G.nslab == 0 || G.wps == 0) return;
     const int tid = threadIdx.x;
     WinGeom wg;
     wg.x_major = G.cls < 2;
@@ -76,9 +103,10 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
     wg.stride_m = wg.x_major ? 1 : g.nx; wg.stride_n = wg.x_major ? g.nx : 1; wg.stride_z = g.nx * g.ny;
     wg.dim_m = wg.x_major ? g.nx : g.ny; wg.dim_n = wg.x_major ? g.ny : g.nx; wg.dim_z = g.nz;
     if (tid < 8) {
-        // {delta, field mask} of a step: fields are n (bits 2-6), row (7-10), z (11-14); additions wrap inside a field
+        // {delta, field mask} of a step: fields are n (bits 2-6), row (7-10), z (11-14); additions wrap inside a field.
+        // PLAN_CODE_FIRST (6) and pad (7) do not move; a zero mask marks the pad (bit 31 of p is never set).
         const int n_plus = wg.x_major ? 2 : 0;
-        int2 e = make_int2(0, 0);
+        int2 e = make_int2(0, tid == PLAN_CODE_FIRST ? (int)0x80000000u : 0);
         if (tid == G.cls) e = make_int2(0x80, 0x780);
         else if (tid == n_plus) e = make_int2(0x4, 0x7C);
         else if (tid == n_plus + 1) e = make_int2(0x7C, 0x7C);
@@ -86,45 +114,53 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
         else if (tid == 5) e = make_int2(0x7800, 0x7800);
         tbl[tid] = e;
     }
-    const bool active = (uint32_t)tid < G.size && pflag[G.start + tid] != 0;
+    const int rk = plan_rank(tid, (int)G.size);
+    const bool active = rk >= 0 && pflag[G.start + rk] != 0;
     uint32_t i = 0, n_vis = 0;
     unsigned p_init = 0;
-    const unsigned long long* cp0 = nullptr;
     if (active) {
-        i = perm[G.start + tid];
+        i = perm[G.start + rk];
         n_vis = N[i];
-        p_init = p0[G.start + tid];
-        cp0 = reinterpret_cast<const unsigned long long*>(codes + code_off[i]);
+        p_init = p0[G.start + rk];
     }
+    const unsigned win_s = (unsigned)__cvta_generic_to_shared(smem), tbl_s = (unsigned)__cvta_generic_to_shared(tbl);
     const uint8_t* my_cnt = cnt + G.cnt_off + tid;
-    float* xs = reinterpret_cast<float*>(smem);
+    const unsigned long long* my_stream = stream + G.stream_off + tid;
+    // this thread's window column for staging / flushing
+    const int col_nq = wg.x_major ? (tid >> 4) & (WIN_N - 1) : tid & (WIN_N - 1);
+    const int col_ml = wg.x_major ? tid & (SLAB - 1) : (tid >> 5) & (SLAB - 1);
+    const int col_zq0 = tid >> 9;                                            // 0 or 1; slots zq0 + 2k
+    const unsigned col_addr = win_addr(win_pack(col_nq, col_ml, col_zq0));    // + k * 4096 bytes
 
     // ---- pass 1: S_i = sum of x over the visits ----------------------------------------------------------------------
-    Walker wk;
-    wk.init(cp0, p_init);
-    float S = 0.f;
-    for (int s = 0; s < G.nslab; ++s) {
-        __syncthreads();                          // previous slab's walkers are done (and tbl is visible)
+    // The x window is double buffered in the two halves of the shared window (pass 1 needs 32 KB of the 64 KB): slab
+    // s + 1 is staged with cp.async while slab s is walked, one barrier per slab.
+    auto stage = [&](int s) {
+        const Column col = slab_column(G, wg, s, col_nq, col_ml);
+        const unsigned dst = win_s + (unsigned)(s & 1) * (WIN_SLOTS * 4) + col_addr;
 #pragma unroll
-        for (int k = 0; k < WIN_SLOTS / GROUP; ++k) {
-            int nq, ml, zq;
-            slot_coords(wg, tid + k * GROUP, nq, ml, zq);
-            const int vox = slot_voxel(G, wg, s, nq, ml, zq);
-            xs[win_addr(win_pack(nq, ml, zq)) >> 2] = vox >= 0 ? __ldg(x + vox) : 0.f;
+        for (int k = 0; k < STAGE_Z; ++k) {
+            const int z = col.zb + ((col_zq0 + 2 * k - col.zb) & (WIN_Z - 1));
+            const bool valid = col.base >= 0 && (unsigned)z < (unsigned)wg.dim_z;
+            cp_async_f32(dst + k * 4096, x + (valid ? col.base + z * wg.stride_z : 0), valid);
         }
-        __syncthreads();
-        int c = active ? (int)my_cnt[(size_t)s * GROUP] : 0;
-        while (c > 0) {
-            if (wk.nrem == 0) { wk.w = __ldg(wk.cp++); wk.nrem = CODES_PER_WORD; }
-            int take = min(c, wk.nrem);
-            c -= take; wk.nrem -= take;
-            for (; take > 0; --take) {
-                const int2 t = tbl[(unsigned)wk.w & 7u];
-                wk.w >>= 3;
-                wk.p = ((wk.p + (unsigned)t.x) & (unsigned)t.y) | (wk.p & ~(unsigned)t.y);
-                S += *reinterpret_cast<const float*>(smem + win_addr(wk.p));
-            }
+    };
+    unsigned p = p_init;
+    float S = 0.f;
+    stage(0);
+    unsigned long long w_next = __ldg(my_stream);
+    for (int s = 0; s < G.nslab; ++s) {
+        const int c = (int)my_cnt[(size_t)s * GROUP];       // 0 for threads without a (windowed) history
+        const unsigned long long w0 = w_next;
+        cp_async_wait_all();
+        __syncthreads();                          // slab s is staged; slab s - 1 is walked (and tbl is visible)
+        if (s + 1 < G.nslab) {
+            stage(s + 1);
+            w_next = __ldg(my_stream + (size_t)(s + 1) * G.wps * GROUP);
         }
+        const int cmax = __reduce_max_sync(0xffffffffu, c);
+        const unsigned xs = win_s + (unsigned)(s & 1) * (WIN_SLOTS * 4);
+        walk_slab(my_stream + (size_t)s * G.wps * GROUP, w0, cmax, tbl_s, p, [&](unsigned q) { S += lds_f32(xs + win_addr(q)); });
     }
     // ---- c_i and the CTA's fixed-point scale (R17, R21) -----------------------------------------------------------------
     float ci = 0.f;
@@ -138,7 +174,6 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
     __syncthreads();                              // all walkers done with xs
     if ((tid & 31) == 0) red[tid >> 5] = mx;
     int* dl = reinterpret_cast<int*>(smem);
-    unsigned* sc = reinterpret_cast<unsigned*>(smem + WIN_SLOTS * 4);
 #pragma unroll
     for (int k = 0; k < 2 * WIN_SLOTS / GROUP; ++k) dl[tid + k * GROUP] = 0;      // clears Delta and s
     __syncthreads();
@@ -151,33 +186,31 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
     const int cfix = __float2int_rn(ci * scale);
 
     // ---- pass 2: {Delta, s} += {c_i, 1} on every visit; flush per slab -------------------------------------------------
-    wk.init(cp0, p_init);
+    p = p_init;
+    w_next = __ldg(my_stream);
     for (int s = 0; s < G.nslab; ++s) {
-        int c = active ? (int)my_cnt[(size_t)s * GROUP] : 0;
-        while (c > 0) {
-            if (wk.nrem == 0) { wk.w = __ldg(wk.cp++); wk.nrem = CODES_PER_WORD; }
-            int take = min(c, wk.nrem);
-            c -= take; wk.nrem -= take;
-            for (; take > 0; --take) {
-                const int2 t = tbl[(unsigned)wk.w & 7u];
-                wk.w >>= 3;
-                wk.p = ((wk.p + (unsigned)t.x) & (unsigned)t.y) | (wk.p & ~(unsigned)t.y);
-                const unsigned a = win_addr(wk.p);
-                atomicAdd(reinterpret_cast<int*>(smem + a), cfix);
-                atomicAdd(reinterpret_cast<unsigned*>(smem + WIN_SLOTS * 4 + a), 1u);
-            }
-        }
+        const int c = (int)my_cnt[(size_t)s * GROUP];
+        const int cmax = __reduce_max_sync(0xffffffffu, c);
+        const unsigned long long w0 = w_next;
+        if (s + 1 < G.nslab) w_next = __ldg(my_stream + (size_t)(s + 1) * G.wps * GROUP);
+        walk_slab(my_stream + (size_t)s * G.wps * GROUP, w0, cmax, tbl_s, p, [&](unsigned q) {
+            const unsigned a = win_s + win_addr(q);
+            atoms_add(a, cfix);
+            atoms_inc(a + WIN_SLOTS * 4);
+        });
         __syncthreads();
+        {
+            const Column col = slab_column(G, wg, s, col_nq, col_ml);
 #pragma unroll
-        for (int k = 0; k < WIN_SLOTS / GROUP; ++k) {
-            int nq, ml, zq;
-            slot_coords(wg, tid + k * GROUP, nq, ml, zq);
-            const unsigned a = win_addr(win_pack(nq, ml, zq)) >> 2;
-            const unsigned cs = sc[a];
-            if (cs != 0u) {
-                const int vox = slot_voxel(G, wg, s, nq, ml, zq);
-                red_add_v2_w(ds + vox, (float)dl[a] * inv_scale, (float)cs);
-                dl[a] = 0; sc[a] = 0u;
+            for (int k = 0; k < STAGE_Z; ++k) {
+                const unsigned a = col_addr + k * 4096;
+                const unsigned cs = *reinterpret_cast<unsigned*>(smem + WIN_SLOTS * 4 + a);
+                if (cs != 0u) {                       // a touched slot is a verified visit: it lies inside the grid
+                    const int z = col.zb + ((col_zq0 + 2 * k - col.zb) & (WIN_Z - 1));
+                    red_add_v2_w(ds + col.base + z * wg.stride_z, (float)*reinterpret_cast<int*>(smem + a) * inv_scale, (float)cs);
+                    *reinterpret_cast<int*>(smem + a) = 0;
+                    *reinterpret_cast<unsigned*>(smem + WIN_SLOTS * 4 + a) = 0u;
+                }
             }
         }
         __syncthreads();
@@ -193,8 +226,8 @@ int launch_block_windowed(pct_ctx* ctx, const pct_paths* P, const SolvePlan* pla
         ctx->k2w_ready = true;
     }
     ProfScope prof(ctx, 1, st);
-    k_block_windowed<<<(unsigned)(g1 - g0), GROUP, K2W_SMEM, st>>>(ctx->cfg, P->N, P->ell, P->code_off, P->codes, plan->perm,
-                                                                  plan->p0, plan->pflag, plan->cnt, plan->groups, g0, b, x, ds);
+    k_block_windowed<<<(unsigned)(g1 - g0), GROUP, K2W_SMEM, st>>>(ctx->cfg, P->N, P->ell, plan->perm, plan->p0, plan->pflag,
+                                                                  plan->cnt, plan->stream, plan->groups, g0, b, x, ds);
     ++ctx->launches;
     PCT_CUDA(ctx, cudaGetLastError());
     return PCT_OK;
