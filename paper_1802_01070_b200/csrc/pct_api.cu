@@ -53,10 +53,13 @@ static void free_paths_arrays(pct_paths* P) {
 static int ensure_ds(pct_ctx* ctx, cudaStream_t st) {
     if (ctx->ds_cap >= ctx->n_vox) return PCT_OK;
     if (ctx->ds) PCT_CUDA(ctx, cudaFree(ctx->ds));
-    ctx->ds = nullptr; ctx->ds_cap = 0;
+    if (ctx->dsum) PCT_CUDA(ctx, cudaFree(ctx->dsum));
+    ctx->ds = nullptr; ctx->dsum = nullptr; ctx->ds_cap = 0;
     PCT_CUDA(ctx, cudaMalloc(&ctx->ds, sizeof(float2) * (size_t)ctx->n_vox));
+    PCT_CUDA(ctx, cudaMalloc(&ctx->dsum, sizeof(float) * (size_t)ctx->n_vox));
     ctx->ds_cap = ctx->n_vox;
     PCT_CUDA(ctx, cudaMemsetAsync(ctx->ds, 0, sizeof(float2) * (size_t)ctx->n_vox, st));
+    PCT_CUDA(ctx, cudaMemsetAsync(ctx->dsum, 0, sizeof(float) * (size_t)ctx->n_vox, st));
     return PCT_OK;
 }
 
@@ -135,7 +138,7 @@ int pct_create(const pct_geometry* geom, const pct_mlp_params* params, int devic
 void pct_destroy(pct_ctx* ctx) {
     if (!ctx) return;
     DeviceGuard guard(ctx->device);
-    cudaFree(ctx->ds); cudaFree(ctx->scan_tmp); cudaFree(ctx->d_stats); cudaFree(ctx->d_total);
+    cudaFree(ctx->ds); cudaFree(ctx->dsum); cudaFree(ctx->scan_tmp); cudaFree(ctx->d_stats); cudaFree(ctx->d_total);
     for (auto& v : ctx->prof_events) { if (v) { for (cudaEvent_t e : *v) cudaEventDestroy(e); delete v; } }
     delete ctx;
 }
@@ -244,7 +247,7 @@ int pct_plan_info(const pct_paths* P, pct_plan_stats* out) {
     const SolvePlan* pl = P->plan;
     if (!pl) return PCT_OK;
     out->block_size = pl->block_size; out->n_blocks = pl->n_blocks; out->n_groups = pl->n_groups; out->n_direct = pl->n_direct;
-    out->plan_bytes = pl->cnt_bytes + 8 * pl->stream_words + P->m * 13 + (pl->n_groups + 1) * (int64_t)sizeof(PlanGroup) + pl->n_blocks * 4;
+    out->plan_bytes = (pl->counts ? 4 * pl->n_blocks * P->n_vox : 0) + pl->cnt_bytes + 8 * pl->stream_words + P->m * 13 + (pl->n_groups + 1) * (int64_t)sizeof(PlanGroup) + pl->n_blocks * 4;
     return PCT_OK;
 }
 
@@ -329,13 +332,19 @@ int pct_solve(pct_ctx* ctx, const pct_paths* P, const float* b, const float* x0,
         for (int64_t t = 0, i0 = 0; i0 < P->m; i0 += block_size, ++t) {
             const int64_t i1 = (P->m - i0) < block_size ? P->m : i0 + block_size;
             if (plan) {
-                if ((rc = launch_block_windowed(ctx, P, plan, t, b, x_out, ctx->ds, st)) != PCT_OK) return rc;
+                // s_j^t does not depend on x (R15): the first sweep over block t counts and stores it, later sweeps
+                // (and later calls with the same paths and block size) accumulate Delta only
+                uint32_t* counts = plan->counts ? plan->counts + (size_t)t * (size_t)ctx->n_vox : nullptr;
+                const bool cached = counts && plan->counts_ready[(size_t)t];
+                if ((rc = launch_block_windowed(ctx, P, plan, t, !cached, b, x_out, ctx->ds, ctx->dsum, st)) != PCT_OK) return rc;
                 const int64_t nd = plan->direct_count[(size_t)t];
-                if (nd > 0 && (rc = launch_block_project_scatter(ctx, P, i0, i0 + nd, plan->direct_list, b, x_out, ctx->ds, st)) != PCT_OK) return rc;
+                if (nd > 0 && (rc = launch_block_project_scatter(ctx, P, i0, i0 + nd, plan->direct_list, !cached, b, x_out, ctx->ds, ctx->dsum, st)) != PCT_OK) return rc;
+                if ((rc = launch_block_update(ctx, x_out, ctx->ds, ctx->dsum, counts, !cached, lambda, st)) != PCT_OK) return rc;
+                if (counts) const_cast<SolvePlan*>(plan)->counts_ready[(size_t)t] = 1;
             } else {
-                if ((rc = launch_block_project_scatter(ctx, P, i0, i1, nullptr, b, x_out, ctx->ds, st)) != PCT_OK) return rc;
+                if ((rc = launch_block_project_scatter(ctx, P, i0, i1, nullptr, true, b, x_out, ctx->ds, ctx->dsum, st)) != PCT_OK) return rc;
+                if ((rc = launch_block_update(ctx, x_out, ctx->ds, ctx->dsum, nullptr, false, lambda, st)) != PCT_OK) return rc;
             }
-            if ((rc = launch_block_update(ctx, x_out, ctx->ds, lambda, st)) != PCT_OK) return rc;
         }
     }
     return PCT_OK;

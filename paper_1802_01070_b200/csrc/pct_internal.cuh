@@ -90,6 +90,8 @@ struct SolvePlan {
     uint32_t* p0;            // packed window coordinate of the first visit, per sorted position
     uint8_t* pflag;          // per sorted position: 1 = windowed, 0 = not (rejected, or listed in direct_list)
     uint8_t* cnt;            // visits per (group, slab, thread)
+    uint32_t* counts;        // cache of s_j^t: n_blocks x n_vox (nullptr if it would not fit the budget)
+    std::vector<uint8_t> counts_ready;   // per block (host): filled by the first sweep that ran with this plan
     unsigned long long* stream;   // slab-aligned copy of the windowed histories' codes (21 codes per word)
     int64_t stream_words;
     PlanGroup* groups;
@@ -114,6 +116,7 @@ struct pct_ctx {
     int solve_mode;      // 0 auto, 1 direct kernel only, 2 windowed plan whenever possible (pct_solve_config)
     int64_t solve_min_block;  // auto: blocks smaller than this take the direct kernel
     float2* ds;          // {Delta_j, s_j} accumulator, n_vox
+    float* dsum;         // Delta_j accumulator used when the block's counts are cached, n_vox
     int64_t ds_cap;
     void* scan_tmp;      // block sums for scans
     int64_t scan_tmp_bytes;
@@ -170,13 +173,13 @@ int launch_decode(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, cons
                   cudaStream_t st);
 int launch_forward_project(pct_ctx* ctx, const pct_paths* P, const float* x, float* b_out, cudaStream_t st);
 int launch_column_counts(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, uint32_t* counts, cudaStream_t st);
-int launch_block_project_scatter(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, const uint32_t* list,
-                                 const float* b, const float* x, float2* ds, cudaStream_t st);
-int launch_block_windowed(pct_ctx* ctx, const pct_paths* P, const SolvePlan* plan, int64_t block, const float* b,
-                          const float* x, float2* ds, cudaStream_t st);
+int launch_block_project_scatter(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, const uint32_t* list, bool count,
+                                 const float* b, const float* x, float2* ds, float* dsum, cudaStream_t st);
+int launch_block_windowed(pct_ctx* ctx, const pct_paths* P, const SolvePlan* plan, int64_t block, bool count, const float* b,
+                          const float* x, float2* ds, float* dsum, cudaStream_t st);
 int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaStream_t st, SolvePlan** out);
 void free_solve_plan(SolvePlan* plan);
-int launch_block_update(pct_ctx* ctx, float* x, float2* ds, float lambda, cudaStream_t st);
+int launch_block_update(pct_ctx* ctx, float* x, float2* ds, float* dsum, uint32_t* counts, bool store, float lambda, cudaStream_t st);
 int launch_fill(pct_ctx* ctx, float* p, int64_t n, float value, cudaStream_t st);
 
 }  // namespace pct

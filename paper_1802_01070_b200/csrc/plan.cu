@@ -307,7 +307,7 @@ k_plan_emit(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, co
 
 void free_solve_plan(SolvePlan* plan) {
     if (!plan) return;
-    cudaFree(plan->perm); cudaFree(plan->p0); cudaFree(plan->pflag); cudaFree(plan->cnt); cudaFree(plan->groups); cudaFree(plan->stream);
+    cudaFree(plan->perm); cudaFree(plan->p0); cudaFree(plan->pflag); cudaFree(plan->cnt); cudaFree(plan->groups); cudaFree(plan->stream); cudaFree(plan->counts);
     cudaFree(plan->direct_list); cudaFree(plan->d_direct_count);
     delete plan;
 }
@@ -321,7 +321,7 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     if (!plan) return set_error(ctx, PCT_E_OOM, "host allocation");
     plan->block_size = block_size; plan->n_blocks = n_blocks; plan->n_groups = 0; plan->n_direct = 0; plan->cnt_bytes = 0;
     plan->perm = nullptr; plan->p0 = nullptr; plan->pflag = nullptr; plan->cnt = nullptr; plan->groups = nullptr;
-    plan->direct_list = nullptr; plan->d_direct_count = nullptr; plan->stream = nullptr; plan->stream_words = 0;
+    plan->direct_list = nullptr; plan->d_direct_count = nullptr; plan->stream = nullptr; plan->stream_words = 0; plan->counts = nullptr;
     uint64_t *keysA = nullptr, *keysB = nullptr, *cnt_off = nullptr;
     uint32_t *valsA = nullptr, *valsB = nullptr, *cnt_len = nullptr;
     void* tmp = nullptr;
@@ -409,6 +409,14 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
                                                      plan->pflag, plan->stream);
     ctx->launches += 3;
     PLAN_CUDA(cudaGetLastError());
+    {   // cache of the per-block column counts, if it fits comfortably (a quarter of the free memory, at most 32 GiB)
+        size_t free_b = 0, total_b = 0;
+        const size_t need = 4 * (size_t)n_blocks * (size_t)P->n_vox;
+        if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && need <= free_b / 4 && need <= ((size_t)32 << 30)) {
+            if (cudaMalloc(&plan->counts, need) != cudaSuccess) { cudaGetLastError(); plan->counts = nullptr; }
+        }
+        plan->counts_ready.assign((size_t)n_blocks, 0);
+    }
     plan->group_begin.resize((size_t)n_blocks + 1);
     plan->direct_count.resize((size_t)n_blocks);
     PLAN_CUDA(cudaMemcpyAsync(plan->group_begin.data(), d_group_begin, sizeof(int64_t) * (size_t)n_blocks, cudaMemcpyDeviceToHost, st));

@@ -92,11 +92,14 @@ __device__ __forceinline__ void red_add_v2(float2* p, float a, float b) {
 
 // A5 + A6 (+A4 fused): for every history of the block, S_i = sum x_j (gather), c_i = (b_i - l_i S_i)/(N_i l_i) (R17),
 // then {Delta_j, s_j} += {c_i, 1} on every visit.  x is frozen during the block (R14): it is only read here.
+// COUNT = false: the block's column counts are cached (R15: they do not depend on x); only Delta_j is accumulated.
+template <bool COUNT>
 __global__ void __launch_bounds__(PROJ_THREADS)
 k_block_project_scatter(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, const int32_t* __restrict__ start,
                         const float* __restrict__ ell, const uint64_t* __restrict__ code_off,
                         const ulonglong2* __restrict__ codes, int64_t i0, int64_t i1, const uint32_t* __restrict__ list,
-                        const float* __restrict__ b, const float* __restrict__ x, float2* __restrict__ ds) {
+                        const float* __restrict__ b, const float* __restrict__ x, float2* __restrict__ ds,
+                        float* __restrict__ dsum) {
     // list == nullptr: histories [i0, i1); else the histories list[i0 .. i1) (a block's direct list, plan.cu)
     const int lane = threadIdx.x & 31;
     const int64_t warps = (int64_t)gridDim.x * PROJ_WARPS;
@@ -111,7 +114,10 @@ k_block_project_scatter(const __grid_constant__ DevCfg g, const uint32_t* __rest
         S = warp_sum(S);
         const float l = ell[i];
         const float c = (b[i] - l * S) / ((float)n * l);
-        for_each_visit(codes, off, st, n, g.sx, g.sy, g.sz, lane, [&](int vox) { red_add_v2(ds + vox, c, 1.0f); });
+        for_each_visit(codes, off, st, n, g.sx, g.sy, g.sz, lane, [&](int vox) {
+            if (COUNT) red_add_v2(ds + vox, c, 1.0f);
+            else asm volatile("red.global.add.f32 [%0], %1;" ::"l"(dsum + vox), "f"(c) : "memory");
+        });
     }
 }
 
@@ -123,6 +129,33 @@ __global__ void __launch_bounds__(256) k_block_update(float* __restrict__ x, flo
         if (a.y > 0.f) {
             x[j] += lambda * a.x / a.y;
             ds[j] = make_float2(0.f, 0.f);
+        }
+    }
+}
+
+// A7, first sweep over a block with a count cache: as k_block_update, and s_j^t is stored (all voxels: zeros too).
+__global__ void __launch_bounds__(256) k_block_update_store(float* __restrict__ x, float2* __restrict__ ds, int64_t n, float lambda,
+                                                            uint32_t* __restrict__ counts) {
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += stride) {
+        const float2 a = ds[j];
+        counts[j] = (uint32_t)a.y;
+        if (a.y > 0.f) {
+            x[j] += lambda * a.x / a.y;
+            ds[j] = make_float2(0.f, 0.f);
+        }
+    }
+}
+
+// A7 with cached counts: x_j += lambda * Delta_j / s_j^t wherever Delta_j != 0 (a zero sum leaves x_j unchanged anyway)
+__global__ void __launch_bounds__(256) k_block_update_cached(float* __restrict__ x, float* __restrict__ dsum, int64_t n, float lambda,
+                                                             const uint32_t* __restrict__ counts) {
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += stride) {
+        const float d = dsum[j];
+        if (d != 0.f) {
+            x[j] += lambda * d / (float)counts[j];
+            dsum[j] = 0.f;
         }
     }
 }
@@ -157,23 +190,31 @@ int launch_column_counts(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i
     return PCT_OK;
 }
 
-int launch_block_project_scatter(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, const uint32_t* list,
-                                 const float* b, const float* x, float2* ds, cudaStream_t st) {
+int launch_block_project_scatter(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, const uint32_t* list, bool count,
+                                 const float* b, const float* x, float2* ds, float* dsum, cudaStream_t st) {
     if (i1 <= i0) return PCT_OK;
     ProfScope prof(ctx, 3, st);
-    k_block_project_scatter<<<proj_grid(ctx, i1 - i0), PROJ_THREADS, 0, st>>>(ctx->cfg, P->N, P->start, P->ell,
-                                                                              P->code_off, P->codes, i0, i1, list, b, x, ds);
+    if (count)
+        k_block_project_scatter<true><<<proj_grid(ctx, i1 - i0), PROJ_THREADS, 0, st>>>(ctx->cfg, P->N, P->start, P->ell, P->code_off,
+                                                                                        P->codes, i0, i1, list, b, x, ds, dsum);
+    else
+        k_block_project_scatter<false><<<proj_grid(ctx, i1 - i0), PROJ_THREADS, 0, st>>>(ctx->cfg, P->N, P->start, P->ell, P->code_off,
+                                                                                         P->codes, i0, i1, list, b, x, ds, dsum);
     ++ctx->launches;
     PCT_CUDA(ctx, cudaGetLastError());
     return PCT_OK;
 }
 
-int launch_block_update(pct_ctx* ctx, float* x, float2* ds, float lambda, cudaStream_t st) {
+// counts == nullptr: fused counts in ds.  store: fused counts, and s_j is written to counts.  else: cached counts, dsum.
+int launch_block_update(pct_ctx* ctx, float* x, float2* ds, float* dsum, uint32_t* counts, bool store, float lambda, cudaStream_t st) {
     const int64_t n = ctx->n_vox;
     const int64_t want = (n + 255) / 256;
     const int64_t cap = (int64_t)ctx->num_sms * 16;
+    const unsigned grid = (unsigned)(want < cap ? want : cap);
     ProfScope prof(ctx, 2, st);
-    k_block_update<<<(unsigned)(want < cap ? want : cap), 256, 0, st>>>(x, ds, n, lambda);
+    if (!counts) k_block_update<<<grid, 256, 0, st>>>(x, ds, n, lambda);
+    else if (store) k_block_update_store<<<grid, 256, 0, st>>>(x, ds, n, lambda, counts);
+    else k_block_update_cached<<<grid, 256, 0, st>>>(x, dsum, n, lambda, counts);
     ++ctx->launches;
     PCT_CUDA(ctx, cudaGetLastError());
     return PCT_OK;

@@ -49,7 +49,8 @@ __device__ __forceinline__ Column slab_column(const PlanGroup& G, const WinGeom&
 }
 
 __device__ __forceinline__ float lds_f32(unsigned a) { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a)); return v; }
-__device__ __forceinline__ int2 lds_v2(unsigned a) { int2 v; asm volatile("ld.shared.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a)); return v; }
+__device__ __forceinline__ unsigned lds_u32(unsigned a) { unsigned v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
+__device__ __forceinline__ void red_add_f32(float* p, float a) { asm volatile("red.global.add.f32 [%0], %1;" ::"l"(p), "f"(a) : "memory"); }
 __device__ __forceinline__ void atoms_add(unsigned a, int v) { asm volatile("red.shared.add.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
 // 4-byte asynchronous global -> shared copy; valid == false writes a zero instead (src-size 0)
 __device__ __forceinline__ void cp_async_f32(unsigned dst, const float* src, bool valid) {
@@ -60,7 +61,7 @@ __device__ __forceinline__ void atoms_inc(unsigned a) { asm volatile("red.shared
 
 // One slab of one thread's walk.  The slab's codes sit in G.wps words [slab][w][thread] (21 codes each, pad = 7); the
 // loop runs to the warp's largest visit count (rounded up to 3) so that all lanes stay converged.  visit(p) is called
-// on every real visit.  tbl_s = shared address of the step table; entry = {delta, field mask}; a zero mask marks a pad.
+// on every real visit.  tbl_s = shared address of the step table; entry = delta | field mask << 16; 0 marks a pad.
 // w0 = the slab's first word (loaded by the caller ahead of time).
 template <typename F>
 __device__ __forceinline__ void walk_slab(const unsigned long long* __restrict__ sp, unsigned long long w0, int cmax,
@@ -73,23 +74,29 @@ __device__ __forceinline__ void walk_slab(const unsigned long long* __restrict__
             if (k3 >= lim) break;
 #pragma unroll
             for (int k = k3; k < k3 + 3; ++k) {
-                const unsigned code8 = (unsigned)(w >> (3 * k)) << 3 & 0x38u;
-                const int2 t = lds_v2(tbl_s + code8);
-                p = ((p + (unsigned)t.x) & (unsigned)t.y) | (p & ~(unsigned)t.y);
-                if (t.y != 0) visit(p);
+                const unsigned code4 = (unsigned)(w >> (3 * k)) << 2 & 0x1Cu;
+                const unsigned t = lds_u32(tbl_s + code4);              // delta | mask << 16; 0 = pad
+                const unsigned fm = t >> 16;
+                p = ((p + (t & 0xFFFFu)) & fm) | (p & ~fm);
+                if (t != 0u) visit(p);
             }
         }
     }
 }
 
+// COUNT = true: fused column counts, {Delta_j, s_j} go to the float2 accumulator `ds` (first sweep over a block, or no
+// count cache).  COUNT = false: s_j^t is already cached per block (it does not depend on x, R15), only Delta_j is
+// accumulated, into `dsum`; the freed half of the window holds a second copy of Delta (odd / even lanes) to halve the
+// serialisation of same-address shared atomics.
+template <bool COUNT>
 __global__ void __launch_bounds__(GROUP, 2)
 k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, const float* __restrict__ ell,
                  const uint32_t* __restrict__ perm, const uint32_t* __restrict__ p0, const uint8_t* __restrict__ pflag,
                  const uint8_t* __restrict__ cnt, const unsigned long long* __restrict__ stream,
                  const PlanGroup* __restrict__ groups, int64_t group0, const float* __restrict__ b, const float* __restrict__ x,
-                 float2* __restrict__ ds) {
+                 float2* __restrict__ ds, float* __restrict__ dsum) {
     extern __shared__ __align__(16) unsigned char smem[];
-    __shared__ int2 tbl[8];
+    __shared__ unsigned tbl[8];
     __shared__ float red[GROUP / 32];
     __shared__ PlanGroup Gs;
     if (threadIdx.x == 0) Gs = groups[group0 + blockIdx.x];
@@ -104,14 +111,14 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
     wg.dim_m = wg.x_major ? g.nx : g.ny; wg.dim_n = wg.x_major ? g.ny : g.nx; wg.dim_z = g.nz;
     if (tid < 8) {
         // {delta, field mask} of a step: fields are n (bits 2-6), row (7-10), z (11-14); additions wrap inside a field.
-        // PLAN_CODE_FIRST (6) and pad (7) do not move; a zero mask marks the pad (bit 31 of p is never set).
+        // PLAN_CODE_FIRST (6) and pad (7) do not move; the pad's entry is 0.
         const int n_plus = wg.x_major ? 2 : 0;
-        int2 e = make_int2(0, tid == PLAN_CODE_FIRST ? (int)0x80000000u : 0);
-        if (tid == G.cls) e = make_int2(0x80, 0x780);
-        else if (tid == n_plus) e = make_int2(0x4, 0x7C);
-        else if (tid == n_plus + 1) e = make_int2(0x7C, 0x7C);
-        else if (tid == 4) e = make_int2(0x800, 0x7800);
-        else if (tid == 5) e = make_int2(0x7800, 0x7800);
+        unsigned e = tid == PLAN_CODE_FIRST ? 0x80000000u : 0u;     // mask bit 15 of p: never set, so no move
+        if (tid == G.cls) e = 0x80u | 0x780u << 16;
+        else if (tid == n_plus) e = 0x4u | 0x7Cu << 16;
+        else if (tid == n_plus + 1) e = 0x7Cu | 0x7Cu << 16;
+        else if (tid == 4) e = 0x800u | 0x7800u << 16;
+        else if (tid == 5) e = 0x7800u | 0x7800u << 16;
         tbl[tid] = e;
     }
     const int rk = plan_rank(tid, (int)G.size);
@@ -193,23 +200,37 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
         const int cmax = __reduce_max_sync(0xffffffffu, c);
         const unsigned long long w0 = w_next;
         if (s + 1 < G.nslab) w_next = __ldg(my_stream + (size_t)(s + 1) * G.wps * GROUP);
-        walk_slab(my_stream + (size_t)s * G.wps * GROUP, w0, cmax, tbl_s, p, [&](unsigned q) {
-            const unsigned a = win_s + win_addr(q);
-            atoms_add(a, cfix);
-            atoms_inc(a + WIN_SLOTS * 4);
-        });
+        if (COUNT) {
+            walk_slab(my_stream + (size_t)s * G.wps * GROUP, w0, cmax, tbl_s, p, [&](unsigned q) {
+                const unsigned a = win_s + win_addr(q);
+                atoms_add(a, cfix);
+                atoms_inc(a + WIN_SLOTS * 4);
+            });
+        } else {
+            const unsigned copy = win_s + (unsigned)(tid & 1) * (WIN_SLOTS * 4);
+            walk_slab(my_stream + (size_t)s * G.wps * GROUP, w0, cmax, tbl_s, p, [&](unsigned q) { atoms_add(copy + win_addr(q), cfix); });
+        }
         __syncthreads();
         {
             const Column col = slab_column(G, wg, s, col_nq, col_ml);
 #pragma unroll
             for (int k = 0; k < STAGE_Z; ++k) {
                 const unsigned a = col_addr + k * 4096;
-                const unsigned cs = *reinterpret_cast<unsigned*>(smem + WIN_SLOTS * 4 + a);
-                if (cs != 0u) {                       // a touched slot is a verified visit: it lies inside the grid
-                    const int z = col.zb + ((col_zq0 + 2 * k - col.zb) & (WIN_Z - 1));
-                    red_add_v2_w(ds + col.base + z * wg.stride_z, (float)*reinterpret_cast<int*>(smem + a) * inv_scale, (float)cs);
-                    *reinterpret_cast<int*>(smem + a) = 0;
-                    *reinterpret_cast<unsigned*>(smem + WIN_SLOTS * 4 + a) = 0u;
+                int* d0 = reinterpret_cast<int*>(smem + a);
+                unsigned* d1 = reinterpret_cast<unsigned*>(smem + WIN_SLOTS * 4 + a);
+                const int z = col.zb + ((col_zq0 + 2 * k - col.zb) & (WIN_Z - 1));
+                if (COUNT) {
+                    const unsigned cs = *d1;
+                    if (cs != 0u) {                   // a touched slot is a verified visit: it lies inside the grid
+                        red_add_v2_w(ds + col.base + z * wg.stride_z, (float)*d0 * inv_scale, (float)cs);
+                        *d0 = 0; *d1 = 0u;
+                    }
+                } else {
+                    const int a0 = *d0, a1 = (int)*d1;
+                    if ((a0 | a1) != 0) {             // only visited slots can be non-zero
+                        if (a0 + a1 != 0) red_add_f32(dsum + col.base + z * wg.stride_z, (float)(a0 + a1) * inv_scale);
+                        *d0 = 0; *d1 = 0u;
+                    }
                 }
             }
         }
@@ -217,17 +238,22 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
     }
 }
 
-int launch_block_windowed(pct_ctx* ctx, const pct_paths* P, const SolvePlan* plan, int64_t block, const float* b,
-                          const float* x, float2* ds, cudaStream_t st) {
+int launch_block_windowed(pct_ctx* ctx, const pct_paths* P, const SolvePlan* plan, int64_t block, bool count, const float* b,
+                          const float* x, float2* ds, float* dsum, cudaStream_t st) {
     const int64_t g0 = plan->group_begin[(size_t)block], g1 = plan->group_begin[(size_t)block + 1];
     if (g1 <= g0) return PCT_OK;
     if (!ctx->k2w_ready) {
-        PCT_CUDA(ctx, cudaFuncSetAttribute(k_block_windowed, cudaFuncAttributeMaxDynamicSharedMemorySize, K2W_SMEM));
+        PCT_CUDA(ctx, cudaFuncSetAttribute(k_block_windowed<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, K2W_SMEM));
+        PCT_CUDA(ctx, cudaFuncSetAttribute(k_block_windowed<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, K2W_SMEM));
         ctx->k2w_ready = true;
     }
     ProfScope prof(ctx, 1, st);
-    k_block_windowed<<<(unsigned)(g1 - g0), GROUP, K2W_SMEM, st>>>(ctx->cfg, P->N, P->ell, plan->perm, plan->p0, plan->pflag,
-                                                                  plan->cnt, plan->stream, plan->groups, g0, b, x, ds);
+    if (count)
+        k_block_windowed<true><<<(unsigned)(g1 - g0), GROUP, K2W_SMEM, st>>>(ctx->cfg, P->N, P->ell, plan->perm, plan->p0, plan->pflag,
+                                                                            plan->cnt, plan->stream, plan->groups, g0, b, x, ds, dsum);
+    else
+        k_block_windowed<false><<<(unsigned)(g1 - g0), GROUP, K2W_SMEM, st>>>(ctx->cfg, P->N, P->ell, plan->perm, plan->p0, plan->pflag,
+                                                                             plan->cnt, plan->stream, plan->groups, g0, b, x, ds, dsum);
     ++ctx->launches;
     PCT_CUDA(ctx, cudaGetLastError());
     return PCT_OK;
