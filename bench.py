@@ -27,7 +27,7 @@ from paper_1802_01070_b200 import synth
 
 METRIC = "path-voxel updates/s per solver iteration; end-to-end recon s at 116M/261M"
 UNIT = "path-voxel updates/s"
-# algorithmic bytes of the dominant kernel (k_block_project_scatter): per visit 3 bit of
+# algorithmic bytes of the dominant kernel (the block projection, k_block_windowed / k_block_project_scatter): per visit 3 bit of
 # code (HBM) + one 4-byte gather of x_j + one 8-byte {Delta,s} reduction; per history 24 bytes of header + b_i.
 BYTES_PER_VISIT = 3.0 / 8.0 + 4.0 + 8.0
 BYTES_PER_HISTORY = 24.0
@@ -190,7 +190,7 @@ def main():
         ctx.solve(paths, b, x0, cfg.iters, cfg.block, cfg.lam, out=x)
         if ev:
             ev[2].record()
-        info.update(visits=paths.total_visits, rejected=paths.n_rejected, ties=paths.n_ties, code_bytes=paths.code_bytes,
+        info.update(plan=paths.plan_info(), visits=paths.total_visits, rejected=paths.n_rejected, ties=paths.n_ties, code_bytes=paths.code_bytes,
                     header_bytes=paths.header_bytes)
         paths.free()
 
@@ -232,7 +232,10 @@ def main():
 
     # ---- roofline of the dominant kernel (live CUDA events around every launch) -----------------------------
     peak, peak_kind = measured_peaks()
-    ps_ms, ps_n = prof["project_scatter"]
+    # dominant kernel = the block projection (windowed K2w + direct K2d launches of the same blocks)
+    ps_ms = prof["project_windowed"][0] + prof["project_direct"][0]
+    ps_n = max(prof["project_windowed"][1], 1) if prof["project_windowed"][1] else max(prof["project_direct"][1], 1)
+    kernel = "k_block_windowed" if prof["project_windowed"][1] else "k_block_project_scatter"
     blocks_per_iter = (cfg.m + cfg.block - 1) // cfg.block
     alg_bytes = args.steps * cfg.iters * (BYTES_PER_VISIT * P + BYTES_PER_HISTORY * cfg.m)
     achieved = alg_bytes / (ps_ms * 1e-3) / 1e9 if ps_ms > 0 else 0.0
@@ -240,15 +243,16 @@ def main():
     tp = os.path.join(ROOT, "profiles", "roofline_traffic.json")
     if os.path.exists(tp):
         try:
-            traffic = json.load(open(tp)).get(cfg.name, {}).get("k_block_project_scatter")
+            traffic = json.load(open(tp)).get(cfg.name, {}).get(kernel)
         except Exception:
             traffic = None
-    roofline = {"bound": "hbm", "kernel": "k_block_project_scatter", "achieved": achieved, "peak": peak, "unit": "GB/s",
+    roofline = {"bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "peak_kind": f"of {peak_kind}", "traffic": traffic,
                 "avg_launch_ms": ps_ms / max(ps_n, 1), "launches": ps_n,
                 "algorithmic_bytes_per_launch": alg_bytes / max(ps_n, 1),
                 "share_of_step": ps_ms / ms_total if ms_total > 0 else None,
-                "kernels_ms": {k: v[0] for k, v in prof.items()}}
+                "kernel_visits_per_s": args.steps * cfg.iters * P / (ps_ms * 1e-3) if ps_ms > 0 else None,
+                "kernels_ms": {k: v[0] for k, v in prof.items()}, "plan": info.get("plan")}
 
     # ---- end to end through the C-ABI on pinned HOST buffers ------------------------------------------------
     e2e = None

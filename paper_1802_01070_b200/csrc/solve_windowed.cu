@@ -137,19 +137,19 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
     const int col_nq = wg.x_major ? (tid >> 4) & (WIN_N - 1) : tid & (WIN_N - 1);
     const int col_ml = wg.x_major ? tid & (SLAB - 1) : (tid >> 5) & (SLAB - 1);
     const int col_zq0 = tid >> 9;                                            // 0 or 1; slots zq0 + 2k
-    const unsigned col_addr = win_addr(win_pack(col_nq, col_ml, col_zq0));    // + k * 4096 bytes
+    const unsigned col_addr = win_addr(win_pack(col_nq, col_ml, col_zq0));    // slot k: (col_addr ^ swizzle of z bit 1) + k * 4096
 
     // ---- pass 1: S_i = sum of x over the visits ----------------------------------------------------------------------
     // The x window is double buffered in the two halves of the shared window (pass 1 needs 32 KB of the 64 KB): slab
     // s + 1 is staged with cp.async while slab s is walked, one barrier per slab.
     auto stage = [&](int s) {
         const Column col = slab_column(G, wg, s, col_nq, col_ml);
-        const unsigned dst = win_s + (unsigned)(s & 1) * (WIN_SLOTS * 4) + col_addr;
+        const unsigned dst = win_s + (unsigned)(s & 1) * (WIN_SLOTS * 4);
 #pragma unroll
         for (int k = 0; k < STAGE_Z; ++k) {
             const int z = col.zb + ((col_zq0 + 2 * k - col.zb) & (WIN_Z - 1));
             const bool valid = col.base >= 0 && (unsigned)z < (unsigned)wg.dim_z;
-            cp_async_f32(dst + k * 4096, x + (valid ? col.base + z * wg.stride_z : 0), valid);
+            cp_async_f32(dst + (col_addr ^ ((k & 1) ? 0x40u : 0u)) + k * 4096, x + (valid ? col.base + z * wg.stride_z : 0), valid);
         }
     };
     unsigned p = p_init;
@@ -215,7 +215,7 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
             const Column col = slab_column(G, wg, s, col_nq, col_ml);
 #pragma unroll
             for (int k = 0; k < STAGE_Z; ++k) {
-                const unsigned a = col_addr + k * 4096;
+                const unsigned a = (col_addr ^ ((k & 1) ? 0x40u : 0u)) + k * 4096;   // z bit 1 enters the bank swizzle
                 int* d0 = reinterpret_cast<int*>(smem + a);
                 unsigned* d1 = reinterpret_cast<unsigned*>(smem + WIN_SLOTS * 4 + a);
                 const int z = col.zb + ((col_zq0 + 2 * k - col.zb) & (WIN_Z - 1));
