@@ -128,7 +128,8 @@ struct CodeWriter {
 };
 
 __global__ void __launch_bounds__(128)
-k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const uint8_t* __restrict__ hull, int64_t i_base,
+k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const uint8_t* __restrict__ hull,
+           const double* __restrict__ logk, int64_t i_base,
            int count, int stage_stride, ulonglong2* __restrict__ stage, uint32_t* __restrict__ nchunks, uint32_t* __restrict__ Nout,
            int32_t* __restrict__ start_out, int32_t* __restrict__ end_out, float* __restrict__ ell_out,
            uint8_t* __restrict__ flags_out, GenStats* __restrict__ stats) {
@@ -193,7 +194,8 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const uint8_t*
                 }
             }
             const double nu_t1 = dt_out - dt_in, nu_v1 = dv_out - dv_in;
-            const double inv_X0 = 1.0 / g.X0;
+            // ln(w1 / X0) = ln k + ln(du / X0) and ln(d2 / X0) = ln(K - k) + ln(du / X0): one log per history, ln k tabulated
+            const double log_du = log(du / g.X0);
             // R9-R11 walk state
             int c[3] = {h_in.c[0], h_in.c[1], h_in.c[2]};
             start_v = c[0] + g.nx * (c[1] + g.ny * c[2]);
@@ -209,7 +211,7 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const uint8_t*
                     // A2 / R7: Gaussian-conditioning form of the MLP of ref [3] (positions only):
                     // y = mu + Sigma1 R1^T (R1 Sigma1 R1^T + Sigma2)^-1 (y2 - R1 mu), mu = R0 y0
                     const double w1 = (double)k * du, d2 = D - w1;
-                    const double l1 = fma(g.log_coeff, log(w1 * inv_X0), 1.0), l2 = fma(g.log_coeff, log(d2 * inv_X0), 1.0);
+                    const double l1 = fma(g.log_coeff, __ldg(logk + k) + log_du, 1.0), l2 = fma(g.log_coeff, __ldg(logk + (K - k)) + log_du, 1.0);
                     const double g1 = l1 * l1, g2 = l2 * l2;
                     const double w1_2 = w1 * w1, d2_2 = d2 * d2;
                     const double C1 = g1 * w1 * horner6(g.s1c[0], w1);
@@ -276,7 +278,7 @@ int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, in
     const int threads = 128;
     const int blocks = (count + threads - 1) / threads;
     ProfScope prof(ctx, 0, st);
-    k_mlp_walk<<<blocks, threads, 0, st>>>(ctx->cfg, pr, hull, i_base, count, stage_stride, stage, nchunks, P->N, P->start, P->end,
+    k_mlp_walk<<<blocks, threads, 0, st>>>(ctx->cfg, pr, hull, ctx->logk, i_base, count, stage_stride, stage, nchunks, P->N, P->start, P->end,
                                            P->ell, P->flags, ctx->d_stats);
     ++ctx->launches;
     PCT_CUDA(ctx, cudaGetLastError());

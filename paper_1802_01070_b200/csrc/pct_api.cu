@@ -128,6 +128,18 @@ int pct_create(const pct_geometry* geom, const pct_mlp_params* params, int devic
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { cudaGetLastError(); pct_destroy(ctx); return PCT_E_CUDA; }
     ctx->num_sms = prop.multiProcessorCount;
+    {   // ln k table: K = ceil(D / (step_frac h)) <= ceil(max_depth / (step_frac h)) samples per history (R8)
+        const double kmax = std::ceil(params->poly_max_depth_mm / (params->step_frac * geom->h_mm)) + 2.0;
+        if (!(kmax < 16.0 * 1024 * 1024)) { pct_destroy(ctx); return PCT_E_INVALID_ARG; }
+        ctx->logk_n = (int)kmax + 1;
+        std::vector<double> tab((size_t)ctx->logk_n);
+        tab[0] = 0.0;
+        for (int k = 1; k < ctx->logk_n; ++k) tab[(size_t)k] = std::log((double)k);
+        if (cudaMalloc(&ctx->logk, sizeof(double) * tab.size()) != cudaSuccess ||
+            cudaMemcpy(ctx->logk, tab.data(), sizeof(double) * tab.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
+            cudaGetLastError(); pct_destroy(ctx); return PCT_E_OOM;
+        }
+    }
     if (cudaMalloc(&ctx->d_stats, sizeof(GenStats)) != cudaSuccess || cudaMalloc(&ctx->d_total, sizeof(unsigned long long)) != cudaSuccess) {
         cudaGetLastError(); pct_destroy(ctx); return PCT_E_OOM;
     }
@@ -138,7 +150,7 @@ int pct_create(const pct_geometry* geom, const pct_mlp_params* params, int devic
 void pct_destroy(pct_ctx* ctx) {
     if (!ctx) return;
     DeviceGuard guard(ctx->device);
-    cudaFree(ctx->ds); cudaFree(ctx->dsum); cudaFree(ctx->scan_tmp); cudaFree(ctx->d_stats); cudaFree(ctx->d_total);
+    cudaFree(ctx->ds); cudaFree(ctx->dsum); cudaFree(ctx->scan_tmp); cudaFree(ctx->logk); cudaFree(ctx->d_stats); cudaFree(ctx->d_total);
     for (auto& v : ctx->prof_events) { if (v) { for (cudaEvent_t e : *v) cudaEventDestroy(e); delete v; } }
     delete ctx;
 }
