@@ -6,6 +6,8 @@
 // samples) and by divergence in the walk, not by memory: 72 B in, ~60-170 B out per history.
 // Codes go to a staging buffer laid out [chunk][history-in-batch] (so that a warp's k-th chunks are contiguous)
 // and are compacted to their final 16-byte-aligned position once the batch's sizes are known.
+#include <cub/device/device_radix_sort.cuh>
+
 #include "pct_internal.cuh"
 
 namespace pct {
@@ -127,51 +129,97 @@ struct CodeWriter {
     __device__ __forceinline__ int finish() { if (nc > 0) flush(); return chunk; }
 };
 
+// Hull record of one history (A1): what k_hull hands to k_mlp_walk.  K = number of MLP segments (R8); K = 0: rejected.
+struct alignas(16) HullRec {
+    double pin[3], pout[3];      // P_0, P_K (grid frame)
+    int32_t vin, vout;           // V_s, V_e (linear voxel index)
+    uint32_t K, flags;
+};
+
+// A1 / R3-R5: tracker record -> hull entry/exit.  One thread per history.  Also emits the sort key K: k_mlp_walk runs
+// the batch in order of K so that the lanes of a warp have the same trip count (the sample loop is the whole cost).
 __global__ void __launch_bounds__(128)
-k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const uint8_t* __restrict__ hull,
+k_hull(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const uint8_t* __restrict__ hull, int64_t i_base, int count,
+       HullRec* __restrict__ recs, uint32_t* __restrict__ keys, uint32_t* __restrict__ vals) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= count) return;
+    const int64_t i = i_base + p;
+    const double phi = pr.phi[i], t_in = pr.t_in[i], v_in = pr.v_in[i], dt_in = pr.dt_in[i], dv_in = pr.dv_in[i];
+    const double t_out = pr.t_out[i], v_out = pr.v_out[i], dt_out = pr.dt_out[i], dv_out = pr.dv_out[i];
+    HullRec r;
+    r.K = 0; r.flags = 0; r.vin = r.vout = -1;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) { r.pin[a] = 0.0; r.pout[a] = 0.0; }
+    do {
+        if (!(isfinite(phi) && isfinite(t_in) && isfinite(v_in) && isfinite(dt_in) && isfinite(dv_in) &&
+              isfinite(t_out) && isfinite(v_out) && isfinite(dt_out) && isfinite(dv_out))) {
+            r.flags = PCT_REJ_NONFINITE; break;
+        }
+        double sph, cph;
+        sincos(phi, &sph, &cph);
+        // R4: entry ray, reversed exit ray (grid frame, R1)
+        Hit h_in, h_out;
+        {
+            const double T[3] = {g.u_in * cph - t_in * sph, g.u_in * sph + t_in * cph, v_in};
+            const double d[3] = {cph - dt_in * sph, sph + dt_in * cph, dv_in};
+            find_hull(g, hull, T, d, h_in);
+        }
+        {
+            const double T[3] = {g.u_out * cph - t_out * sph, g.u_out * sph + t_out * cph, v_out};
+            const double d[3] = {-(cph - dt_out * sph), -(sph + dt_out * cph), -dv_out};
+            find_hull(g, hull, T, d, h_out);
+        }
+        if (!h_in.ok || !h_out.ok) { r.flags = PCT_REJ_MISS; break; }
+        if (h_in.tie || h_out.tie) r.flags |= PCT_TIE;
+        const double u0 = h_in.P[0] * cph + h_in.P[1] * sph, u2 = h_out.P[0] * cph + h_out.P[1] * sph;
+        const double D = u2 - u0;
+        if (!(D > 0.0)) { r.flags = PCT_REJ_ORDER; break; }
+        if (D > g.max_depth) { r.flags = PCT_REJ_DEPTH; break; }
+        r.K = (uint32_t)max(1, (int)ceil(D / (g.step_frac * g.h) - 1e-9));     // R8
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { r.pin[a] = h_in.P[a]; r.pout[a] = h_out.P[a]; }
+        r.vin = h_in.c[0] + g.nx * (h_in.c[1] + g.ny * h_in.c[2]);
+        r.vout = h_out.c[0] + g.nx * (h_out.c[1] + g.ny * h_out.c[2]);
+    } while (false);
+    recs[p] = r;
+    keys[p] = r.K;
+    vals[p] = (uint32_t)p;
+}
+
+// A2 + A3.  Thread q of the batch takes history p = order[q] (the batch sorted by K, see k_hull).
+__global__ void __launch_bounds__(128)
+k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const HullRec* __restrict__ recs, const uint32_t* __restrict__ order,
            const double* __restrict__ logk, int64_t i_base,
            int count, int stage_stride, ulonglong2* __restrict__ stage, uint32_t* __restrict__ nchunks, uint32_t* __restrict__ Nout,
            int32_t* __restrict__ start_out, int32_t* __restrict__ end_out, float* __restrict__ ell_out,
            uint8_t* __restrict__ flags_out, GenStats* __restrict__ stats) {
-    const int p = blockIdx.x * blockDim.x + threadIdx.x;
-    const bool active = p < count;
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool active = q < count;
     unsigned flags = 0;
     unsigned N = 0;
     int n_chunks = 0;
     if (active) {
+        const int p = (int)order[q];
         const int64_t i = i_base + p;
-        const double phi = pr.phi[i], t_in = pr.t_in[i], v_in = pr.v_in[i], dt_in = pr.dt_in[i], dv_in = pr.dv_in[i];
-        const double t_out = pr.t_out[i], v_out = pr.v_out[i], dt_out = pr.dt_out[i], dv_out = pr.dv_out[i];
+        const HullRec rec = recs[p];
+        flags = rec.flags;
         int32_t start_v = -1, end_v = -1;
         float ell = 0.f;
-        do {
-            if (!(isfinite(phi) && isfinite(t_in) && isfinite(v_in) && isfinite(dt_in) && isfinite(dv_in) &&
-                  isfinite(t_out) && isfinite(v_out) && isfinite(dt_out) && isfinite(dv_out))) {
-                flags = PCT_REJ_NONFINITE; break;
-            }
+        if (rec.K > 0) do {
+            const double phi = pr.phi[i], dt_in = pr.dt_in[i], dv_in = pr.dv_in[i], dt_out = pr.dt_out[i], dv_out = pr.dv_out[i];
             double sph, cph;
             sincos(phi, &sph, &cph);
-            // R4: entry ray, reversed exit ray (grid frame, R1)
-            Hit h_in, h_out;
-            {
-                const double T[3] = {g.u_in * cph - t_in * sph, g.u_in * sph + t_in * cph, v_in};
-                const double d[3] = {cph - dt_in * sph, sph + dt_in * cph, dv_in};
-                find_hull(g, hull, T, d, h_in);
-            }
-            {
-                const double T[3] = {g.u_out * cph - t_out * sph, g.u_out * sph + t_out * cph, v_out};
-                const double d[3] = {-(cph - dt_out * sph), -(sph + dt_out * cph), -dv_out};
-                find_hull(g, hull, T, d, h_out);
-            }
-            if (!h_in.ok || !h_out.ok) { flags = PCT_REJ_MISS; break; }
-            if (h_in.tie || h_out.tie) flags |= PCT_TIE;
+            struct { double P[3]; int c[3]; } h_in, h_out;
+#pragma unroll
+            for (int a = 0; a < 3; ++a) { h_in.P[a] = rec.pin[a]; h_out.P[a] = rec.pout[a]; }
+            h_in.c[0] = rec.vin % g.nx; h_in.c[1] = (rec.vin / g.nx) % g.ny; h_in.c[2] = rec.vin / (g.nx * g.ny);
+            h_out.c[0] = rec.vout % g.nx; h_out.c[1] = (rec.vout / g.nx) % g.ny; h_out.c[2] = rec.vout / (g.nx * g.ny);
             // R5: MLP end states in the gantry frame
             const double u0 = h_in.P[0] * cph + h_in.P[1] * sph, t0 = -h_in.P[0] * sph + h_in.P[1] * cph, v0 = h_in.P[2];
             const double u2 = h_out.P[0] * cph + h_out.P[1] * sph, t2 = -h_out.P[0] * sph + h_out.P[1] * cph, v2 = h_out.P[2];
             const double D = u2 - u0;
-            if (!(D > 0.0)) { flags = PCT_REJ_ORDER; break; }
-            if (D > g.max_depth) { flags = PCT_REJ_DEPTH; break; }
-            const int K = max(1, (int)ceil(D / (g.step_frac * g.h) - 1e-9));     // R8
+            const int K = (int)rec.K;                                             // R8 (k_hull)
+
             const double du = D / (double)K;
             // Sigma2 moments: J_q(d2) = int_0^d2 r^q f(D-r) dr = d2^(q+1) sum_j cq[q][j] d2^j,
             // f(D-r) = sum_j c_j r^j (Taylor shift of the polynomial about the exit depth D)
@@ -255,6 +303,7 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const uint8_t*
             end_v = c[0] + g.nx * (c[1] + g.ny * c[2]);
         } while (false);
         if (N == 0) { n_chunks = 0; start_v = -1; end_v = -1; ell = 0.f; }
+        flags &= 0xffu;
         nchunks[p] = (uint32_t)n_chunks;
         Nout[i] = N;
         start_out[i] = start_v;
@@ -277,8 +326,32 @@ int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, in
                      ulonglong2* stage, uint32_t* nchunks, pct_paths* P, cudaStream_t st) {
     const int threads = 128;
     const int blocks = (count + threads - 1) / threads;
+    // scratch: hull records, sort keys/values (double buffered), cub temporary storage
+    size_t sort_tmp = 0;
+    {
+        cub::DoubleBuffer<uint32_t> dk(nullptr, nullptr), dv(nullptr, nullptr);
+        PCT_CUDA(ctx, cub::DeviceRadixSort::SortPairs(nullptr, sort_tmp, dk, dv, count, 0, 32, st));
+    }
+    auto up = [](size_t v) { return (v + 255) & ~(size_t)255; };
+    const size_t o_rec = 0, o_k0 = up(sizeof(HullRec) * (size_t)count), o_k1 = o_k0 + up(4 * (size_t)count),
+                 o_v0 = o_k1 + up(4 * (size_t)count), o_v1 = o_v0 + up(4 * (size_t)count), o_tmp = o_v1 + up(4 * (size_t)count),
+                 total = o_tmp + up(sort_tmp);
+    if (total > ctx->gen_scratch_bytes) {
+        if (ctx->gen_scratch) PCT_CUDA(ctx, cudaFree(ctx->gen_scratch));
+        ctx->gen_scratch = nullptr; ctx->gen_scratch_bytes = 0;
+        PCT_CUDA(ctx, cudaMalloc(&ctx->gen_scratch, total));
+        ctx->gen_scratch_bytes = total;
+    }
+    char* base = (char*)ctx->gen_scratch;
+    HullRec* recs = (HullRec*)(base + o_rec);
+    cub::DoubleBuffer<uint32_t> dk((uint32_t*)(base + o_k0), (uint32_t*)(base + o_k1)), dv((uint32_t*)(base + o_v0), (uint32_t*)(base + o_v1));
     ProfScope prof(ctx, 0, st);
-    k_mlp_walk<<<blocks, threads, 0, st>>>(ctx->cfg, pr, hull, ctx->logk, i_base, count, stage_stride, stage, nchunks, P->N, P->start, P->end,
+    k_hull<<<blocks, threads, 0, st>>>(ctx->cfg, pr, hull, i_base, count, recs, dk.Current(), dv.Current());
+    int key_bits = 1;
+    while ((1 << key_bits) < ctx->logk_n) ++key_bits;                  // K < logk_n
+    PCT_CUDA(ctx, cub::DeviceRadixSort::SortPairs(base + o_tmp, sort_tmp, dk, dv, count, 0, key_bits, st));
+    ctx->launches += 2;
+    k_mlp_walk<<<blocks, threads, 0, st>>>(ctx->cfg, pr, recs, dv.Current(), ctx->logk, i_base, count, stage_stride, stage, nchunks, P->N, P->start, P->end,
                                            P->ell, P->flags, ctx->d_stats);
     ++ctx->launches;
     PCT_CUDA(ctx, cudaGetLastError());

@@ -150,7 +150,7 @@ int pct_create(const pct_geometry* geom, const pct_mlp_params* params, int devic
 void pct_destroy(pct_ctx* ctx) {
     if (!ctx) return;
     DeviceGuard guard(ctx->device);
-    cudaFree(ctx->ds); cudaFree(ctx->dsum); cudaFree(ctx->scan_tmp); cudaFree(ctx->logk); cudaFree(ctx->d_stats); cudaFree(ctx->d_total);
+    cudaFree(ctx->ds); cudaFree(ctx->dsum); cudaFree(ctx->scan_tmp); cudaFree(ctx->logk); cudaFree(ctx->gen_scratch); cudaFree(ctx->d_stats); cudaFree(ctx->d_total);
     for (auto& v : ctx->prof_events) { if (v) { for (cudaEvent_t e : *v) cudaEventDestroy(e); delete v; } }
     delete ctx;
 }
