@@ -49,48 +49,85 @@ __device__ __forceinline__ int lazy_step(const DevCfg& g, const double (&A)[3], 
 struct Hit { bool ok, tie; int c[3]; double P[3]; };
 
 // A1 / R3-R4: slab-clip the ray {T + s d, s >= 0} to the grid box, then walk the chord to the first hull voxel.
+// The clip box is the bounding box of the hull voxels (g.bmin..g.bmax; the whole grid if hull == NULL): a straight
+// chord visits the same voxels wherever the walk starts, so the air between the grid faces and that box is skipped.
+// Crossing parameters inside the loop use one reciprocal per axis instead of a division per step; a decision that
+// this could change is a tie far below tie_eps and is flagged as such; the entry point P_0 itself is recomputed with
+// the exact quotient of the last crossing.
 __device__ __noinline__ void find_hull(const DevCfg& g, const uint8_t* __restrict__ hull, const double (&T)[3],
                                        const double (&d)[3], Hit& hit) {
     hit.ok = false; hit.tie = false;
+    double blo[3], bhi[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) { blo[a] = face_coord(g, a, g.bmin[a]); bhi[a] = face_coord(g, a, g.bmax[a] + 1); }
     double s_min = 0.0, s_max = INFINITY, near_s[3];
     int enter_axis = -1;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
         near_s[a] = -INFINITY;
         if (d[a] != 0.0) {
-            const double s1 = (g.lo[a] - T[a]) / d[a], s2 = (g.hi[a] - T[a]) / d[a];
+            const double s1 = (blo[a] - T[a]) / d[a], s2 = (bhi[a] - T[a]) / d[a];
             near_s[a] = fmin(s1, s2);
             if (near_s[a] > s_min) { s_min = near_s[a]; enter_axis = a; }
             s_max = fmin(s_max, fmax(s1, s2));
-        } else if (T[a] < g.lo[a] || T[a] > g.hi[a]) return;
+        } else if (T[a] < blo[a] || T[a] > bhi[a]) return;
     }
     if (!(s_min < s_max)) return;
     const double d_len = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
     double A[3], B[3];
     int c[3];
-    const int nn[3] = {g.nx, g.ny, g.nz};
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
         A[a] = T[a] + s_min * d[a];
         B[a] = T[a] + s_max * d[a];
         if (a == enter_axis) {
-            A[a] = d[a] > 0 ? g.lo[a] : g.hi[a];
-            c[a] = d[a] > 0 ? 0 : nn[a] - 1;
+            A[a] = d[a] > 0 ? blo[a] : bhi[a];
+            c[a] = d[a] > 0 ? g.bmin[a] : g.bmax[a];
         } else {
             if (enter_axis >= 0 && (s_min - near_s[a]) * d_len < g.tie_eps) hit.tie = true;
             const int i = (int)floor((A[a] - g.lo[a]) / g.h);
-            c[a] = min(max(i, 0), nn[a] - 1);
+            c[a] = min(max(i, g.bmin[a]), g.bmax[a]);
         }
     }
     const double dx = B[0] - A[0], dy = B[1] - A[1], dz = B[2] - A[2];
     const double seg_len = sqrt(dx * dx + dy * dy + dz * dz);
     Step last; last.axis = -1; last.dir = 0; last.s = 0.0; last.tie = false;
     if (hull != nullptr) {
+        double inv[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) inv[a] = 1.0 / (B[a] - A[a]);          // +-inf on a degenerate axis: never a candidate
         while (hull[c[0] + g.nx * (c[1] + g.ny * c[2])] == 0) {
-            Step st;
-            if (lazy_step(g, A, B, seg_len, c, st) != 1) return;
-            if (st.tie) hit.tie = true;
-            last = st;
+            // R9 along the chord: candidates = axes on which B lies strictly outside box(c)
+            double s[3];
+            int dir[3], best = -1;
+            double sb = 0.0;
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                const double f_lo = face_coord(g, a, c[a]), f_hi = face_coord(g, a, c[a] + 1);
+                dir[a] = 0; s[a] = 0.0;
+                if (B[a] > f_hi) { dir[a] = 1; s[a] = (f_hi - A[a]) * inv[a]; }
+                else if (B[a] < f_lo) { dir[a] = -1; s[a] = (f_lo - A[a]) * inv[a]; }
+                if (dir[a] != 0 && (best < 0 || s[a] < sb)) { best = a; sb = s[a]; }
+            }
+            if (best < 0) return;                                           // chord ends without meeting the hull
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+                if (a != best && dir[a] != 0 && (s[a] - sb) * seg_len < g.tie_eps) hit.tie = true;
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+                if (a == best) {
+                    c[a] += dir[a];
+                    if (c[a] < g.bmin[a] || c[a] > g.bmax[a]) return;       // left the hull's bounding box: miss
+                    last.axis = a; last.dir = dir[a];
+                }
+        }
+        if (last.axis >= 0) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+                if (a == last.axis) {
+                    const double face = last.dir > 0 ? face_coord(g, a, c[a]) : face_coord(g, a, c[a] + 1);
+                    last.s = (face - A[a]) / (B[a] - A[a]);
+                }
         }
     }
 #pragma unroll
@@ -353,6 +390,34 @@ int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, in
     ctx->launches += 2;
     k_mlp_walk<<<blocks, threads, 0, st>>>(ctx->cfg, pr, recs, dv.Current(), ctx->logk, i_base, count, stage_stride, stage, nchunks, P->N, P->start, P->end,
                                            P->ell, P->flags, ctx->d_stats);
+    ++ctx->launches;
+    PCT_CUDA(ctx, cudaGetLastError());
+    return PCT_OK;
+}
+
+// ---- bounding box of the hull mask: box6 = {min x, min y, min z, max x, max y, max z} (pre-set to {n.., -1..}) --------
+__global__ void __launch_bounds__(256) k_hull_bbox(const __grid_constant__ DevCfg g, const uint8_t* __restrict__ hull, int* __restrict__ box6) {
+    const int64_t n = (int64_t)g.nx * g.ny * g.nz, stride = (int64_t)gridDim.x * blockDim.x;
+    int lo[3] = {INT_MAX, INT_MAX, INT_MAX}, hi[3] = {-1, -1, -1};
+    for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += stride) {
+        if (hull[j]) {
+            const int c[3] = {(int)(j % g.nx), (int)((j / g.nx) % g.ny), (int)(j / ((int64_t)g.nx * g.ny))};
+#pragma unroll
+            for (int a = 0; a < 3; ++a) { lo[a] = min(lo[a], c[a]); hi[a] = max(hi[a], c[a]); }
+        }
+    }
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        lo[a] = __reduce_min_sync(0xffffffffu, lo[a]);
+        hi[a] = __reduce_max_sync(0xffffffffu, hi[a]);
+        if ((threadIdx.x & 31) == 0 && hi[a] >= 0) { atomicMin(box6 + a, lo[a]); atomicMax(box6 + 3 + a, hi[a]); }
+    }
+}
+
+int launch_hull_bbox(pct_ctx* ctx, const uint8_t* hull, int* d_box6, cudaStream_t st) {
+    const int init[6] = {INT_MAX, INT_MAX, INT_MAX, -1, -1, -1};
+    PCT_CUDA(ctx, cudaMemcpyAsync(d_box6, init, sizeof(init), cudaMemcpyHostToDevice, st));
+    k_hull_bbox<<<ctx->num_sms * 8, 256, 0, st>>>(ctx->cfg, hull, d_box6);
     ++ctx->launches;
     PCT_CUDA(ctx, cudaGetLastError());
     return PCT_OK;

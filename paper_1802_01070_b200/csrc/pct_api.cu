@@ -192,6 +192,22 @@ int pct_generate_mlp(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hull, v
     DeviceGuard guard(ctx->device);
     cudaStream_t st = (cudaStream_t)stream;
     ctx->cfg.u_in = pr->u_in_mm; ctx->cfg.u_out = pr->u_out_mm;
+    {   // clip box of the hull search (find_hull): bounding box of the hull voxels, or the grid
+        const int nn[3] = {ctx->geom.nx, ctx->geom.ny, ctx->geom.nz};
+        for (int a = 0; a < 3; ++a) { ctx->cfg.bmin[a] = 0; ctx->cfg.bmax[a] = nn[a] - 1; }
+        if (hull && pr->m > 0) {
+            int box[6];
+            int* d_box = reinterpret_cast<int*>(ctx->d_stats);      // scratch of 24 bytes; d_stats is cleared below
+            int rc0;
+            if ((rc0 = launch_hull_bbox(ctx, hull, d_box, st)) != PCT_OK) return rc0;
+            PCT_CUDA(ctx, cudaMemcpyAsync(box, d_box, sizeof(box), cudaMemcpyDeviceToHost, st));
+            PCT_CUDA(ctx, cudaStreamSynchronize(st));
+            for (int a = 0; a < 3; ++a) {
+                if (box[3 + a] >= box[a]) { ctx->cfg.bmin[a] = box[a]; ctx->cfg.bmax[a] = box[3 + a]; }
+                else { ctx->cfg.bmin[a] = 0; ctx->cfg.bmax[a] = -1; }               // empty hull: every ray misses
+            }
+        }
+    }
     pct_paths* P = new (std::nothrow) pct_paths();
     if (!P) return set_error(ctx, PCT_E_OOM, "host allocation");
     std::memset(P, 0, sizeof(*P));

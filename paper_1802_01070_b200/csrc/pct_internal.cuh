@@ -30,6 +30,7 @@ struct DevCfg {
     int max_visits;
     int stage_chunks;          // chunks per history in the staging buffer
     double u_in, u_out;
+    int bmin[3], bmax[3];      // bounding box of the hull voxels (inclusive); the whole grid if hull == NULL
 };
 
 struct ProtonPtrs {
@@ -170,6 +171,7 @@ struct ProfScope {
 // launchers implemented in the .cu files (all enqueue on `st`, none synchronises unless stated)
 int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, int64_t i_base, int count, int stage_stride,
                      ulonglong2* stage, uint32_t* nchunks, pct_paths* P, cudaStream_t st);
+int launch_hull_bbox(pct_ctx* ctx, const uint8_t* hull, int* d_box6, cudaStream_t st);
 int launch_scan_u32(pct_ctx* ctx, const uint32_t* in, uint64_t* out, int64_t n, uint64_t base,
                     unsigned long long* d_total, cudaStream_t st);
 int launch_compact(pct_ctx* ctx, const ulonglong2* stage, const uint32_t* nchunks, const uint64_t* off, int count,
