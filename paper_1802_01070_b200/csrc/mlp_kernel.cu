@@ -93,31 +93,42 @@ __device__ __noinline__ void find_hull(const DevCfg& g, const uint8_t* __restric
     const double seg_len = sqrt(dx * dx + dy * dy + dz * dz);
     Step last; last.axis = -1; last.dir = 0; last.s = 0.0; last.tie = false;
     if (hull != nullptr) {
-        double inv[3];
+        // incremental form of the R9 rule along one chord: per axis the next face in the direction of travel, its
+        // crossing parameter s = (face - A) * 1/(B - A), refreshed only on the axis that was stepped
+        double inv[3], fnext[3], sn[3];
+        int dir[3];
+        const int stride[3] = {1, g.nx, g.nx * g.ny};
 #pragma unroll
-        for (int a = 0; a < 3; ++a) inv[a] = 1.0 / (B[a] - A[a]);          // +-inf on a degenerate axis: never a candidate
-        while (hull[c[0] + g.nx * (c[1] + g.ny * c[2])] == 0) {
-            // R9 along the chord: candidates = axes on which B lies strictly outside box(c)
-            double s[3];
-            int dir[3], best = -1;
+        for (int a = 0; a < 3; ++a) {
+            const double dd = B[a] - A[a];
+            dir[a] = dd > 0.0 ? 1 : (dd < 0.0 ? -1 : 0);
+            inv[a] = dir[a] != 0 ? 1.0 / dd : 0.0;
+            fnext[a] = face_coord(g, a, c[a] + (dir[a] > 0 ? 1 : 0));
+            sn[a] = (fnext[a] - A[a]) * inv[a];
+        }
+        int lin = c[0] + g.nx * (c[1] + g.ny * c[2]);
+        while (hull[lin] == 0) {
+            // candidates = axes on which B lies strictly beyond the next face (B outside closed box(c) on that axis)
+            bool cand[3];
+            int best = -1;
             double sb = 0.0;
 #pragma unroll
             for (int a = 0; a < 3; ++a) {
-                const double f_lo = face_coord(g, a, c[a]), f_hi = face_coord(g, a, c[a] + 1);
-                dir[a] = 0; s[a] = 0.0;
-                if (B[a] > f_hi) { dir[a] = 1; s[a] = (f_hi - A[a]) * inv[a]; }
-                else if (B[a] < f_lo) { dir[a] = -1; s[a] = (f_lo - A[a]) * inv[a]; }
-                if (dir[a] != 0 && (best < 0 || s[a] < sb)) { best = a; sb = s[a]; }
+                cand[a] = dir[a] > 0 ? B[a] > fnext[a] : (dir[a] < 0 ? B[a] < fnext[a] : false);
+                if (cand[a] && (best < 0 || sn[a] < sb)) { best = a; sb = sn[a]; }
             }
             if (best < 0) return;                                           // chord ends without meeting the hull
 #pragma unroll
             for (int a = 0; a < 3; ++a)
-                if (a != best && dir[a] != 0 && (s[a] - sb) * seg_len < g.tie_eps) hit.tie = true;
+                if (a != best && cand[a] && (sn[a] - sb) * seg_len < g.tie_eps) hit.tie = true;
 #pragma unroll
             for (int a = 0; a < 3; ++a)
                 if (a == best) {
                     c[a] += dir[a];
                     if (c[a] < g.bmin[a] || c[a] > g.bmax[a]) return;       // left the hull's bounding box: miss
+                    lin += dir[a] * stride[a];
+                    fnext[a] = face_coord(g, a, c[a] + (dir[a] > 0 ? 1 : 0));
+                    sn[a] = (fnext[a] - A[a]) * inv[a];
                     last.axis = a; last.dir = dir[a];
                 }
         }
