@@ -147,7 +147,7 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--config", default=os.environ.get("PCT_BENCH_CONFIG", "head"), choices=sorted(synth.CONFIGS))
+    ap.add_argument("--config", default=os.environ.get("PCT_BENCH_CONFIG", "paperA"), choices=sorted(synth.CONFIGS))
     ap.add_argument("--m", type=int, default=0, help="override the number of histories (parity/debug only)")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--oracle-sample", type=int, default=100_000)

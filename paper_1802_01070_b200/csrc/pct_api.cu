@@ -19,17 +19,22 @@ int set_error(pct_ctx* ctx, int code, const char* fmt, ...) {
     return code;
 }
 
+// events come from a per-context pool (creating one per launch would cost more than the short kernels it brackets)
+static bool pool_get(pct_ctx* ctx, cudaEvent_t* e) {
+    if (!ctx->prof_pool->empty()) { *e = ctx->prof_pool->back(); ctx->prof_pool->pop_back(); return true; }
+    return cudaEventCreate(e) == cudaSuccess;
+}
 ProfScope::ProfScope(pct_ctx* c, int k, cudaStream_t s) : ctx(c), kind(k), st(s), on(c && c->profiling) {
     if (!on) return;
     cudaEvent_t e;
-    if (cudaEventCreate(&e) != cudaSuccess) { on = false; return; }
+    if (!pool_get(ctx, &e)) { on = false; return; }
     cudaEventRecord(e, st);
     ctx->prof_events[kind]->push_back(e);
 }
 ProfScope::~ProfScope() {
     if (!on) return;
     cudaEvent_t e;
-    if (cudaEventCreate(&e) != cudaSuccess) { cudaEventDestroy(ctx->prof_events[kind]->back()); ctx->prof_events[kind]->pop_back(); return; }
+    if (!pool_get(ctx, &e)) { ctx->prof_pool->push_back(ctx->prof_events[kind]->back()); ctx->prof_events[kind]->pop_back(); return; }
     cudaEventRecord(e, st);
     ctx->prof_events[kind]->push_back(e);
 }
@@ -102,6 +107,7 @@ int pct_create(const pct_geometry* geom, const pct_mlp_params* params, int devic
     if (!ctx) return PCT_E_OOM;
     std::memset(ctx, 0, sizeof(*ctx));
     for (auto& v : ctx->prof_events) v = new std::vector<cudaEvent_t>();
+    ctx->prof_pool = new std::vector<cudaEvent_t>();
     ctx->geom = *geom;
     ctx->params = *params;
     ctx->device = device;
@@ -152,6 +158,7 @@ void pct_destroy(pct_ctx* ctx) {
     DeviceGuard guard(ctx->device);
     cudaFree(ctx->ds); cudaFree(ctx->dsum); cudaFree(ctx->scan_tmp); cudaFree(ctx->logk); cudaFree(ctx->gen_scratch); cudaFree(ctx->d_stats); cudaFree(ctx->d_total);
     for (auto& v : ctx->prof_events) { if (v) { for (cudaEvent_t e : *v) cudaEventDestroy(e); delete v; } }
+    if (ctx->prof_pool) { for (cudaEvent_t e : *ctx->prof_pool) cudaEventDestroy(e); delete ctx->prof_pool; }
     delete ctx;
 }
 
@@ -171,7 +178,7 @@ int pct_profile_read(pct_ctx* ctx, pct_profile* out) {
             float ms = 0.f;
             if (cudaEventElapsedTime(&ms, v[i], v[i + 1]) == cudaSuccess) { out->ms[k] += ms; out->launches[k] += 1; }
         }
-        for (cudaEvent_t e : v) cudaEventDestroy(e);
+        for (cudaEvent_t e : v) ctx->prof_pool->push_back(e);
         v.clear();
     }
     cudaGetLastError();

@@ -131,6 +131,7 @@ struct pct_ctx {
     // optional per-kernel event timing (pct_profile_enable)
     bool profiling;
     std::vector<cudaEvent_t>* prof_events[PCT_PROFILE_KINDS];   // start/stop pairs per kind
+    std::vector<cudaEvent_t>* prof_pool;   // recycled events
     bool k2w_ready;      // dynamic shared memory attribute of k_block_windowed set on this device
 };
 
