@@ -298,6 +298,9 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const HullRec*
             CodeWriter cw;
             cw.init(stage + p, (size_t)stage_stride);
             double A[3] = {h_in.P[0], h_in.P[1], h_in.P[2]};
+            double f_lo[3], f_hi[3];
+#pragma unroll
+            for (int a = 0; a < 3; ++a) { f_lo[a] = face_coord(g, a, c[a]); f_hi[a] = face_coord(g, a, c[a] + 1); }
             double L = 0.0;
             unsigned n_vis = 1;
             bool tie = false, bad = false;
@@ -331,14 +334,44 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const HullRec*
                 const double dx = B[0] - A[0], dy = B[1] - A[1], dz = B[2] - A[2];
                 const double seg_len = sqrt(dx * dx + dy * dy + dz * dz);
                 L += seg_len;
+                // R9 closed-voxel lazy stepping along A -> B.  The faces of the current voxel are kept in registers; a
+                // crossing parameter is only computed when B lies strictly outside on more than one axis (with a single
+                // candidate the choice, and the absence of a tie, need no arithmetic).
                 for (;;) {
-                    Step st;
-                    const int r = lazy_step(g, A, B, seg_len, c, st);
-                    if (r == 0) break;
-                    if (r == 2) { flags = PCT_REJ_LEFT_GRID; bad = true; break; }
-                    if (st.tie) tie = true;
+                    int dir[3], n_cand = 0, best = -1;
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) {
+                        dir[a] = B[a] > f_hi[a] ? 1 : (B[a] < f_lo[a] ? -1 : 0);
+                        if (dir[a] != 0) { ++n_cand; if (best < 0) best = a; }
+                    }
+                    if (n_cand == 0) break;
+                    if (n_cand > 1) {
+                        double sb = 0.0, sc[3];
+                        best = -1;
+#pragma unroll
+                        for (int a = 0; a < 3; ++a) {
+                            sc[a] = 0.0;
+                            if (dir[a] != 0) {
+                                sc[a] = ((dir[a] > 0 ? f_hi[a] : f_lo[a]) - A[a]) / (B[a] - A[a]);
+                                if (best < 0 || sc[a] < sb) { best = a; sb = sc[a]; }
+                            }
+                        }
+#pragma unroll
+                        for (int a = 0; a < 3; ++a)
+                            if (a != best && dir[a] != 0 && (sc[a] - sb) * seg_len < g.tie_eps) tie = true;
+                    }
+                    int db = 0;
+#pragma unroll
+                    for (int a = 0; a < 3; ++a)
+                        if (a == best) {
+                            db = dir[a];
+                            c[a] += db;
+                            if (db > 0) { f_lo[a] = f_hi[a]; f_hi[a] = face_coord(g, a, c[a] + 1); }
+                            else { f_hi[a] = f_lo[a]; f_lo[a] = face_coord(g, a, c[a]); }
+                        }
+                    if (c[0] < 0 || c[0] >= g.nx || c[1] < 0 || c[1] >= g.ny || c[2] < 0 || c[2] >= g.nz) { flags = PCT_REJ_LEFT_GRID; bad = true; break; }
                     if (++n_vis > (unsigned)g.max_visits) { flags = PCT_REJ_CAPACITY; bad = true; break; }
-                    cw.push(2 * st.axis + (st.dir < 0 ? 1 : 0));
+                    cw.push(2 * best + (db < 0 ? 1 : 0));
                 }
                 A[0] = B[0]; A[1] = B[1]; A[2] = B[2];
             }

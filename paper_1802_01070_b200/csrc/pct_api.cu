@@ -74,8 +74,8 @@ static int ensure_codes(pct_ctx* ctx, pct_paths* P, int64_t need, cudaStream_t s
     int64_t cap = P->chunks_cap + P->chunks_cap / 2;
     if (cap < need) cap = need;
     ulonglong2* fresh = nullptr;
-    cudaError_t e = cudaMalloc(&fresh, sizeof(ulonglong2) * (size_t)cap);
-    if (e != cudaSuccess && cap > need) { cudaGetLastError(); cap = need; e = cudaMalloc(&fresh, sizeof(ulonglong2) * (size_t)cap); }
+    cudaError_t e = cudaMallocAsync(&fresh, sizeof(ulonglong2) * (size_t)cap, st);
+    if (e != cudaSuccess && cap > need) { cudaGetLastError(); cap = need; e = cudaMallocAsync(&fresh, sizeof(ulonglong2) * (size_t)cap, st); }
     if (e != cudaSuccess) { cudaGetLastError(); return set_error(ctx, PCT_E_OOM, "code stream of %lld chunks does not fit", (long long)cap); }
     if (P->chunks_used > 0)
         PCT_CUDA(ctx, cudaMemcpyAsync(fresh, P->codes, sizeof(ulonglong2) * (size_t)P->chunks_used, cudaMemcpyDeviceToDevice, st));
@@ -148,6 +148,15 @@ int pct_create(const pct_geometry* geom, const pct_mlp_params* params, int devic
     }
     if (cudaMalloc(&ctx->d_stats, sizeof(GenStats)) != cudaSuccess || cudaMalloc(&ctx->d_total, sizeof(unsigned long long)) != cudaSuccess) {
         cudaGetLastError(); pct_destroy(ctx); return PCT_E_OOM;
+    }
+    {   // large buffers come from the device's stream-ordered pool; keep freed memory cached (paths and plans are
+        // rebuilt per reconstruction, and a multi-GB cudaMalloc/cudaFree pair costs tens of milliseconds)
+        cudaMemPool_t pool;
+        if (cudaDeviceGetDefaultMemPool(&pool, device) == cudaSuccess) {
+            unsigned long long keep = ~0ull;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        }
+        cudaGetLastError();
     }
     *out = ctx;
     return PCT_OK;
@@ -228,15 +237,15 @@ int pct_generate_mlp(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hull, v
 #define GEN_CUDA(call)                                                                                          \
     do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { cudaGetLastError();                               \
         return fail(set_error(ctx, e__ == cudaErrorMemoryAllocation ? PCT_E_OOM : PCT_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e__))); } } while (0)
-    GEN_CUDA(cudaMalloc(&P->N, sizeof(uint32_t) * mm));
-    GEN_CUDA(cudaMalloc(&P->start, sizeof(int32_t) * mm));
-    GEN_CUDA(cudaMalloc(&P->end, sizeof(int32_t) * mm));
-    GEN_CUDA(cudaMalloc(&P->ell, sizeof(float) * mm));
-    GEN_CUDA(cudaMalloc(&P->flags, sizeof(uint8_t) * mm));
-    GEN_CUDA(cudaMalloc(&P->code_off, sizeof(uint64_t) * mm));
+    GEN_CUDA(cudaMallocAsync(&P->N, sizeof(uint32_t) * mm, st));
+    GEN_CUDA(cudaMallocAsync(&P->start, sizeof(int32_t) * mm, st));
+    GEN_CUDA(cudaMallocAsync(&P->end, sizeof(int32_t) * mm, st));
+    GEN_CUDA(cudaMallocAsync(&P->ell, sizeof(float) * mm, st));
+    GEN_CUDA(cudaMallocAsync(&P->flags, sizeof(uint8_t) * mm, st));
+    GEN_CUDA(cudaMallocAsync(&P->code_off, sizeof(uint64_t) * mm, st));
     const int batch_max = (int)(m < GEN_BATCH ? (m > 0 ? m : 1) : GEN_BATCH);
-    GEN_CUDA(cudaMalloc(&stage, sizeof(ulonglong2) * (size_t)batch_max * (size_t)ctx->cfg.stage_chunks));
-    GEN_CUDA(cudaMalloc(&nchunks, sizeof(uint32_t) * (size_t)batch_max));
+    GEN_CUDA(cudaMallocAsync(&stage, sizeof(ulonglong2) * (size_t)batch_max * (size_t)ctx->cfg.stage_chunks, st));
+    GEN_CUDA(cudaMallocAsync(&nchunks, sizeof(uint32_t) * (size_t)batch_max, st));
     GEN_CUDA(cudaMemsetAsync(ctx->d_stats, 0, sizeof(GenStats), st));
     const ProtonPtrs pp = {pr->phi, pr->t_in, pr->v_in, pr->dt_in, pr->dv_in, pr->t_out, pr->v_out, pr->dt_out, pr->dv_out};
     for (int64_t i0 = 0; i0 < m; i0 += GEN_BATCH) {
@@ -406,10 +415,10 @@ int pct_reconstruct_host(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hul
     do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { cudaGetLastError(); cleanup();                    \
         return set_error(ctx, e__ == cudaErrorMemoryAllocation ? PCT_E_OOM : PCT_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e__)); } } while (0)
     for (auto& e : ev) REC_CUDA(cudaEventCreate(&e));
-    REC_CUDA(cudaMalloc(&d_tr, sizeof(double) * 9 * mm));
-    REC_CUDA(cudaMalloc(&d_b, sizeof(float) * mm));
-    REC_CUDA(cudaMalloc(&d_x, sizeof(float) * (size_t)n));
-    if (hull_host) REC_CUDA(cudaMalloc(&d_hull, (size_t)n));
+    REC_CUDA(cudaMallocAsync(&d_tr, sizeof(double) * 9 * mm, st));
+    REC_CUDA(cudaMallocAsync(&d_b, sizeof(float) * mm, st));
+    REC_CUDA(cudaMallocAsync(&d_x, sizeof(float) * (size_t)n, st));
+    if (hull_host) REC_CUDA(cudaMallocAsync(&d_hull, (size_t)n, st));
     REC_CUDA(cudaEventRecord(ev[0], st));
     const double* src[9] = {pr->phi, pr->t_in, pr->v_in, pr->dt_in, pr->dv_in, pr->t_out, pr->v_out, pr->dt_out, pr->dv_out};
     for (int k = 0; k < 9 && m > 0; ++k) REC_CUDA(cudaMemcpyAsync(d_tr + (size_t)k * mm, src[k], sizeof(double) * (size_t)m, cudaMemcpyHostToDevice, st));

@@ -336,8 +336,8 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { cudaGetLastError();                               \
         return fail(set_error(ctx, e__ == cudaErrorMemoryAllocation ? PCT_E_OOM : PCT_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e__))); } } while (0)
     const size_t mm = (size_t)m;
-    PLAN_CUDA(cudaMalloc(&keysA, 8 * mm)); PLAN_CUDA(cudaMalloc(&keysB, 8 * mm));
-    PLAN_CUDA(cudaMalloc(&valsA, 4 * mm)); PLAN_CUDA(cudaMalloc(&valsB, 4 * mm));
+    PLAN_CUDA(cudaMallocAsync(&keysA, 8 * mm, st)); PLAN_CUDA(cudaMallocAsync(&keysB, 8 * mm, st));
+    PLAN_CUDA(cudaMallocAsync(&valsA, 4 * mm, st)); PLAN_CUDA(cudaMallocAsync(&valsB, 4 * mm, st));
     const unsigned nb256 = (unsigned)((m + 255) / 256);
     k_plan_keys<<<nb256, 256, 0, st>>>(ctx->cfg, P->N, P->start, P->end, m, block_size, keysA, valsA);
     ++ctx->launches;
@@ -348,7 +348,7 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     cub::DoubleBuffer<uint32_t> dv(valsA, valsB);
     size_t tmp_bytes = 0;
     PLAN_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, dk, dv, m, 0, KEY_BLOCK_SHIFT + block_bits, st));
-    PLAN_CUDA(cudaMalloc(&tmp, tmp_bytes > 0 ? tmp_bytes : 16));
+    PLAN_CUDA(cudaMallocAsync(&tmp, tmp_bytes > 0 ? tmp_bytes : 16, st));
     PLAN_CUDA(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, dk, dv, m, 0, KEY_BLOCK_SHIFT + block_bits, st));
     const uint64_t* keys = dk.Current();
     uint64_t* gid = dk.Alternate();            // reused: group id per sorted position
@@ -364,10 +364,10 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     PLAN_CUDA(cudaMemcpyAsync(&n_groups, ctx->d_total, sizeof(n_groups), cudaMemcpyDeviceToHost, st));
     PLAN_CUDA(cudaStreamSynchronize(st));
     plan->n_groups = (int64_t)n_groups;
-    PLAN_CUDA(cudaMalloc(&plan->groups, sizeof(PlanGroup) * (size_t)(n_groups + 1)));
-    PLAN_CUDA(cudaMalloc(&d_group_begin, sizeof(int64_t) * (size_t)(n_blocks + 1)));
-    PLAN_CUDA(cudaMalloc(&cnt_len, sizeof(uint32_t) * (size_t)n_groups));
-    PLAN_CUDA(cudaMalloc(&cnt_off, sizeof(uint64_t) * (size_t)n_groups));
+    PLAN_CUDA(cudaMallocAsync(&plan->groups, sizeof(PlanGroup) * (size_t)(n_groups + 1), st));
+    PLAN_CUDA(cudaMallocAsync(&d_group_begin, sizeof(int64_t) * (size_t)(n_blocks + 1), st));
+    PLAN_CUDA(cudaMallocAsync(&cnt_len, sizeof(uint32_t) * (size_t)n_groups, st));
+    PLAN_CUDA(cudaMallocAsync(&cnt_off, sizeof(uint64_t) * (size_t)n_groups, st));
     k_plan_starts<<<nb256, 256, 0, st>>>(keys, head, gid, m, plan->groups, d_group_begin);
     k_plan_params<<<(unsigned)n_groups, 256, 0, st>>>(ctx->cfg, P->start, P->end, plan->perm, m, (int64_t)n_groups, plan->groups, cnt_len);
     ctx->launches += 2;
@@ -383,12 +383,12 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     PLAN_CUDA(cudaStreamSynchronize(st));
     cudaFree(keysA); cudaFree(keysB); cudaFree(valsA); cudaFree(valsB); cudaFree(tmp);
     keysA = keysB = nullptr; valsA = valsB = nullptr; tmp = nullptr;
-    PLAN_CUDA(cudaMalloc(&plan->cnt, cnt_bytes > 0 ? (size_t)cnt_bytes : 16));
+    PLAN_CUDA(cudaMallocAsync(&plan->cnt, cnt_bytes > 0 ? (size_t)cnt_bytes : 16, st));
     PLAN_CUDA(cudaMemsetAsync(plan->cnt, 0, cnt_bytes > 0 ? (size_t)cnt_bytes : 16, st));
-    PLAN_CUDA(cudaMalloc(&plan->p0, 4 * mm));
-    PLAN_CUDA(cudaMalloc(&plan->pflag, mm));
-    PLAN_CUDA(cudaMalloc(&plan->direct_list, 4 * mm));
-    PLAN_CUDA(cudaMalloc(&plan->d_direct_count, sizeof(uint32_t) * (size_t)n_blocks));
+    PLAN_CUDA(cudaMallocAsync(&plan->p0, 4 * mm, st));
+    PLAN_CUDA(cudaMallocAsync(&plan->pflag, mm, st));
+    PLAN_CUDA(cudaMallocAsync(&plan->direct_list, 4 * mm, st));
+    PLAN_CUDA(cudaMallocAsync(&plan->d_direct_count, sizeof(uint32_t) * (size_t)n_blocks, st));
     PLAN_CUDA(cudaMemsetAsync(plan->d_direct_count, 0, sizeof(uint32_t) * (size_t)n_blocks, st));
     k_plan_verify<<<(unsigned)n_groups, GROUP, 0, st>>>(ctx->cfg, P->N, P->start, P->code_off, P->codes, plan->perm, plan->groups,
                                                        block_size, plan->p0, plan->pflag, plan->cnt, plan->direct_list,
@@ -402,7 +402,7 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     PLAN_CUDA(cudaMemcpyAsync(&stream_words, ctx->d_total, sizeof(stream_words), cudaMemcpyDeviceToHost, st));
     PLAN_CUDA(cudaStreamSynchronize(st));
     plan->stream_words = (int64_t)stream_words;
-    PLAN_CUDA(cudaMalloc(&plan->stream, stream_words > 0 ? 8 * (size_t)stream_words : 16));
+    PLAN_CUDA(cudaMallocAsync(&plan->stream, stream_words > 0 ? 8 * (size_t)stream_words : 16, st));
     PLAN_CUDA(cudaMemsetAsync(plan->stream, 0xFF, stream_words > 0 ? 8 * (size_t)stream_words : 16, st));
     k_plan_stream_off<<<(unsigned)((n_groups + 255) / 256), 256, 0, st>>>(cnt_off, (int64_t)n_groups, plan->groups);
     k_plan_emit<<<(unsigned)n_groups, GROUP, 0, st>>>(ctx->cfg, P->N, P->start, P->code_off, P->codes, plan->perm, plan->groups,
@@ -413,7 +413,7 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
         size_t free_b = 0, total_b = 0;
         const size_t need = 4 * (size_t)n_blocks * (size_t)P->n_vox;
         if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && need <= free_b / 4 && need <= ((size_t)32 << 30)) {
-            if (cudaMalloc(&plan->counts, need) != cudaSuccess) { cudaGetLastError(); plan->counts = nullptr; }
+            if (cudaMallocAsync(&plan->counts, need, st) != cudaSuccess) { cudaGetLastError(); plan->counts = nullptr; }
         }
         plan->counts_ready.assign((size_t)n_blocks, 0);
     }
