@@ -184,13 +184,33 @@ struct alignas(16) HullRec {
     uint32_t K, flags;
 };
 
-// A1 / R3-R5: tracker record -> hull entry/exit.  One thread per history.  Also emits the sort key K: k_mlp_walk runs
-// the batch in order of K so that the lanes of a warp have the same trip count (the sample loop is the whole cost).
-__global__ void __launch_bounds__(128)
-k_hull(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const uint8_t* __restrict__ hull, int64_t i_base, int count,
-       HullRec* __restrict__ recs, uint32_t* __restrict__ keys, uint32_t* __restrict__ vals) {
+// Spatial sort key of a history inside its batch: 2 mm cell of the entry tracker hit, v-major.  Neighbouring threads
+// of k_hull then shoot neighbouring, near-parallel rays: the hull search and (through the stable K sort) the voxel walk
+// of a warp take nearly the same steps.  The key only orders the work; it has no influence on any result.
+__global__ void __launch_bounds__(256)
+k_hull_keys(const ProtonPtrs pr, int64_t i_base, int count, double t_lo, double v_lo, double inv_cell, int nt, int nv,
+            uint32_t* __restrict__ keys, uint32_t* __restrict__ vals) {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= count) return;
+    const double t = pr.t_in[i_base + p], v = pr.v_in[i_base + p];
+    uint32_t key = 0;
+    if (isfinite(t) && isfinite(v)) {
+        const int tc = min(max((int)((t - t_lo) * inv_cell), 0), nt - 1), vc = min(max((int)((v - v_lo) * inv_cell), 0), nv - 1);
+        key = (uint32_t)vc * (uint32_t)nt + (uint32_t)tc;
+    }
+    keys[p] = key;
+    vals[p] = (uint32_t)p;
+}
+
+// A1 / R3-R5: tracker record -> hull entry/exit.  Thread q takes history p = order[q] (spatial order, k_hull_keys).
+// Also emits, in that order, the sort key K: k_mlp_walk runs the batch in order of K so that the lanes of a warp have the
+// same trip count (the sample loop is the whole cost); the K sort is stable, so equal-K neighbours stay neighbours in space.
+__global__ void __launch_bounds__(128)
+k_hull(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const uint8_t* __restrict__ hull, int64_t i_base, int count,
+       const uint32_t* __restrict__ order, HullRec* __restrict__ recs, uint32_t* __restrict__ keys, uint32_t* __restrict__ vals) {
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= count) return;
+    const int p = (int)order[q];
     const int64_t i = i_base + p;
     const double phi = pr.phi[i], t_in = pr.t_in[i], v_in = pr.v_in[i], dt_in = pr.dt_in[i], dv_in = pr.dv_in[i];
     const double t_out = pr.t_out[i], v_out = pr.v_out[i], dt_out = pr.dt_out[i], dv_out = pr.dv_out[i];
@@ -230,8 +250,8 @@ k_hull(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const uint8_t* __r
         r.vout = h_out.c[0] + g.nx * (h_out.c[1] + g.ny * h_out.c[2]);
     } while (false);
     recs[p] = r;
-    keys[p] = r.K;
-    vals[p] = (uint32_t)p;
+    keys[q] = r.K;
+    vals[q] = (uint32_t)p;
 }
 
 // A2 + A3.  Thread q of the batch takes history p = order[q] (the batch sorted by K, see k_hull).
@@ -414,9 +434,9 @@ int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, in
         PCT_CUDA(ctx, cub::DeviceRadixSort::SortPairs(nullptr, sort_tmp, dk, dv, count, 0, 32, st));
     }
     auto up = [](size_t v) { return (v + 255) & ~(size_t)255; };
-    const size_t o_rec = 0, o_k0 = up(sizeof(HullRec) * (size_t)count), o_k1 = o_k0 + up(4 * (size_t)count),
-                 o_v0 = o_k1 + up(4 * (size_t)count), o_v1 = o_v0 + up(4 * (size_t)count), o_tmp = o_v1 + up(4 * (size_t)count),
-                 total = o_tmp + up(sort_tmp);
+    const size_t arr = up(4 * (size_t)count);
+    const size_t o_rec = 0, o_k0 = up(sizeof(HullRec) * (size_t)count), o_k1 = o_k0 + arr, o_v0 = o_k1 + arr, o_v1 = o_v0 + arr,
+                 o_k2 = o_v1 + arr, o_k3 = o_k2 + arr, o_v2 = o_k3 + arr, o_v3 = o_v2 + arr, o_tmp = o_v3 + arr, total = o_tmp + up(sort_tmp);
     if (total > ctx->gen_scratch_bytes) {
         if (ctx->gen_scratch) PCT_CUDA(ctx, cudaFree(ctx->gen_scratch));
         ctx->gen_scratch = nullptr; ctx->gen_scratch_bytes = 0;
@@ -426,12 +446,23 @@ int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, in
     char* base = (char*)ctx->gen_scratch;
     HullRec* recs = (HullRec*)(base + o_rec);
     cub::DoubleBuffer<uint32_t> dk((uint32_t*)(base + o_k0), (uint32_t*)(base + o_k1)), dv((uint32_t*)(base + o_v0), (uint32_t*)(base + o_v1));
+    cub::DoubleBuffer<uint32_t> sk((uint32_t*)(base + o_k2), (uint32_t*)(base + o_k3)), sv((uint32_t*)(base + o_v2), (uint32_t*)(base + o_v3));
     ProfScope prof(ctx, 0, st);
-    k_hull<<<blocks, threads, 0, st>>>(ctx->cfg, pr, hull, i_base, count, recs, dk.Current(), dv.Current());
+    {   // spatial order of the batch: 2 mm cells of the entry tracker plane
+        const DevCfg& c = ctx->cfg;
+        const double ex = fmax(fabs(c.lo[0]), fabs(c.hi[0])), ey = fmax(fabs(c.lo[1]), fabs(c.hi[1]));
+        const double t_half = sqrt(ex * ex + ey * ey), cell = 2.0 * c.h;
+        const int nt = (int)fmin(4096.0, ceil(2.0 * t_half / cell) + 1.0), nv = (int)fmin(4096.0, ceil((c.hi[2] - c.lo[2]) / cell) + 1.0);
+        k_hull_keys<<<(count + 255) / 256, 256, 0, st>>>(pr, i_base, count, -t_half, c.lo[2], 1.0 / cell, nt, nv, sk.Current(), sv.Current());
+        int bits = 1;
+        while ((1LL << bits) < (long long)nt * nv) ++bits;
+        PCT_CUDA(ctx, cub::DeviceRadixSort::SortPairs(base + o_tmp, sort_tmp, sk, sv, count, 0, bits, st));
+    }
+    k_hull<<<blocks, threads, 0, st>>>(ctx->cfg, pr, hull, i_base, count, sv.Current(), recs, dk.Current(), dv.Current());
     int key_bits = 1;
     while ((1 << key_bits) < ctx->logk_n) ++key_bits;                  // K < logk_n
     PCT_CUDA(ctx, cub::DeviceRadixSort::SortPairs(base + o_tmp, sort_tmp, dk, dv, count, 0, key_bits, st));
-    ctx->launches += 2;
+    ctx->launches += 4;
     k_mlp_walk<<<blocks, threads, 0, st>>>(ctx->cfg, pr, recs, dv.Current(), ctx->logk, i_base, count, stage_stride, stage, nchunks, P->N, P->start, P->end,
                                            P->ell, P->flags, ctx->d_stats);
     ++ctx->launches;
