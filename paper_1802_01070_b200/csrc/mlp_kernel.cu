@@ -255,7 +255,7 @@ k_hull(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const uint8_t* __r
 }
 
 // A2 + A3.  Thread q of the batch takes history p = order[q] (the batch sorted by K, see k_hull).
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, 4)
 k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const HullRec* __restrict__ recs, const uint32_t* __restrict__ order,
            const double* __restrict__ logk, int64_t i_base,
            int count, int stage_stride, ulonglong2* __restrict__ stage, uint32_t* __restrict__ nchunks, uint32_t* __restrict__ Nout,
