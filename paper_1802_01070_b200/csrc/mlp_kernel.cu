@@ -160,21 +160,28 @@ __device__ __forceinline__ double horner6(const double (&c)[6], double x) {
 
 // 16-byte chunk writer: 42 codes, field k at bits 3(k%21) of word k/21; unused fields stay 7 (pad).
 struct CodeWriter {
-    unsigned long long w0, w1;
-    int nc, chunk;
-    ulonglong2* stage;       // stage[chunk * stride + p]
+    unsigned long long cur, w0;   // word being filled (fields start as pad = 7), finished first word of the chunk
+    int nc, chunk;                // codes in cur (0..20) + 21 if w0 is finished; chunks written
+    ulonglong2* stage;            // stage[chunk * stride + p]
     size_t stride;
-    __device__ __forceinline__ void init(ulonglong2* s, size_t str) { w0 = w1 = ~0ull; nc = 0; chunk = 0; stage = s; stride = str; }
-    __device__ __forceinline__ void flush() {
-        stage[(size_t)chunk * stride] = make_ulonglong2(w0, w1);
-        w0 = w1 = ~0ull; nc = 0; ++chunk;
-    }
+    __device__ __forceinline__ void init(ulonglong2* s, size_t str) { cur = w0 = ~0ull; nc = 0; chunk = 0; stage = s; stride = str; }
     __device__ __forceinline__ void push(int code) {
-        const unsigned long long x = (unsigned long long)(7 ^ code);
-        if (nc < CODES_PER_WORD) w0 ^= x << (3 * nc); else w1 ^= x << (3 * (nc - CODES_PER_WORD));
-        if (++nc == CODES_PER_CHUNK) flush();
+        const int k = nc >= CODES_PER_WORD ? nc - CODES_PER_WORD : nc;
+        cur ^= (unsigned long long)(7 ^ code) << (3 * k);
+        ++nc;
+        if (nc == CODES_PER_WORD) { w0 = cur; cur = ~0ull; }
+        else if (nc == CODES_PER_CHUNK) {
+            stage[(size_t)chunk * stride] = make_ulonglong2(w0, cur);
+            cur = w0 = ~0ull; nc = 0; ++chunk;
+        }
     }
-    __device__ __forceinline__ int finish() { if (nc > 0) flush(); return chunk; }
+    __device__ __forceinline__ int finish() {
+        if (nc > 0) {
+            stage[(size_t)chunk * stride] = nc >= CODES_PER_WORD ? make_ulonglong2(w0, cur) : make_ulonglong2(cur, ~0ull);
+            ++chunk;
+        }
+        return chunk;
+    }
 };
 
 // Hull record of one history (A1): what k_hull hands to k_mlp_walk.  K = number of MLP segments (R8); K = 0: rejected.
@@ -354,41 +361,42 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const HullRec*
                 const double dx = B[0] - A[0], dy = B[1] - A[1], dz = B[2] - A[2];
                 const double seg_len = sqrt(dx * dx + dy * dy + dz * dz);
                 L += seg_len;
-                // R9 closed-voxel lazy stepping along A -> B.  The faces of the current voxel are kept in registers; a
-                // crossing parameter is only computed when B lies strictly outside on more than one axis (with a single
-                // candidate the choice, and the absence of a tie, need no arithmetic).
+                // R9 closed-voxel lazy stepping along A -> B, branch-free inside a step (the lanes that step stay together).
+                // The faces of the current voxel are kept in registers.  Crossing parameters s_a = num_a / den_a (both
+                // positive) are compared by cross-multiplication, s_a < s_b <=> num_a den_b < num_b den_a, and the tie test
+                // (s_a - s_b) |B - A| < eps likewise without a quotient; against the quotient form this can only change a
+                // decision whose two crossings coincide to rounding, i.e. a tie, which is flagged.
                 for (;;) {
-                    int dir[3], n_cand = 0, best = -1;
+                    int dir[3];
 #pragma unroll
-                    for (int a = 0; a < 3; ++a) {
-                        dir[a] = B[a] > f_hi[a] ? 1 : (B[a] < f_lo[a] ? -1 : 0);
-                        if (dir[a] != 0) { ++n_cand; if (best < 0) best = a; }
-                    }
-                    if (n_cand == 0) break;
-                    if (n_cand > 1) {
-                        double sb = 0.0, sc[3];
-                        best = -1;
+                    for (int a = 0; a < 3; ++a) dir[a] = B[a] > f_hi[a] ? 1 : (B[a] < f_lo[a] ? -1 : 0);
+                    if ((dir[0] | dir[1] | dir[2]) == 0) break;
+                    // lowest candidate axis with the smallest s (strict comparison: x before y before z on equality)
+                    int best = dir[0] != 0 ? 0 : (dir[1] != 0 ? 1 : 2);
+                    if ((dir[0] != 0) + (dir[1] != 0) + (dir[2] != 0) > 1) {
+                        double num[3], den[3];
 #pragma unroll
                         for (int a = 0; a < 3; ++a) {
-                            sc[a] = 0.0;
-                            if (dir[a] != 0) {
-                                sc[a] = ((dir[a] > 0 ? f_hi[a] : f_lo[a]) - A[a]) / (B[a] - A[a]);
-                                if (best < 0 || sc[a] < sb) { best = a; sb = sc[a]; }
-                            }
+                            num[a] = fabs((dir[a] > 0 ? f_hi[a] : f_lo[a]) - A[a]);
+                            den[a] = fabs(B[a] - A[a]);
                         }
+                        double nb = best == 0 ? num[0] : num[1], db_ = best == 0 ? den[0] : den[1];
+                        if (best == 0 && dir[1] != 0 && num[1] * db_ < nb * den[1]) { best = 1; nb = num[1]; db_ = den[1]; }
+                        if (dir[2] != 0 && num[2] * db_ < nb * den[2]) { best = 2; nb = num[2]; db_ = den[2]; }
 #pragma unroll
                         for (int a = 0; a < 3; ++a)
-                            if (a != best && dir[a] != 0 && (sc[a] - sb) * seg_len < g.tie_eps) tie = true;
+                            if (a != best && dir[a] != 0 && (num[a] * db_ - nb * den[a]) * seg_len < g.tie_eps * (den[a] * db_)) tie = true;
                     }
-                    int db = 0;
+                    const int db = best == 0 ? dir[0] : (best == 1 ? dir[1] : dir[2]);
 #pragma unroll
-                    for (int a = 0; a < 3; ++a)
-                        if (a == best) {
-                            db = dir[a];
-                            c[a] += db;
-                            if (db > 0) { f_lo[a] = f_hi[a]; f_hi[a] = face_coord(g, a, c[a] + 1); }
-                            else { f_hi[a] = f_lo[a]; f_lo[a] = face_coord(g, a, c[a]); }
-                        }
+                    for (int a = 0; a < 3; ++a) {
+                        const bool mv = a == best;
+                        c[a] += mv ? db : 0;
+                        const double nf = face_coord(g, a, c[a] + (db > 0 ? 1 : 0));
+                        const double lo_new = db > 0 ? f_hi[a] : nf, hi_new = db > 0 ? nf : f_lo[a];
+                        f_lo[a] = mv ? lo_new : f_lo[a];
+                        f_hi[a] = mv ? hi_new : f_hi[a];
+                    }
                     if (c[0] < 0 || c[0] >= g.nx || c[1] < 0 || c[1] >= g.ny || c[2] < 0 || c[2] >= g.nz) { flags = PCT_REJ_LEFT_GRID; bad = true; break; }
                     if (++n_vis > (unsigned)g.max_visits) { flags = PCT_REJ_CAPACITY; bad = true; break; }
                     cw.push(2 * best + (db < 0 ? 1 : 0));
