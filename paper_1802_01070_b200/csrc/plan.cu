@@ -120,7 +120,8 @@ k_plan_params(const __grid_constant__ DevCfg g, const int32_t* __restrict__ star
     PlanGroup G = groups[gi];
     const uint32_t size = (uint32_t)(((gi + 1 < n_groups) ? (int64_t)groups[gi + 1].start : m) - (int64_t)G.start);
     if (G.cls == 7) {
-        if (threadIdx.x == 0) { G.size = size; G.nslab = 0; G.m_first = 0; G.nb0 = G.zb0 = G.sn = G.sz = 0; G.wps = 0; G.cnt_off = G.stream_off = 0; groups[gi] = G; cnt_len[gi] = 0; }
+        if (threadIdx.x == 0) { G.size = size; G.nslab = 0; G.m_first = 0; G.nb0 = G.zb0 = G.sn = G.sz = 0; G.wps = 0; G.cnt_off = G.stream_off = 0;
+                                G.dn_lo = G.dz_lo = 0; G.dn_hi = G.dz_hi = -1; groups[gi] = G; cnt_len[gi] = 0; }
         return;
     }
     const int dir = (G.cls & 1) ? -1 : 1;
@@ -161,6 +162,7 @@ k_plan_params(const __grid_constant__ DevCfg g, const int32_t* __restrict__ star
     G.sz = (int)llrint((double)s_z * dir * 65536.0);
     G.wps = 0;               // k_plan_verify collects the largest visits-per-slab here
     G.cnt_off = G.stream_off = 0;
+    G.dn_lo = WIN_N; G.dn_hi = -1; G.dz_lo = WIN_Z; G.dz_hi = -1;      // empty; k_plan_verify widens them
     groups[gi] = G;
     cnt_len[gi] = (uint32_t)G.nslab * GROUP;
 }
@@ -220,6 +222,7 @@ k_plan_verify(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, 
     int nrem = 0, row_cnt = 0, slab_cnt = 0, max_cnt = 0, cur_slab = ok ? r / SLAB : 0;
     int nb = ok ? plan_nbase(G, r) : 0, zb = ok ? plan_zbase(G, r) : 0;
     const uint32_t p0 = win_pack(n, r, z);
+    int on_lo = WIN_N, on_hi = -1, oz_lo = WIN_Z, oz_hi = -1;
     for (uint32_t v = 0; v < mw.n_vis && ok; ++v) {
         if (v > 0) {
             if (nrem == 0) { w = __ldg(mw.cp++); nrem = CODES_PER_WORD; }
@@ -240,8 +243,15 @@ k_plan_verify(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, 
         }
         if ((unsigned)(n - nb) >= (unsigned)WIN_N || (unsigned)(z - zb) >= (unsigned)WIN_Z || ++row_cnt > MAX_ROW_VISITS) { ok = false; break; }
         ++slab_cnt;
+        on_lo = min(on_lo, n - nb); on_hi = max(on_hi, n - nb); oz_lo = min(oz_lo, z - zb); oz_hi = max(oz_hi, z - zb);
     }
     if (ok) {
+        // widen the group's visited extent (the plain read only filters out the atomics that cannot change anything)
+        PlanGroup* Gp = groups + blockIdx.x;
+        if (on_lo < *(volatile int32_t*)&Gp->dn_lo) atomicMin(&Gp->dn_lo, on_lo);
+        if (on_hi > *(volatile int32_t*)&Gp->dn_hi) atomicMax(&Gp->dn_hi, on_hi);
+        if (oz_lo < *(volatile int32_t*)&Gp->dz_lo) atomicMin(&Gp->dz_lo, oz_lo);
+        if (oz_hi > *(volatile int32_t*)&Gp->dz_hi) atomicMax(&Gp->dz_hi, oz_hi);
         my_cnt[(size_t)cur_slab * GROUP] = (uint8_t)slab_cnt;
         max_cnt = max(max_cnt, slab_cnt);
         p0_out[mw.pos] = p0;

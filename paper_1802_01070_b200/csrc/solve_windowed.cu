@@ -35,14 +35,28 @@ constexpr int STAGE_Z = WIN_SLOTS / GROUP;   // 8
 struct Column {
     int base;        // voxel index of (row, n, z = 0), or -1 if the column lies outside the grid in n or in the row
     int zb;          // first slice of the window in this row
+    int on;          // n offset of the column from the row's window base
 };
+
+// Calls f(k, z, byte offset of the slot) for the slots of a thread's column that the group's members can visit
+// (PlanGroup::dn_*, dz_*): slot k of the column holds z with (z mod 16) = zq0 + 2k.
+template <typename F>
+__device__ __forceinline__ void for_visited_slots(const PlanGroup& G, const Column& col, int zq0, unsigned col_addr, F&& f) {
+    if (col.on < G.dn_lo || col.on > G.dn_hi) return;
+#pragma unroll
+    for (int k = 0; k < STAGE_Z; ++k) {
+        const int o = (zq0 + 2 * k - col.zb) & (WIN_Z - 1);
+        if (o >= G.dz_lo && o <= G.dz_hi) f(k, col.zb + o, (col_addr ^ ((k & 1) ? 0x40u : 0u)) + (unsigned)k * 4096u);   // z bit 1 enters the bank swizzle
+    }
+}
 
 __device__ __forceinline__ Column slab_column(const PlanGroup& G, const WinGeom& w, int s, int nq, int ml) {
     const int r = s * SLAB + ml;
     const int nb = plan_nbase(G, r);
-    const int n = nb + ((nq - nb) & (WIN_N - 1));
-    const int mj = G.m_first + w.dir * r;
     Column c;
+    c.on = (nq - nb) & (WIN_N - 1);
+    const int n = nb + c.on;
+    const int mj = G.m_first + w.dir * r;
     c.zb = plan_zbase(G, r);
     c.base = ((unsigned)n < (unsigned)w.dim_n && (unsigned)mj < (unsigned)w.dim_m) ? mj * w.stride_m + n * w.stride_n : -1;
     return c;
@@ -145,12 +159,10 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
     auto stage = [&](int s) {
         const Column col = slab_column(G, wg, s, col_nq, col_ml);
         const unsigned dst = win_s + (unsigned)(s & 1) * (WIN_SLOTS * 4);
-#pragma unroll
-        for (int k = 0; k < STAGE_Z; ++k) {
-            const int z = col.zb + ((col_zq0 + 2 * k - col.zb) & (WIN_Z - 1));
+        for_visited_slots(G, col, col_zq0, col_addr, [&](int, int z, unsigned off) {
             const bool valid = col.base >= 0 && (unsigned)z < (unsigned)wg.dim_z;
-            cp_async_f32(dst + (col_addr ^ ((k & 1) ? 0x40u : 0u)) + k * 4096, x + (valid ? col.base + z * wg.stride_z : 0), valid);
-        }
+            cp_async_f32(dst + off, x + (valid ? col.base + z * wg.stride_z : 0), valid);
+        });
     };
     unsigned p = p_init;
     float S = 0.f;
@@ -213,12 +225,9 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
         __syncthreads();
         {
             const Column col = slab_column(G, wg, s, col_nq, col_ml);
-#pragma unroll
-            for (int k = 0; k < STAGE_Z; ++k) {
-                const unsigned a = (col_addr ^ ((k & 1) ? 0x40u : 0u)) + k * 4096;   // z bit 1 enters the bank swizzle
+            for_visited_slots(G, col, col_zq0, col_addr, [&](int, int z, unsigned a) {
                 int* d0 = reinterpret_cast<int*>(smem + a);
                 unsigned* d1 = reinterpret_cast<unsigned*>(smem + WIN_SLOTS * 4 + a);
-                const int z = col.zb + ((col_zq0 + 2 * k - col.zb) & (WIN_Z - 1));
                 if (COUNT) {
                     const unsigned cs = *d1;
                     if (cs != 0u) {                   // a touched slot is a verified visit: it lies inside the grid
@@ -232,7 +241,7 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
                         *d0 = 0; *d1 = 0u;
                     }
                 }
-            }
+            });
         }
         __syncthreads();
     }
