@@ -100,6 +100,7 @@ struct SolvePlan {
     unsigned long long* stream;   // slab-aligned copy of the windowed histories' codes (21 codes per word)
     int64_t stream_words;
     PlanGroup* groups;
+    uint32_t* launch_order;  // CTA -> group: a block's groups in order of decreasing work (longest first, shorter tail)
     uint32_t* direct_list;   // histories that take the direct path; block t owns [t*block_size, t*block_size + direct_count[t])
     uint32_t* d_direct_count;
     std::vector<int64_t> group_begin;    // per block, + sentinel (host)

@@ -315,9 +315,21 @@ k_plan_emit(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, co
     if (k % CODES_PER_WORD != 0) out[((size_t)cur_slab * G.wps + k / CODES_PER_WORD) * GROUP] = acc;
 }
 
+// launch order of a block's groups: key = (block, -work), work = slabs x words per slab x members
+__global__ void k_plan_work_keys(const PlanGroup* __restrict__ groups, const uint32_t* __restrict__ perm, int64_t n_groups,
+                                 int64_t block_size, uint64_t* __restrict__ keys, uint32_t* __restrict__ vals) {
+    const int64_t gi = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gi >= n_groups) return;
+    const PlanGroup G = groups[gi];
+    const uint64_t t = (uint64_t)perm[G.start] / (uint64_t)block_size;
+    const uint32_t work = (uint32_t)G.nslab * (uint32_t)G.wps * G.size;
+    keys[gi] = (t << 32) | (uint64_t)(0xffffffffu - work);
+    vals[gi] = (uint32_t)gi;
+}
+
 void free_solve_plan(SolvePlan* plan) {
     if (!plan) return;
-    cudaFree(plan->perm); cudaFree(plan->p0); cudaFree(plan->pflag); cudaFree(plan->cnt); cudaFree(plan->groups); cudaFree(plan->stream); cudaFree(plan->counts);
+    cudaFree(plan->perm); cudaFree(plan->p0); cudaFree(plan->pflag); cudaFree(plan->cnt); cudaFree(plan->groups); cudaFree(plan->stream); cudaFree(plan->counts); cudaFree(plan->launch_order);
     cudaFree(plan->direct_list); cudaFree(plan->d_direct_count);
     delete plan;
 }
@@ -331,7 +343,7 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     if (!plan) return set_error(ctx, PCT_E_OOM, "host allocation");
     plan->block_size = block_size; plan->n_blocks = n_blocks; plan->n_groups = 0; plan->n_direct = 0; plan->cnt_bytes = 0;
     plan->perm = nullptr; plan->p0 = nullptr; plan->pflag = nullptr; plan->cnt = nullptr; plan->groups = nullptr;
-    plan->direct_list = nullptr; plan->d_direct_count = nullptr; plan->stream = nullptr; plan->stream_words = 0; plan->counts = nullptr;
+    plan->direct_list = nullptr; plan->d_direct_count = nullptr; plan->stream = nullptr; plan->stream_words = 0; plan->counts = nullptr; plan->launch_order = nullptr;
     uint64_t *keysA = nullptr, *keysB = nullptr, *cnt_off = nullptr;
     uint32_t *valsA = nullptr, *valsB = nullptr, *cnt_len = nullptr;
     void* tmp = nullptr;
@@ -419,6 +431,30 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
                                                      plan->pflag, plan->stream);
     ctx->launches += 3;
     PLAN_CUDA(cudaGetLastError());
+    {   // longest-first launch order inside every block
+        uint64_t *wk0 = nullptr, *wk1 = nullptr;
+        uint32_t *wv0 = nullptr, *wv1 = nullptr;
+        void* wtmp = nullptr;
+        const size_t ng = (size_t)n_groups;
+        auto wfree = [&]() { cudaFree(wk0); cudaFree(wk1); cudaFree(wv0); cudaFree(wv1); cudaFree(wtmp); };
+#define WORK_CUDA(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { cudaGetLastError(); wfree(); \
+        return fail(set_error(ctx, e__ == cudaErrorMemoryAllocation ? PCT_E_OOM : PCT_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e__))); } } while (0)
+        WORK_CUDA(cudaMallocAsync(&wk0, 8 * ng, st)); WORK_CUDA(cudaMallocAsync(&wk1, 8 * ng, st));
+        WORK_CUDA(cudaMallocAsync(&wv0, 4 * ng, st)); WORK_CUDA(cudaMallocAsync(&wv1, 4 * ng, st));
+        k_plan_work_keys<<<(unsigned)((n_groups + 255) / 256), 256, 0, st>>>(plan->groups, plan->perm, (int64_t)n_groups, block_size, wk0, wv0);
+        cub::DoubleBuffer<uint64_t> wk(wk0, wk1);
+        cub::DoubleBuffer<uint32_t> wv(wv0, wv1);
+        size_t wbytes = 0;
+        WORK_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, wbytes, wk, wv, (int64_t)n_groups, 0, 32 + block_bits, st));
+        WORK_CUDA(cudaMallocAsync(&wtmp, wbytes > 0 ? wbytes : 16, st));
+        WORK_CUDA(cub::DeviceRadixSort::SortPairs(wtmp, wbytes, wk, wv, (int64_t)n_groups, 0, 32 + block_bits, st));
+        WORK_CUDA(cudaStreamSynchronize(st));
+        plan->launch_order = wv.Current();
+        if (plan->launch_order == wv0) wv0 = nullptr; else wv1 = nullptr;
+        wfree();
+#undef WORK_CUDA
+        ++ctx->launches;
+    }
     {   // cache of the per-block column counts, if it fits comfortably (a quarter of the free memory, at most 32 GiB)
         size_t free_b = 0, total_b = 0;
         const size_t need = 4 * (size_t)n_blocks * (size_t)P->n_vox;

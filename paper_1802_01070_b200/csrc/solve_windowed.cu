@@ -107,13 +107,13 @@ __global__ void __launch_bounds__(GROUP, 2)
 k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, const float* __restrict__ ell,
                  const uint32_t* __restrict__ perm, const uint32_t* __restrict__ p0, const uint8_t* __restrict__ pflag,
                  const uint8_t* __restrict__ cnt, const unsigned long long* __restrict__ stream,
-                 const PlanGroup* __restrict__ groups, int64_t group0, const float* __restrict__ b, const float* __restrict__ x,
+                 const PlanGroup* __restrict__ groups, const uint32_t* __restrict__ launch_order, int64_t group0, const float* __restrict__ b, const float* __restrict__ x,
                  float2* __restrict__ ds, float* __restrict__ dsum) {
     extern __shared__ __align__(16) unsigned char smem[];
     __shared__ unsigned tbl[8];
     __shared__ float red[GROUP / 32];
     __shared__ PlanGroup Gs;
-    if (threadIdx.x == 0) Gs = groups[group0 + blockIdx.x];
+    if (threadIdx.x == 0) Gs = groups[launch_order[group0 + blockIdx.x]];
     __syncthreads();
     const PlanGroup& G = Gs;
     if (G.cls == 7 || G.nslab == 0 || G.wps == 0) return;
@@ -259,10 +259,10 @@ int launch_block_windowed(pct_ctx* ctx, const pct_paths* P, const SolvePlan* pla
     ProfScope prof(ctx, 1, st);
     if (count)
         k_block_windowed<true><<<(unsigned)(g1 - g0), GROUP, K2W_SMEM, st>>>(ctx->cfg, P->N, P->ell, plan->perm, plan->p0, plan->pflag,
-                                                                            plan->cnt, plan->stream, plan->groups, g0, b, x, ds, dsum);
+                                                                            plan->cnt, plan->stream, plan->groups, plan->launch_order, g0, b, x, ds, dsum);
     else
         k_block_windowed<false><<<(unsigned)(g1 - g0), GROUP, K2W_SMEM, st>>>(ctx->cfg, P->N, P->ell, plan->perm, plan->p0, plan->pflag,
-                                                                             plan->cnt, plan->stream, plan->groups, g0, b, x, ds, dsum);
+                                                                             plan->cnt, plan->stream, plan->groups, plan->launch_order, g0, b, x, ds, dsum);
     ++ctx->launches;
     PCT_CUDA(ctx, cudaGetLastError());
     return PCT_OK;
