@@ -85,9 +85,20 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def pick_config(name: str, m: int):
+def pick_config(name: str, m: int, block: int = 0, lam: float = 0.0, iters: int = 0):
+    """BASELINE.json config by name; m / block / lam / iters override it (config 4 = block-size / relaxation sweep on the
+    config-1 phantom and histories)."""
+    import dataclasses
     cfg = synth.CONFIGS[name]
-    return synth.scaled(cfg, m) if m else cfg
+    if m:
+        cfg = dataclasses.replace(cfg, m=m)
+    if block:
+        cfg = dataclasses.replace(cfg, block=block)
+    if lam:
+        cfg = dataclasses.replace(cfg, lam=lam)
+    if iters:
+        cfg = dataclasses.replace(cfg, iters=iters)
+    return cfg
 
 
 def oracle_sample_run(cfg, sample: int, iters: int, threads: int = 0):
@@ -115,7 +126,7 @@ def run_reference(args, rank):
     """--impl reference: the CPU oracle on the host cores (rank 0 only)."""
     if rank != 0:
         return
-    cfg = pick_config(args.config, args.m)
+    cfg = pick_config(args.config, args.m, args.block, args.lam, args.iters)
     cores = os.cpu_count() or 1
     sample = args.oracle_sample
     iters = min(cfg.iters, 2)
@@ -149,6 +160,9 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--config", default=os.environ.get("PCT_BENCH_CONFIG", "paperA"), choices=sorted(synth.CONFIGS))
     ap.add_argument("--m", type=int, default=0, help="override the number of histories (parity/debug only)")
+    ap.add_argument("--block", type=int, default=0, help="override the block size (config-4 sweep)")
+    ap.add_argument("--lam", type=float, default=0.0, help="override the relaxation (config-4 sweep)")
+    ap.add_argument("--iters", type=int, default=0, help="override the number of sweeps")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--oracle-sample", type=int, default=100_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -168,7 +182,7 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
-    cfg = pick_config(args.config, args.m)
+    cfg = pick_config(args.config, args.m, args.block, args.lam, args.iters)
 
     # ---- untimed setup: synthetic workload resident in HBM --------------------------------------------------
     x_true, hull, shadow = synth.make_phantom(cfg, dev)
@@ -239,11 +253,14 @@ def main():
     blocks_per_iter = (cfg.m + cfg.block - 1) // cfg.block
     alg_bytes = args.steps * cfg.iters * (BYTES_PER_VISIT * P + BYTES_PER_HISTORY * cfg.m)
     achieved = alg_bytes / (ps_ms * 1e-3) / 1e9 if ps_ms > 0 else 0.0
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+    traffic = None          # dram bytes per launch of the dominant kernel from the committed ncu --set full capture
+    tp = os.path.join(ROOT, "profiles", "roofline_traffic.csv")
     if os.path.exists(tp):
         try:
-            traffic = json.load(open(tp)).get(cfg.name, {}).get(kernel)
+            for ln in open(tp).read().splitlines()[1:]:
+                c, k, v = ln.split(",")
+                if c == cfg.name and k == kernel:
+                    traffic = float(v)
         except Exception:
             traffic = None
     roofline = {"bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "GB/s",
