@@ -200,15 +200,17 @@ def test_reconstruct_host_matches_device_calls(binding, oracle):
     assert np.max(np.abs(x_out.numpy() - x_o)) <= MAX_ABS_TOL
 
 
-def test_head_full_size_sampled(binding, oracle):
-    """BASELINE.json config 1 at FULL size (20 M histories, the launch configuration bench.py times): voxel lists of
-    sampled runs of histories vs the oracle one by one, plus size-independent properties of the full result."""
-    m = int(os.environ.get("PCT_TEST_FULL_M", 20_000_000))
-    cfg = synth.scaled(synth.CONFIGS["head"], m)
+@pytest.mark.parametrize("name", ["head", "paperA"])
+def test_full_size_sampled(binding, oracle, name):
+    """BASELINE.json configs 1 (20 M histories) and 2 (116 M, bench.py's default workload) at FULL size, in the launch
+    configuration bench.py times: voxel lists of sampled runs of histories vs the oracle one by one, size-independent
+    properties of the full result, and the first two blocks of the configured solve against the oracle."""
+    m = int(os.environ.get("PCT_TEST_FULL_M", synth.CONFIGS[name].m))
+    cfg = synth.scaled(synth.CONFIGS[name], m)
     x_true, hull, shadow = synth.make_phantom(cfg, "cuda")
     pr = synth.generate_protons(cfg, x_true, shadow, device="cuda")
     ctx, paths = gpu_paths(binding, cfg, pr, hull)
-    assert paths.m == m and paths.n_rejected < 0.05 * m
+    assert paths.m == m and paths.n_rejected < 0.12 * m      # cone beam: ~9 % of the field passes beside the object
     rng = np.random.default_rng(0)
     starts = np.sort(rng.integers(0, m - 400, 24))
     total_mis = 0
@@ -231,8 +233,9 @@ def test_head_full_size_sampled(binding, oracle):
     assert torch.allclose(L, N * ell.to(torch.float64), rtol=1e-5)
     counts = ctx.column_counts(paths, 0, m)
     assert int(counts.to(torch.int64).sum().item()) == paths.total_visits
-    # two blocks of the configured solve (B = 200 k) against the oracle on the same histories
-    sub_m = min(m, 400_000)
+    del counts, L, N, row_ptr, ell, flags
+    # two blocks of the configured solve (B = 200 k / 1 M) against the oracle on the same histories
+    sub_m = min(m, 2 * cfg.block)
     if os.environ.get("PCT_TEST_SKIP_BLOCKS", "0") != "1":
         sub = {k: v[:sub_m].contiguous() for k, v in pr.items()}
         ctx2, paths2 = gpu_paths(binding, cfg, sub, hull)
