@@ -274,7 +274,7 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const HullRec*
     unsigned N = 0;
     int n_chunks = 0;
     if (active) {
-        const int p = (int)order[q];
+        const int p = (int)order[count - 1 - q];      // longest first: the CTAs launched last are the cheapest (short tail)
         const int64_t i = i_base + p;
         const HullRec rec = recs[p];
         flags = rec.flags;
