@@ -79,7 +79,8 @@ typedef struct {
 
 typedef struct {
     int64_t m, total_visits, n_rejected, n_ties;
-    double ms_h2d, ms_mlp, ms_solve, ms_d2h; /* CUDA-event times of the four phases */
+    double ms_h2d, ms_mlp, ms_solve, ms_d2h; /* CUDA-event times of the four phases; the H2D copies of the tracker
+                                              * arrays run on a copy stream and overlap ms_mlp */
 } pct_recon_stats;
 
 /* Create a context on CUDA device `device`.  Validates geometry/params.  HOST pointers. */

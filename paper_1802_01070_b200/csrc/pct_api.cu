@@ -250,6 +250,7 @@ int pct_generate_mlp(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hull, v
     const ProtonPtrs pp = {pr->phi, pr->t_in, pr->v_in, pr->dt_in, pr->dv_in, pr->t_out, pr->v_out, pr->dt_out, pr->dv_out};
     for (int64_t i0 = 0; i0 < m; i0 += GEN_BATCH) {
         const int count = (int)((m - i0) < GEN_BATCH ? (m - i0) : GEN_BATCH);
+        if (ctx->batch_ready && i0 / GEN_BATCH < ctx->n_batch_ready) GEN_CUDA(cudaStreamWaitEvent(st, ctx->batch_ready[i0 / GEN_BATCH], 0));
         if ((rc = launch_mlp_batch(ctx, pp, hull, i0, count, batch_max, stage, nchunks, P, st)) != PCT_OK) return fail(rc);
         if ((rc = launch_scan_u32(ctx, nchunks, P->code_off + i0, count, (uint64_t)P->chunks_used, ctx->d_total, st)) != PCT_OK) return fail(rc);
         unsigned long long batch_chunks = 0;
@@ -405,11 +406,24 @@ int pct_reconstruct_host(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hul
     double* d_tr = nullptr; float* d_b = nullptr; float* d_x = nullptr; uint8_t* d_hull = nullptr;
     pct_paths* P = nullptr;
     cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    // the tracker arrays travel on a copy stream, one generation batch at a time, while K1 works on the batches that
+    // have arrived; b follows them and is awaited before the solve
+    cudaStream_t cs = nullptr;
+    cudaEvent_t ev_alloc = nullptr, ev_c0 = nullptr, ev_c1 = nullptr;
+    const int n_batches = (int)((m + GEN_BATCH - 1) / GEN_BATCH);
+    std::vector<cudaEvent_t> ready((size_t)n_batches, nullptr);
     int rc = PCT_OK;
     auto cleanup = [&]() {
+        ctx->batch_ready = nullptr; ctx->n_batch_ready = 0;
+        if (cs) cudaStreamSynchronize(cs);
         cudaFree(d_tr); cudaFree(d_b); cudaFree(d_x); cudaFree(d_hull);
         if (P) pct_paths_free(P);
         for (auto& e : ev) if (e) cudaEventDestroy(e);
+        for (auto& e : ready) if (e) cudaEventDestroy(e);
+        if (ev_alloc) cudaEventDestroy(ev_alloc);
+        if (ev_c0) cudaEventDestroy(ev_c0);
+        if (ev_c1) cudaEventDestroy(ev_c1);
+        if (cs) cudaStreamDestroy(cs);
     };
 #define REC_CUDA(call)                                                                                          \
     do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { cudaGetLastError(); cleanup();                    \
@@ -419,18 +433,37 @@ int pct_reconstruct_host(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hul
     REC_CUDA(cudaMallocAsync(&d_b, sizeof(float) * mm, st));
     REC_CUDA(cudaMallocAsync(&d_x, sizeof(float) * (size_t)n, st));
     if (hull_host) REC_CUDA(cudaMallocAsync(&d_hull, (size_t)n, st));
+    REC_CUDA(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
+    REC_CUDA(cudaEventCreateWithFlags(&ev_alloc, cudaEventDisableTiming));
+    REC_CUDA(cudaEventCreate(&ev_c0));
+    REC_CUDA(cudaEventCreate(&ev_c1));
+    for (auto& e : ready) REC_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     REC_CUDA(cudaEventRecord(ev[0], st));
+    REC_CUDA(cudaEventRecord(ev_alloc, st));
+    REC_CUDA(cudaStreamWaitEvent(cs, ev_alloc, 0));          // the stream-ordered allocations above
+    REC_CUDA(cudaEventRecord(ev_c0, cs));
     const double* src[9] = {pr->phi, pr->t_in, pr->v_in, pr->dt_in, pr->dv_in, pr->t_out, pr->v_out, pr->dt_out, pr->dv_out};
-    for (int k = 0; k < 9 && m > 0; ++k) REC_CUDA(cudaMemcpyAsync(d_tr + (size_t)k * mm, src[k], sizeof(double) * (size_t)m, cudaMemcpyHostToDevice, st));
-    if (m > 0) REC_CUDA(cudaMemcpyAsync(d_b, b_host, sizeof(float) * (size_t)m, cudaMemcpyHostToDevice, st));
+    for (int bi = 0; bi < n_batches; ++bi) {
+        const int64_t i0 = (int64_t)bi * GEN_BATCH;
+        const size_t cnt = (size_t)((m - i0) < GEN_BATCH ? (m - i0) : GEN_BATCH);
+        for (int k = 0; k < 9; ++k)
+            REC_CUDA(cudaMemcpyAsync(d_tr + (size_t)k * mm + i0, src[k] + i0, sizeof(double) * cnt, cudaMemcpyHostToDevice, cs));
+        REC_CUDA(cudaEventRecord(ready[(size_t)bi], cs));
+    }
+    if (m > 0) REC_CUDA(cudaMemcpyAsync(d_b, b_host, sizeof(float) * (size_t)m, cudaMemcpyHostToDevice, cs));
+    REC_CUDA(cudaEventRecord(ev_c1, cs));
     if (hull_host) REC_CUDA(cudaMemcpyAsync(d_hull, hull_host, (size_t)n, cudaMemcpyHostToDevice, st));
     if (x0_host) REC_CUDA(cudaMemcpyAsync(d_x, x0_host, sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, st));
     REC_CUDA(cudaEventRecord(ev[1], st));
     pct_protons dev = *pr;
     dev.phi = d_tr; dev.t_in = d_tr + mm; dev.v_in = d_tr + 2 * mm; dev.dt_in = d_tr + 3 * mm; dev.dv_in = d_tr + 4 * mm;
     dev.t_out = d_tr + 5 * mm; dev.v_out = d_tr + 6 * mm; dev.dt_out = d_tr + 7 * mm; dev.dv_out = d_tr + 8 * mm;
-    if ((rc = pct_generate_mlp(ctx, &dev, d_hull, stream, &P)) != PCT_OK) { cleanup(); return rc; }
+    ctx->batch_ready = ready.data(); ctx->n_batch_ready = n_batches;
+    rc = pct_generate_mlp(ctx, &dev, d_hull, stream, &P);
+    ctx->batch_ready = nullptr; ctx->n_batch_ready = 0;
+    if (rc != PCT_OK) { cleanup(); return rc; }
     REC_CUDA(cudaEventRecord(ev[2], st));
+    REC_CUDA(cudaStreamWaitEvent(st, ev_c1, 0));              // b has arrived
     if (!x0_host && (rc = launch_fill(ctx, d_x, n, 1.0f, st)) != PCT_OK) { cleanup(); return rc; }   // x0 = 1 (BASELINE.json configs)
     if ((rc = pct_solve(ctx, P, d_b, d_x, iters, block_size, lambda, d_x, stream)) != PCT_OK) { cleanup(); return rc; }
     REC_CUDA(cudaEventRecord(ev[3], st));
@@ -441,6 +474,7 @@ int pct_reconstruct_host(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hul
         stats->m = m; stats->total_visits = P->total_visits; stats->n_rejected = P->n_rejected; stats->n_ties = P->n_ties;
         float ms[4] = {0, 0, 0, 0};
         for (int k = 0; k < 4; ++k) cudaEventElapsedTime(&ms[k], ev[k], ev[k + 1]);
+        cudaEventElapsedTime(&ms[0], ev_c0, ev_c1);          // span of the copy stream; it overlaps ms_mlp
         stats->ms_h2d = ms[0]; stats->ms_mlp = ms[1]; stats->ms_solve = ms[2]; stats->ms_d2h = ms[3];
     }
 #undef REC_CUDA

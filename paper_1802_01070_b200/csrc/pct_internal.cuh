@@ -126,6 +126,8 @@ struct pct_ctx {
     int64_t ds_cap;
     void* scan_tmp;      // block sums for scans
     int64_t scan_tmp_bytes;
+    cudaEvent_t* batch_ready;   // pct_reconstruct_host: event b = tracker data of generation batch b has arrived (else NULL)
+    int n_batch_ready;
     void* gen_scratch;   // pct_generate_mlp: hull records + sort buffers of one batch
     size_t gen_scratch_bytes;
     double* logk;        // ln k for k = 0..logk_n-1 (k = 0 unused): the MLP's two log terms are ln(k du / X0), R8
