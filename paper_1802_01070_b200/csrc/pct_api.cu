@@ -441,6 +441,10 @@ int pct_reconstruct_host(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hul
     REC_CUDA(cudaEventRecord(ev[0], st));
     REC_CUDA(cudaEventRecord(ev_alloc, st));
     REC_CUDA(cudaStreamWaitEvent(cs, ev_alloc, 0));          // the stream-ordered allocations above
+    // small inputs first: the copy engine serves requests in issue order, and K1 needs the hull before its first batch
+    if (hull_host) REC_CUDA(cudaMemcpyAsync(d_hull, hull_host, (size_t)n, cudaMemcpyHostToDevice, st));
+    if (x0_host) REC_CUDA(cudaMemcpyAsync(d_x, x0_host, sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, st));
+    REC_CUDA(cudaEventRecord(ev[1], st));
     REC_CUDA(cudaEventRecord(ev_c0, cs));
     const double* src[9] = {pr->phi, pr->t_in, pr->v_in, pr->dt_in, pr->dv_in, pr->t_out, pr->v_out, pr->dt_out, pr->dv_out};
     for (int bi = 0; bi < n_batches; ++bi) {
@@ -452,9 +456,6 @@ int pct_reconstruct_host(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hul
     }
     if (m > 0) REC_CUDA(cudaMemcpyAsync(d_b, b_host, sizeof(float) * (size_t)m, cudaMemcpyHostToDevice, cs));
     REC_CUDA(cudaEventRecord(ev_c1, cs));
-    if (hull_host) REC_CUDA(cudaMemcpyAsync(d_hull, hull_host, (size_t)n, cudaMemcpyHostToDevice, st));
-    if (x0_host) REC_CUDA(cudaMemcpyAsync(d_x, x0_host, sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, st));
-    REC_CUDA(cudaEventRecord(ev[1], st));
     pct_protons dev = *pr;
     dev.phi = d_tr; dev.t_in = d_tr + mm; dev.v_in = d_tr + 2 * mm; dev.dt_in = d_tr + 3 * mm; dev.dv_in = d_tr + 4 * mm;
     dev.t_out = d_tr + 5 * mm; dev.v_out = d_tr + 6 * mm; dev.dt_out = d_tr + 7 * mm; dev.dv_out = d_tr + 8 * mm;
