@@ -164,7 +164,7 @@ def main():
     ap.add_argument("--lam", type=float, default=0.0, help="override the relaxation (config-4 sweep)")
     ap.add_argument("--iters", type=int, default=0, help="override the number of sweeps")
     ap.add_argument("--e2e-steps", type=int, default=2)
-    ap.add_argument("--oracle-sample", type=int, default=100_000)
+    ap.add_argument("--oracle-sample", type=int, default=1_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", 0))
