@@ -31,6 +31,10 @@ UNIT = "path-voxel updates/s"
 # code (HBM) + one 4-byte gather of x_j + one 8-byte {Delta,s} reduction; per history 24 bytes of header + b_i.
 BYTES_PER_VISIT = 3.0 / 8.0 + 4.0 + 8.0
 BYTES_PER_HISTORY = 24.0
+# K1 (MLP + walk) is bound by the plain FP64 ALUs: FP64 instructions per MLP sample of the Gaussian-conditioning form
+# (30 FMA of six Horner polynomials + 69 other FP64 operations incl. one division and one square root
+# counted as one each); hull search, stepping compares and integer work are not counted.
+FP64_OPS_PER_SAMPLE = 99.0
 
 
 def measured_peaks():
@@ -204,7 +208,7 @@ def main():
         ctx.solve(paths, b, x0, cfg.iters, cfg.block, cfg.lam, out=x)
         if ev:
             ev[2].record()
-        info.update(plan=paths.plan_info(), visits=paths.total_visits, rejected=paths.n_rejected, ties=paths.n_ties, code_bytes=paths.code_bytes,
+        info.update(samples=paths.total_samples, plan=paths.plan_info(), visits=paths.total_visits, rejected=paths.n_rejected, ties=paths.n_ties, code_bytes=paths.code_bytes,
                     header_bytes=paths.header_bytes)
         paths.free()
 
@@ -271,6 +275,14 @@ def main():
                 "kernel_visits_per_s": args.steps * cfg.iters * P / (ps_ms * 1e-3) if ps_ms > 0 else None,
                 "kernels_ms": {k: v[0] for k, v in prof.items()}, "plan": info.get("plan")}
 
+    fp64_peak = ctx.measure_peaks()["fp64_fma_per_s"]          # register-resident fma.rn.f64 chains, measured now
+    k1_ms = prof["mlp"][0]
+    k1_ops = FP64_OPS_PER_SAMPLE * info["samples"] * args.steps
+    roofline_k1 = {"bound": "alu", "kernel": "k_hull + k_mlp_walk (K1)", "achieved": k1_ops / (k1_ms * 1e-3) if k1_ms > 0 else 0.0,
+                   "peak": fp64_peak, "unit": "FP64 instructions/s", "frac": (k1_ops / (k1_ms * 1e-3) / fp64_peak) if k1_ms > 0 else 0.0,
+                   "peak_kind": "measured (pct_measure_peaks)", "fp64_ops_per_sample": FP64_OPS_PER_SAMPLE,
+                   "mlp_samples": info["samples"], "share_of_step": k1_ms / ms_total if ms_total > 0 else None}
+
     # ---- end to end through the C-ABI on pinned HOST buffers ------------------------------------------------
     e2e = None
     if args.e2e_steps > 0:
@@ -325,7 +337,7 @@ def main():
             "solver_ms_per_iter": ms_solve / (args.steps * cfg.iters),
             "mlp_histories_per_s": world * cfg.m * args.steps / (ms_mlp * 1e-3),
             "recon_s": ms_total * 1e-3 / args.steps,
-            "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+            "roofline": roofline, "roofline_k1": roofline_k1, "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
         }
         print(json.dumps(line), flush=True)
     if dist is not None:

@@ -75,6 +75,7 @@ typedef struct {
 
 typedef struct {
     int64_t m, total_visits, n_rejected, n_ties, code_bytes, header_bytes;
+    int64_t total_samples; /* sum of K over the accepted histories: MLP segments evaluated (R8); K1's unit of FP64 work */
 } pct_paths_stats;
 
 typedef struct {

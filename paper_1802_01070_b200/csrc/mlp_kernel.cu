@@ -271,7 +271,7 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const HullRec*
     const int q = blockIdx.x * blockDim.x + threadIdx.x;
     const bool active = q < count;
     unsigned flags = 0;
-    unsigned N = 0;
+    unsigned N = 0, n_samples = 0;
     int n_chunks = 0;
     if (active) {
         const int p = (int)order[count - 1 - q];      // longest first: the CTAs launched last are the cheapest (short tail)
@@ -406,6 +406,7 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const HullRec*
             if (bad) break;
             n_chunks = cw.finish();
             N = n_vis;
+            n_samples = (unsigned)K;
             if (tie) flags |= PCT_TIE;
             if (c[0] != h_out.c[0] || c[1] != h_out.c[1] || c[2] != h_out.c[2]) flags |= PCT_END_MISMATCH;   // R10
             ell = (float)(L / (double)N);                                                                    // R11
@@ -424,7 +425,9 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const HullRec*
     const unsigned vis = __reduce_add_sync(0xffffffffu, N);
     const unsigned rej = __reduce_add_sync(0xffffffffu, (active && N == 0) ? 1u : 0u);
     const unsigned tie_n = __reduce_add_sync(0xffffffffu, (flags & PCT_TIE) ? 1u : 0u);
+    const unsigned smp = __reduce_add_sync(0xffffffffu, n_samples);
     if ((threadIdx.x & 31) == 0) {
+        if (smp) atomicAdd(&stats->total_samples, (unsigned long long)smp);
         if (vis) atomicAdd(&stats->total_visits, (unsigned long long)vis);
         if (rej) atomicAdd(&stats->n_rejected, (unsigned long long)rej);
         if (tie_n) atomicAdd(&stats->n_ties, (unsigned long long)tie_n);
