@@ -159,25 +159,32 @@ __device__ __forceinline__ double horner6(const double (&c)[6], double x) {
 }
 
 // 16-byte chunk writer: 42 codes, field k at bits 3(k%21) of word k/21; unused fields stay 7 (pad).
+// 16-byte chunk writer: 42 codes, field k at bits 3(k%21) of word k/21; unused fields are 7 (pad).  A code is inserted
+// at the top of the word being filled and the word shifted down by one field per push, so that after 21 pushes the first
+// code sits in field 0 (one funnel shift and one OR per code, no variable shifts).
 struct CodeWriter {
-    unsigned long long cur, w0;   // word being filled (fields start as pad = 7), finished first word of the chunk
-    int nc, chunk;                // codes in cur (0..20) + 21 if w0 is finished; chunks written
+    unsigned long long acc, w0;   // word being filled; finished first word of the chunk
+    int nc, chunk;                // codes in the current chunk (0..41); chunks written
     ulonglong2* stage;            // stage[chunk * stride + p]
     size_t stride;
-    __device__ __forceinline__ void init(ulonglong2* s, size_t str) { cur = w0 = ~0ull; nc = 0; chunk = 0; stage = s; stride = str; }
+    __device__ __forceinline__ void init(ulonglong2* s, size_t str) { acc = 0ull; w0 = 0ull; nc = 0; chunk = 0; stage = s; stride = str; }
     __device__ __forceinline__ void push(int code) {
-        const int k = nc >= CODES_PER_WORD ? nc - CODES_PER_WORD : nc;
-        cur ^= (unsigned long long)(7 ^ code) << (3 * k);
+        acc = (acc >> 3) | ((unsigned long long)code << 60);
         ++nc;
-        if (nc == CODES_PER_WORD) { w0 = cur; cur = ~0ull; }
+        if (nc == CODES_PER_WORD) { w0 = acc; acc = 0ull; }
         else if (nc == CODES_PER_CHUNK) {
-            stage[(size_t)chunk * stride] = make_ulonglong2(w0, cur);
-            cur = w0 = ~0ull; nc = 0; ++chunk;
+            stage[(size_t)chunk * stride] = make_ulonglong2(w0, acc);
+            acc = 0ull; nc = 0; ++chunk;
         }
+    }
+    // a word holding k < 21 codes: shift them down to field 0 and fill the rest with pads
+    __device__ __forceinline__ static unsigned long long partial(unsigned long long a, int k) {
+        return k == 0 ? ~0ull : ((a >> (3 * (CODES_PER_WORD - k))) | (~0ull << (3 * k)));
     }
     __device__ __forceinline__ int finish() {
         if (nc > 0) {
-            stage[(size_t)chunk * stride] = nc >= CODES_PER_WORD ? make_ulonglong2(w0, cur) : make_ulonglong2(cur, ~0ull);
+            stage[(size_t)chunk * stride] = nc >= CODES_PER_WORD ? make_ulonglong2(w0, partial(acc, nc - CODES_PER_WORD))
+                                                                 : make_ulonglong2(partial(acc, nc), ~0ull);
             ++chunk;
         }
         return chunk;
@@ -361,19 +368,20 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const HullRec*
                 const double dx = B[0] - A[0], dy = B[1] - A[1], dz = B[2] - A[2];
                 const double seg_len = sqrt(dx * dx + dy * dy + dz * dz);
                 L += seg_len;
-                // R9 closed-voxel lazy stepping along A -> B, branch-free inside a step (the lanes that step stay together).
-                // The faces of the current voxel are kept in registers.  Crossing parameters s_a = num_a / den_a (both
-                // positive) are compared by cross-multiplication, s_a < s_b <=> num_a den_b < num_b den_a, and the tie test
-                // (s_a - s_b) |B - A| < eps likewise without a quotient; against the quotient form this can only change a
-                // decision whose two crossings coincide to rounding, i.e. a tie, which is flagged.
-                for (;;) {
-                    int dir[3];
-#pragma unroll
-                    for (int a = 0; a < 3; ++a) dir[a] = B[a] > f_hi[a] ? 1 : (B[a] < f_lo[a] ? -1 : 0);
-                    if ((dir[0] | dir[1] | dir[2]) == 0) break;
+                // R9 closed-voxel lazy stepping along A -> B.  The faces of the current voxel are kept in registers; d_a is
+                // the state of axis a (B beyond the high face, beyond the low face, inside) and only the axis that moved is
+                // re-examined.  With one candidate the step needs no arithmetic; with several, the crossing parameters
+                // s_a = num_a / den_a (both positive) are compared by cross-multiplication, s_a < s_b <=> num_a den_b <
+                // num_b den_a, and the tie test (s_a - s_b) |B - A| < eps likewise without a quotient; against the quotient
+                // form this can only change a decision whose crossings coincide to rounding, i.e. a tie, which is flagged.
+                int d0 = B[0] > f_hi[0] ? 1 : (B[0] < f_lo[0] ? -1 : 0);
+                int d1 = B[1] > f_hi[1] ? 1 : (B[1] < f_lo[1] ? -1 : 0);
+                int d2 = B[2] > f_hi[2] ? 1 : (B[2] < f_lo[2] ? -1 : 0);
+                while ((d0 | d1 | d2) != 0) {
                     // lowest candidate axis with the smallest s (strict comparison: x before y before z on equality)
-                    int best = dir[0] != 0 ? 0 : (dir[1] != 0 ? 1 : 2);
-                    if ((dir[0] != 0) + (dir[1] != 0) + (dir[2] != 0) > 1) {
+                    int best = d0 != 0 ? 0 : (d1 != 0 ? 1 : 2);
+                    if ((d0 != 0) + (d1 != 0) + (d2 != 0) > 1) {
+                        const int dir[3] = {d0, d1, d2};
                         double num[3], den[3];
 #pragma unroll
                         for (int a = 0; a < 3; ++a) {
@@ -381,25 +389,32 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const HullRec*
                             den[a] = fabs(B[a] - A[a]);
                         }
                         double nb = best == 0 ? num[0] : num[1], db_ = best == 0 ? den[0] : den[1];
-                        if (best == 0 && dir[1] != 0 && num[1] * db_ < nb * den[1]) { best = 1; nb = num[1]; db_ = den[1]; }
-                        if (dir[2] != 0 && num[2] * db_ < nb * den[2]) { best = 2; nb = num[2]; db_ = den[2]; }
+                        if (best == 0 && d1 != 0 && num[1] * db_ < nb * den[1]) { best = 1; nb = num[1]; db_ = den[1]; }
+                        if (d2 != 0 && num[2] * db_ < nb * den[2]) { best = 2; nb = num[2]; db_ = den[2]; }
 #pragma unroll
                         for (int a = 0; a < 3; ++a)
                             if (a != best && dir[a] != 0 && (num[a] * db_ - nb * den[a]) * seg_len < g.tie_eps * (den[a] * db_)) tie = true;
                     }
-                    const int db = best == 0 ? dir[0] : (best == 1 ? dir[1] : dir[2]);
-#pragma unroll
-                    for (int a = 0; a < 3; ++a) {
-                        const bool mv = a == best;
-                        c[a] += mv ? db : 0;
-                        const double nf = face_coord(g, a, c[a] + (db > 0 ? 1 : 0));
-                        const double lo_new = db > 0 ? f_hi[a] : nf, hi_new = db > 0 ? nf : f_lo[a];
-                        f_lo[a] = mv ? lo_new : f_lo[a];
-                        f_hi[a] = mv ? hi_new : f_hi[a];
+                    // move across the face of axis `best`; neighbouring lanes follow neighbouring paths and mostly take the
+                    // same branch
+                    int code;
+                    bool inside;
+#define PCT_MOVE_AXIS(a, d, n_a)                                                                            \
+                    {                                                                                       \
+                        c[a] += d;                                                                          \
+                        code = 2 * a + (d < 0 ? 1 : 0);                                                     \
+                        inside = (unsigned)c[a] < (unsigned)(n_a);                                          \
+                        if (d > 0) { f_lo[a] = f_hi[a]; f_hi[a] = face_coord(g, a, c[a] + 1); }             \
+                        else { f_hi[a] = f_lo[a]; f_lo[a] = face_coord(g, a, c[a]); }                       \
+                        d = B[a] > f_hi[a] ? 1 : (B[a] < f_lo[a] ? -1 : 0);                                 \
                     }
-                    if (c[0] < 0 || c[0] >= g.nx || c[1] < 0 || c[1] >= g.ny || c[2] < 0 || c[2] >= g.nz) { flags = PCT_REJ_LEFT_GRID; bad = true; break; }
+                    if (best == 0) PCT_MOVE_AXIS(0, d0, g.nx)
+                    else if (best == 1) PCT_MOVE_AXIS(1, d1, g.ny)
+                    else PCT_MOVE_AXIS(2, d2, g.nz)
+#undef PCT_MOVE_AXIS
+                    if (!inside) { flags = PCT_REJ_LEFT_GRID; bad = true; break; }
                     if (++n_vis > (unsigned)g.max_visits) { flags = PCT_REJ_CAPACITY; bad = true; break; }
-                    cw.push(2 * best + (db < 0 ? 1 : 0));
+                    cw.push(code);
                 }
                 A[0] = B[0]; A[1] = B[1]; A[2] = B[2];
             }
