@@ -95,42 +95,45 @@ __device__ __noinline__ void find_hull(const DevCfg& g, const uint8_t* __restric
     if (hull != nullptr) {
         // incremental form of the R9 rule along one chord: per axis the next face in the direction of travel, its
         // crossing parameter s = (face - A) * 1/(B - A), refreshed only on the axis that was stepped
-        double inv[3], fnext[3], sn[3];
-        int dir[3];
+        // se[a] = s of the next crossing on axis a, or +inf if B does not lie strictly beyond that face (not a candidate);
+        // left[a] = steps the axis may still take inside the hull's bounding box
+        double inv[3], se[3];
+        int dir[3], left[3], dlin[3];
         const int stride[3] = {1, g.nx, g.nx * g.ny};
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
             const double dd = B[a] - A[a];
             dir[a] = dd > 0.0 ? 1 : (dd < 0.0 ? -1 : 0);
             inv[a] = dir[a] != 0 ? 1.0 / dd : 0.0;
-            fnext[a] = face_coord(g, a, c[a] + (dir[a] > 0 ? 1 : 0));
-            sn[a] = (fnext[a] - A[a]) * inv[a];
+            const double fnext = face_coord(g, a, c[a] + (dir[a] > 0 ? 1 : 0));
+            const bool cand = dir[a] > 0 ? B[a] > fnext : (dir[a] < 0 ? B[a] < fnext : false);
+            se[a] = cand ? (fnext - A[a]) * inv[a] : INFINITY;
+            left[a] = dir[a] > 0 ? g.bmax[a] - c[a] : c[a] - g.bmin[a];
+            dlin[a] = dir[a] * stride[a];
         }
+        const double tie_thr = seg_len > 0.0 ? g.tie_eps / seg_len : 0.0;
         int lin = c[0] + g.nx * (c[1] + g.ny * c[2]);
         while (hull[lin] == 0) {
-            // candidates = axes on which B lies strictly beyond the next face (B outside closed box(c) on that axis)
-            bool cand[3];
-            int best = -1;
-            double sb = 0.0;
-#pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                cand[a] = dir[a] > 0 ? B[a] > fnext[a] : (dir[a] < 0 ? B[a] < fnext[a] : false);
-                if (cand[a] && (best < 0 || sn[a] < sb)) { best = a; sb = sn[a]; }
+            int best = 0;
+            double sb = se[0];
+            if (se[1] < sb) { best = 1; sb = se[1]; }                       // strict: x before y before z on equality
+            if (se[2] < sb) { best = 2; sb = se[2]; }
+            if (sb == INFINITY) return;                                     // chord ends without meeting the hull
+            if ((best != 0 && se[0] - sb < tie_thr) || (best != 1 && se[1] - sb < tie_thr) || (best != 2 && se[2] - sb < tie_thr)) hit.tie = true;
+#define PCT_HULL_MOVE(a)                                                                                       \
+            {                                                                                                  \
+                c[a] += dir[a];                                                                                \
+                if (--left[a] < 0) return;                     /* left the hull's bounding box: miss */         \
+                lin += dlin[a];                                                                                \
+                const double fnext = face_coord(g, a, c[a] + (dir[a] > 0 ? 1 : 0));                            \
+                const bool cand = dir[a] > 0 ? B[a] > fnext : B[a] < fnext;                                    \
+                se[a] = cand ? (fnext - A[a]) * inv[a] : INFINITY;                                             \
+                last.axis = a; last.dir = dir[a];                                                              \
             }
-            if (best < 0) return;                                           // chord ends without meeting the hull
-#pragma unroll
-            for (int a = 0; a < 3; ++a)
-                if (a != best && cand[a] && (sn[a] - sb) * seg_len < g.tie_eps) hit.tie = true;
-#pragma unroll
-            for (int a = 0; a < 3; ++a)
-                if (a == best) {
-                    c[a] += dir[a];
-                    if (c[a] < g.bmin[a] || c[a] > g.bmax[a]) return;       // left the hull's bounding box: miss
-                    lin += dir[a] * stride[a];
-                    fnext[a] = face_coord(g, a, c[a] + (dir[a] > 0 ? 1 : 0));
-                    sn[a] = (fnext[a] - A[a]) * inv[a];
-                    last.axis = a; last.dir = dir[a];
-                }
+            if (best == 0) PCT_HULL_MOVE(0)
+            else if (best == 1) PCT_HULL_MOVE(1)
+            else PCT_HULL_MOVE(2)
+#undef PCT_HULL_MOVE
         }
         if (last.axis >= 0) {
 #pragma unroll
