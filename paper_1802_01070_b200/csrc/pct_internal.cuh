@@ -82,12 +82,12 @@ __host__ __device__ __forceinline__ int plan_nbase(const PlanGroup& g, int r) { 
 __host__ __device__ __forceinline__ int plan_zbase(const PlanGroup& g, int r) { return (int)(((long long)g.zb0 + (long long)r * g.sz) >> 16); }
 
 // Packed window coordinate of a visit = byte offset of its 4-byte slot: (n mod 32) << 2 | (row mod 16) << 7 |
-// (z mod 16) << 11.  The shared-memory address XORs the row and the two low bits of z into the n field: the lanes of a
+// (z mod 16) << 11.  The shared-memory address XORs the row and the low bit of z into the n field (one shift, one LOP3): the lanes of a
 // warp sit in the same few rows but in different (n, z) columns of the tube, so the bank must depend on n AND z.
 __host__ __device__ __forceinline__ unsigned win_pack(int n, int r, int z) {
     return ((unsigned)(n & (WIN_N - 1)) << 2) | ((unsigned)(r & (SLAB - 1)) << 7) | ((unsigned)(z & (WIN_Z - 1)) << 11);
 }
-__host__ __device__ __forceinline__ unsigned win_addr(unsigned p) { return p ^ ((p >> 5) & 0x3Cu) ^ ((p >> 6) & 0x60u); }
+__host__ __device__ __forceinline__ unsigned win_addr(unsigned p) { return p ^ ((p >> 5) & 0x7Cu); }
 
 struct SolvePlan {
     int64_t block_size, n_blocks, n_groups, n_direct, cnt_bytes;

@@ -46,7 +46,7 @@ __device__ __forceinline__ void for_visited_slots(const PlanGroup& G, const Colu
 #pragma unroll
     for (int k = 0; k < STAGE_Z; ++k) {
         const int o = (zq0 + 2 * k - col.zb) & (WIN_Z - 1);
-        if (o >= G.dz_lo && o <= G.dz_hi) f(k, col.zb + o, (col_addr ^ ((k & 1) ? 0x40u : 0u)) + (unsigned)k * 4096u);   // z bit 1 enters the bank swizzle
+        if (o >= G.dz_lo && o <= G.dz_hi) f(k, col.zb + o, col_addr + (unsigned)k * 4096u);   // z bit 1 enters the bank swizzle
     }
 }
 
