@@ -15,7 +15,11 @@
 
 namespace pct {
 
-constexpr int K2W_SMEM = WIN_SLOTS * 8;      // pass 1: float x[8192] in the first half; pass 2: int Delta[8192], uint s[8192]
+// pass 1: two float x[8192] buffers; pass 2: int Delta[8192], uint s[8192] (or a second Delta copy).  The 64 KB window is
+// aligned to 32 KB inside the allocation so that a thread's packed coordinate can carry the window's shared address in
+// its upper bits (field arithmetic touches bits 2-14 only): no base addition per visit.
+constexpr int K2W_WIN = WIN_SLOTS * 8;
+constexpr int K2W_SMEM = K2W_WIN + 32768;
 constexpr int FIX_BITS = 17;                 // |c_i| 2^e < 2^17; <= MAX_ROW_VISITS * GROUP = 6144 additions per slot < 2^31
 
 __device__ __forceinline__ void red_add_v2_w(float2* p, float a, float b) {
@@ -144,7 +148,9 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
         n_vis = N[i];
         p_init = p0[G.start + rk];
     }
-    const unsigned win_s = (unsigned)__cvta_generic_to_shared(smem), tbl_s = (unsigned)__cvta_generic_to_shared(tbl);
+    const unsigned raw_s = (unsigned)__cvta_generic_to_shared(smem), tbl_s = (unsigned)__cvta_generic_to_shared(tbl);
+    const unsigned win_s = (raw_s + 0x7FFFu) & ~0x7FFFu;                      // 32 KB aligned
+    unsigned char* const win = smem + (win_s - raw_s);
     const uint8_t* my_cnt = cnt + G.cnt_off + tid;
     const unsigned long long* my_stream = stream + G.stream_off + tid;
     // this thread's window column for staging / flushing
@@ -164,7 +170,7 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
             cp_async_f32(dst + off, x + (valid ? col.base + z * wg.stride_z : 0), valid);
         });
     };
-    unsigned p = p_init;
+    unsigned p = win_s + p_init;                  // window address + packed coordinate; starts in x buffer 0
     float S = 0.f;
     stage(0);
     unsigned long long w_next = __ldg(my_stream);
@@ -178,8 +184,8 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
             w_next = __ldg(my_stream + (size_t)(s + 1) * G.wps * GROUP);
         }
         const int cmax = __reduce_max_sync(0xffffffffu, c);
-        const unsigned xs = win_s + (unsigned)(s & 1) * (WIN_SLOTS * 4);
-        walk_slab(my_stream + (size_t)s * G.wps * GROUP, w0, cmax, tbl_s, p, [&](unsigned q) { S += lds_f32(xs + win_addr(q)); });
+        if (s > 0) p += (s & 1) ? 0x8000u : 0xFFFF8000u;          // switch to the other x buffer (the fields sit below bit 15)
+        walk_slab(my_stream + (size_t)s * G.wps * GROUP, w0, cmax, tbl_s, p, [&](unsigned q) { S += lds_f32(win_addr(q)); });
     }
     // ---- c_i and the CTA's fixed-point scale (R17, R21) -----------------------------------------------------------------
     float ci = 0.f;
@@ -192,7 +198,7 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
     for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
     __syncthreads();                              // all walkers done with xs
     if ((tid & 31) == 0) red[tid >> 5] = mx;
-    int* dl = reinterpret_cast<int*>(smem);
+    int* dl = reinterpret_cast<int*>(win);
 #pragma unroll
     for (int k = 0; k < 2 * WIN_SLOTS / GROUP; ++k) dl[tid + k * GROUP] = 0;      // clears Delta and s
     __syncthreads();
@@ -205,7 +211,7 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
     const int cfix = __float2int_rn(ci * scale);
 
     // ---- pass 2: {Delta, s} += {c_i, 1} on every visit; flush per slab -------------------------------------------------
-    p = p_init;
+    p = win_s + p_init + (COUNT ? 0u : (unsigned)(tid & 1) * (WIN_SLOTS * 4));     // odd lanes: second Delta copy
     w_next = __ldg(my_stream);
     for (int s = 0; s < G.nslab; ++s) {
         const int c = (int)my_cnt[(size_t)s * GROUP];
@@ -214,20 +220,19 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
         if (s + 1 < G.nslab) w_next = __ldg(my_stream + (size_t)(s + 1) * G.wps * GROUP);
         if (COUNT) {
             walk_slab(my_stream + (size_t)s * G.wps * GROUP, w0, cmax, tbl_s, p, [&](unsigned q) {
-                const unsigned a = win_s + win_addr(q);
+                const unsigned a = win_addr(q);
                 atoms_add(a, cfix);
                 atoms_inc(a + WIN_SLOTS * 4);
             });
         } else {
-            const unsigned copy = win_s + (unsigned)(tid & 1) * (WIN_SLOTS * 4);
-            walk_slab(my_stream + (size_t)s * G.wps * GROUP, w0, cmax, tbl_s, p, [&](unsigned q) { atoms_add(copy + win_addr(q), cfix); });
+            walk_slab(my_stream + (size_t)s * G.wps * GROUP, w0, cmax, tbl_s, p, [&](unsigned q) { atoms_add(win_addr(q), cfix); });
         }
         __syncthreads();
         {
             const Column col = slab_column(G, wg, s, col_nq, col_ml);
             for_visited_slots(G, col, col_zq0, col_addr, [&](int, int z, unsigned a) {
-                int* d0 = reinterpret_cast<int*>(smem + a);
-                unsigned* d1 = reinterpret_cast<unsigned*>(smem + WIN_SLOTS * 4 + a);
+                int* d0 = reinterpret_cast<int*>(win + a);
+                unsigned* d1 = reinterpret_cast<unsigned*>(win + WIN_SLOTS * 4 + a);
                 if (COUNT) {
                     const unsigned cs = *d1;
                     if (cs != 0u) {                   // a touched slot is a verified visit: it lies inside the grid
