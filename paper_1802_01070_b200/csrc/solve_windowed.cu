@@ -95,7 +95,7 @@ __device__ __forceinline__ void walk_slab(const unsigned long long* __restrict__
                 const unsigned code4 = (unsigned)(w >> (3 * k)) << 2 & 0x1Cu;
                 const unsigned t = lds_u32(tbl_s + code4);              // delta | mask << 16; 0 = pad
                 const unsigned fm = t >> 16;
-                p = ((p + (t & 0xFFFFu)) & fm) | (p & ~fm);
+                p = ((p + t) & fm) | (p & ~fm);                        // the mask half of t is discarded by the select
                 if (t != 0u) visit(p);
             }
         }
