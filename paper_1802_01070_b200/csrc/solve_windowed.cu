@@ -42,15 +42,18 @@ struct Column {
     int on;          // n offset of the column from the row's window base
 };
 
-// Calls f(k, z, byte offset of the slot) for the slots of a thread's column that the group's members can visit
-// (PlanGroup::dn_*, dz_*): slot k of the column holds z with (z mod 16) = zq0 + 2k.
+// Calls f(z, byte offset of the slot) for the slots of a thread's column that the group's members can visit
+// (PlanGroup::dn_*, dz_*) and that lie inside the grid.  The thread owns the slots of one parity of z; col_a0 = window
+// offset of the column for z = 0 (the swizzle only involves the parity of z, a thread constant).
 template <typename F>
-__device__ __forceinline__ void for_visited_slots(const PlanGroup& G, const Column& col, int zq0, unsigned col_addr, F&& f) {
-    if (col.on < G.dn_lo || col.on > G.dn_hi) return;
-#pragma unroll
-    for (int k = 0; k < STAGE_Z; ++k) {
-        const int o = (zq0 + 2 * k - col.zb) & (WIN_Z - 1);
-        if (o >= G.dz_lo && o <= G.dz_hi) f(k, col.zb + o, col_addr + (unsigned)k * 4096u);   // z bit 1 enters the bank swizzle
+__device__ __forceinline__ void for_visited_slots(const PlanGroup& G, const Column& col, int zq0, unsigned col_a0, int dim_z, F&& f) {
+    if (col.base < 0 || col.on < G.dn_lo || col.on > G.dn_hi) return;
+    const int o0 = (zq0 - col.zb) & 1;                                   // this thread's offsets from zb: o0, o0 + 2, ...
+    const int lo = max(G.dz_lo, -col.zb), hi = min(G.dz_hi, dim_z - 1 - col.zb);
+    const int k_hi = min(STAGE_Z - 1, (hi - o0) >> 1);
+    for (int k = max(0, (lo - o0 + 1) >> 1); k <= k_hi; ++k) {
+        const int z = col.zb + o0 + 2 * k;
+        f(z, col_a0 + ((unsigned)(z & (WIN_Z - 1)) << 11));
     }
 }
 
@@ -157,7 +160,7 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
     const int col_nq = wg.x_major ? (tid >> 4) & (WIN_N - 1) : tid & (WIN_N - 1);
     const int col_ml = wg.x_major ? tid & (SLAB - 1) : (tid >> 5) & (SLAB - 1);
     const int col_zq0 = tid >> 9;                                            // 0 or 1; slots zq0 + 2k
-    const unsigned col_addr = win_addr(win_pack(col_nq, col_ml, col_zq0));    // slot k: (col_addr ^ swizzle of z bit 1) + k * 4096
+    const unsigned col_a0 = win_addr(win_pack(col_nq, col_ml, col_zq0)) - ((unsigned)col_zq0 << 11);   // the column's slot for z = 0
 
     // ---- pass 1: S_i = sum of x over the visits ----------------------------------------------------------------------
     // The x window is double buffered in the two halves of the shared window (pass 1 needs 32 KB of the 64 KB): slab
@@ -165,9 +168,8 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
     auto stage = [&](int s) {
         const Column col = slab_column(G, wg, s, col_nq, col_ml);
         const unsigned dst = win_s + (unsigned)(s & 1) * (WIN_SLOTS * 4);
-        for_visited_slots(G, col, col_zq0, col_addr, [&](int, int z, unsigned off) {
-            const bool valid = col.base >= 0 && (unsigned)z < (unsigned)wg.dim_z;
-            cp_async_f32(dst + off, x + (valid ? col.base + z * wg.stride_z : 0), valid);
+        for_visited_slots(G, col, col_zq0, col_a0, wg.dim_z, [&](int z, unsigned off) {
+            cp_async_f32(dst + off, x + (col.base + z * wg.stride_z), true);
         });
     };
     unsigned p = win_s + p_init;                  // window address + packed coordinate; starts in x buffer 0
@@ -230,7 +232,7 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
         __syncthreads();
         {
             const Column col = slab_column(G, wg, s, col_nq, col_ml);
-            for_visited_slots(G, col, col_zq0, col_addr, [&](int, int z, unsigned a) {
+            for_visited_slots(G, col, col_zq0, col_a0, wg.dim_z, [&](int z, unsigned a) {
                 int* d0 = reinterpret_cast<int*>(win + a);
                 unsigned* d1 = reinterpret_cast<unsigned*>(win + WIN_SLOTS * 4 + a);
                 if (COUNT) {
