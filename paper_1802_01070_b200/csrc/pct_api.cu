@@ -1,4 +1,5 @@
 // pct_api.cu -- the extern "C" boundary of libpct.so (include/pct.h) and the iteration driver (A8).
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -165,7 +166,7 @@ int pct_create(const pct_geometry* geom, const pct_mlp_params* params, int devic
 void pct_destroy(pct_ctx* ctx) {
     if (!ctx) return;
     DeviceGuard guard(ctx->device);
-    cudaFree(ctx->ds); cudaFree(ctx->dsum); cudaFree(ctx->scan_tmp); cudaFree(ctx->logk); cudaFree(ctx->gen_scratch); cudaFree(ctx->d_stats); cudaFree(ctx->d_total);
+    cudaFree(ctx->ds); cudaFree(ctx->dsum); cudaFree(ctx->counts_buf); cudaFree(ctx->scan_tmp); cudaFree(ctx->logk); cudaFree(ctx->gen_scratch); cudaFree(ctx->d_stats); cudaFree(ctx->d_total);
     for (auto& v : ctx->prof_events) { if (v) { for (cudaEvent_t e : *v) cudaEventDestroy(e); delete v; } }
     if (ctx->prof_pool) { for (cudaEvent_t e : *ctx->prof_pool) cudaEventDestroy(e); delete ctx->prof_pool; }
     delete ctx;
@@ -292,7 +293,7 @@ int pct_plan_info(const pct_paths* P, pct_plan_stats* out) {
     const SolvePlan* pl = P->plan;
     if (!pl) return PCT_OK;
     out->block_size = pl->block_size; out->n_blocks = pl->n_blocks; out->n_groups = pl->n_groups; out->n_direct = pl->n_direct;
-    out->plan_bytes = (pl->counts ? 4 * pl->n_blocks * P->n_vox : 0) + pl->cnt_bytes + 8 * pl->stream_words + P->m * 13 + (pl->n_groups + 1) * (int64_t)sizeof(PlanGroup) + pl->n_blocks * 4;
+    out->plan_bytes = pl->cnt_bytes + 8 * pl->stream_words + P->m * 13 + (pl->n_groups + 1) * (int64_t)sizeof(PlanGroup) + pl->n_blocks * 4;
     return PCT_OK;
 }
 
@@ -374,13 +375,35 @@ int pct_solve(pct_ctx* ctx, const pct_paths* P, const float* b, const float* x0,
         }
         plan = Pm->plan;
     }
+    // count cache (R23): one buffer per context, owned by the plan that filled it last
+    uint32_t* plan_counts = nullptr;
+    if (plan) {
+        const size_t need = 4 * (size_t)plan->n_blocks * (size_t)ctx->n_vox;
+        if (need > ctx->counts_cap) {
+            size_t free_b = 0, total_b = 0;
+            if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && need <= (free_b + ctx->counts_cap) / 4 && need <= ((size_t)32 << 30)) {
+                PCT_CUDA(ctx, cudaStreamSynchronize(st));
+                cudaFree(ctx->counts_buf);
+                ctx->counts_buf = nullptr; ctx->counts_cap = 0; ctx->counts_owner = nullptr;
+                if (cudaMalloc(&ctx->counts_buf, need) == cudaSuccess) ctx->counts_cap = need;
+                else cudaGetLastError();
+            }
+        }
+        if (need <= ctx->counts_cap) {
+            if (ctx->counts_owner != plan) {
+                std::fill(const_cast<SolvePlan*>(plan)->counts_ready.begin(), const_cast<SolvePlan*>(plan)->counts_ready.end(), (uint8_t)0);
+                ctx->counts_owner = plan;
+            }
+            plan_counts = ctx->counts_buf;
+        }
+    }
     for (int it = 0; it < iters; ++it) {
         for (int64_t t = 0, i0 = 0; i0 < P->m; i0 += block_size, ++t) {
             const int64_t i1 = (P->m - i0) < block_size ? P->m : i0 + block_size;
             if (plan) {
                 // s_j^t does not depend on x (R15): the first sweep over block t counts and stores it, later sweeps
                 // (and later calls with the same paths and block size) accumulate Delta only
-                uint32_t* counts = plan->counts ? plan->counts + (size_t)t * (size_t)ctx->n_vox : nullptr;
+                uint32_t* counts = plan_counts ? plan_counts + (size_t)t * (size_t)ctx->n_vox : nullptr;
                 const bool cached = counts && plan->counts_ready[(size_t)t];
                 if ((rc = launch_block_windowed(ctx, P, plan, t, !cached, b, x_out, ctx->ds, ctx->dsum, st)) != PCT_OK) return rc;
                 const int64_t nd = plan->direct_count[(size_t)t];

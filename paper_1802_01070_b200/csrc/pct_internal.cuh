@@ -95,8 +95,7 @@ struct SolvePlan {
     uint32_t* p0;            // packed window coordinate of the first visit, per sorted position
     uint8_t* pflag;          // per sorted position: 1 = windowed, 0 = not (rejected, or listed in direct_list)
     uint8_t* cnt;            // visits per (group, slab, thread)
-    uint32_t* counts;        // cache of s_j^t: n_blocks x n_vox (nullptr if it would not fit the budget)
-    std::vector<uint8_t> counts_ready;   // per block (host): filled by the first sweep that ran with this plan
+    std::vector<uint8_t> counts_ready;   // per block (host): s^t of that block is in the context's count cache
     unsigned long long* stream;   // slab-aligned copy of the windowed histories' codes (21 codes per word)
     int64_t stream_words;
     PlanGroup* groups;
@@ -122,6 +121,9 @@ struct pct_ctx {
     int solve_mode;      // 0 auto, 1 direct kernel only, 2 windowed plan whenever possible (pct_solve_config)
     int64_t solve_min_block;  // auto: blocks smaller than this take the direct kernel
     float2* ds;          // {Delta_j, s_j} accumulator, n_vox
+    uint32_t* counts_buf;     // cache of s_j^t, n_blocks x n_vox, of the plan `counts_owner` (one buffer per context, grown
+    size_t counts_cap;        // on demand and kept: a multi-GB allocation per reconstruction is not free)
+    const void* counts_owner;
     float* dsum;         // Delta_j accumulator used when the block's counts are cached, n_vox
     int64_t ds_cap;
     void* scan_tmp;      // block sums for scans

@@ -17,6 +17,10 @@
 //                       A history that fails is appended to its block's direct list.
 // Correctness of the solver never depends on the sort or the centre-line fit: a history is either verified to stay
 // in its group's window or it takes the direct kernel.
+#include <chrono>
+#include <cstdio>
+#include <cstdlib>
+
 #include <cub/device/device_radix_sort.cuh>
 
 #include "pct_internal.cuh"
@@ -329,7 +333,7 @@ __global__ void k_plan_work_keys(const PlanGroup* __restrict__ groups, const uin
 
 void free_solve_plan(SolvePlan* plan) {
     if (!plan) return;
-    cudaFree(plan->perm); cudaFree(plan->p0); cudaFree(plan->pflag); cudaFree(plan->cnt); cudaFree(plan->groups); cudaFree(plan->stream); cudaFree(plan->counts); cudaFree(plan->launch_order);
+    cudaFree(plan->perm); cudaFree(plan->p0); cudaFree(plan->pflag); cudaFree(plan->cnt); cudaFree(plan->groups); cudaFree(plan->stream); cudaFree(plan->launch_order);
     cudaFree(plan->direct_list); cudaFree(plan->d_direct_count);
     delete plan;
 }
@@ -343,7 +347,7 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     if (!plan) return set_error(ctx, PCT_E_OOM, "host allocation");
     plan->block_size = block_size; plan->n_blocks = n_blocks; plan->n_groups = 0; plan->n_direct = 0; plan->cnt_bytes = 0;
     plan->perm = nullptr; plan->p0 = nullptr; plan->pflag = nullptr; plan->cnt = nullptr; plan->groups = nullptr;
-    plan->direct_list = nullptr; plan->d_direct_count = nullptr; plan->stream = nullptr; plan->stream_words = 0; plan->counts = nullptr; plan->launch_order = nullptr;
+    plan->direct_list = nullptr; plan->d_direct_count = nullptr; plan->stream = nullptr; plan->stream_words = 0; plan->launch_order = nullptr;
     uint64_t *keysA = nullptr, *keysB = nullptr, *cnt_off = nullptr;
     uint32_t *valsA = nullptr, *valsB = nullptr, *cnt_len = nullptr;
     void* tmp = nullptr;
@@ -358,6 +362,15 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { cudaGetLastError();                               \
         return fail(set_error(ctx, e__ == cudaErrorMemoryAllocation ? PCT_E_OOM : PCT_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e__))); } } while (0)
     const size_t mm = (size_t)m;
+    const bool dbg = getenv("PCT_PLAN_DEBUG") != nullptr;
+    auto t_last = std::chrono::steady_clock::now();
+    auto lap = [&](const char* what) {
+        if (!dbg) return;
+        cudaStreamSynchronize(st);
+        const auto now = std::chrono::steady_clock::now();
+        fprintf(stderr, "[plan] %-28s %8.2f ms\n", what, std::chrono::duration<double, std::milli>(now - t_last).count());
+        t_last = now;
+    };
     PLAN_CUDA(cudaMallocAsync(&keysA, 8 * mm, st)); PLAN_CUDA(cudaMallocAsync(&keysB, 8 * mm, st));
     PLAN_CUDA(cudaMallocAsync(&valsA, 4 * mm, st)); PLAN_CUDA(cudaMallocAsync(&valsB, 4 * mm, st));
     const unsigned nb256 = (unsigned)((m + 255) / 256);
@@ -377,6 +390,7 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     uint32_t* head = dv.Alternate();           // reused: head flags
     plan->perm = dv.Current();
     if (plan->perm == valsA) valsA = nullptr; else valsB = nullptr;   // ownership moved to the plan
+    lap("keys + sort");
     k_plan_heads<<<nb256, 256, 0, st>>>(keys, m, head);
     ++ctx->launches;
     PLAN_CUDA(cudaGetLastError());
@@ -390,6 +404,7 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     PLAN_CUDA(cudaMallocAsync(&d_group_begin, sizeof(int64_t) * (size_t)(n_blocks + 1), st));
     PLAN_CUDA(cudaMallocAsync(&cnt_len, sizeof(uint32_t) * (size_t)n_groups, st));
     PLAN_CUDA(cudaMallocAsync(&cnt_off, sizeof(uint64_t) * (size_t)n_groups, st));
+    lap("heads + scan");
     k_plan_starts<<<nb256, 256, 0, st>>>(keys, head, gid, m, plan->groups, d_group_begin);
     k_plan_params<<<(unsigned)n_groups, 256, 0, st>>>(ctx->cfg, P->start, P->end, plan->perm, m, (int64_t)n_groups, plan->groups, cnt_len);
     ctx->launches += 2;
@@ -405,6 +420,7 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     PLAN_CUDA(cudaStreamSynchronize(st));
     cudaFree(keysA); cudaFree(keysB); cudaFree(valsA); cudaFree(valsB); cudaFree(tmp);
     keysA = keysB = nullptr; valsA = valsB = nullptr; tmp = nullptr;
+    lap("starts + params + cnt scan");
     PLAN_CUDA(cudaMallocAsync(&plan->cnt, cnt_bytes > 0 ? (size_t)cnt_bytes : 16, st));
     PLAN_CUDA(cudaMemsetAsync(plan->cnt, 0, cnt_bytes > 0 ? (size_t)cnt_bytes : 16, st));
     PLAN_CUDA(cudaMallocAsync(&plan->p0, 4 * mm, st));
@@ -412,11 +428,13 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     PLAN_CUDA(cudaMallocAsync(&plan->direct_list, 4 * mm, st));
     PLAN_CUDA(cudaMallocAsync(&plan->d_direct_count, sizeof(uint32_t) * (size_t)n_blocks, st));
     PLAN_CUDA(cudaMemsetAsync(plan->d_direct_count, 0, sizeof(uint32_t) * (size_t)n_blocks, st));
+    lap("allocs before verify");
     k_plan_verify<<<(unsigned)n_groups, GROUP, 0, st>>>(ctx->cfg, P->N, P->start, P->code_off, P->codes, plan->perm, plan->groups,
                                                        block_size, plan->p0, plan->pflag, plan->cnt, plan->direct_list,
                                                        plan->d_direct_count);
     ++ctx->launches;
     PLAN_CUDA(cudaGetLastError());
+    lap("verify");
     // slab-aligned code stream of the verified members
     k_plan_stream_len<<<(unsigned)((n_groups + 255) / 256), 256, 0, st>>>((int64_t)n_groups, plan->groups, cnt_len);
     if ((rc = launch_scan_u32(ctx, cnt_len, cnt_off, (int64_t)n_groups, 0, ctx->d_total, st)) != PCT_OK) return fail(rc);
@@ -427,10 +445,12 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     PLAN_CUDA(cudaMallocAsync(&plan->stream, stream_words > 0 ? 8 * (size_t)stream_words : 16, st));
     PLAN_CUDA(cudaMemsetAsync(plan->stream, 0xFF, stream_words > 0 ? 8 * (size_t)stream_words : 16, st));
     k_plan_stream_off<<<(unsigned)((n_groups + 255) / 256), 256, 0, st>>>(cnt_off, (int64_t)n_groups, plan->groups);
+    lap("stream alloc + memset");
     k_plan_emit<<<(unsigned)n_groups, GROUP, 0, st>>>(ctx->cfg, P->N, P->start, P->code_off, P->codes, plan->perm, plan->groups,
                                                      plan->pflag, plan->stream);
     ctx->launches += 3;
     PLAN_CUDA(cudaGetLastError());
+    lap("emit");
     {   // longest-first launch order inside every block
         uint64_t *wk0 = nullptr, *wk1 = nullptr;
         uint32_t *wv0 = nullptr, *wv1 = nullptr;
@@ -455,14 +475,8 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
 #undef WORK_CUDA
         ++ctx->launches;
     }
-    {   // cache of the per-block column counts, if it fits comfortably (a quarter of the free memory, at most 32 GiB)
-        size_t free_b = 0, total_b = 0;
-        const size_t need = 4 * (size_t)n_blocks * (size_t)P->n_vox;
-        if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && need <= free_b / 4 && need <= ((size_t)32 << 30)) {
-            if (cudaMallocAsync(&plan->counts, need, st) != cudaSuccess) { cudaGetLastError(); plan->counts = nullptr; }
-        }
-        plan->counts_ready.assign((size_t)n_blocks, 0);
-    }
+    lap("launch order");
+    plan->counts_ready.assign((size_t)n_blocks, 0);      // the count cache itself belongs to the context (pct_solve)
     plan->group_begin.resize((size_t)n_blocks + 1);
     plan->direct_count.resize((size_t)n_blocks);
     PLAN_CUDA(cudaMemcpyAsync(plan->group_begin.data(), d_group_begin, sizeof(int64_t) * (size_t)n_blocks, cudaMemcpyDeviceToHost, st));
