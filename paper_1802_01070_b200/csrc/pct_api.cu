@@ -51,7 +51,8 @@ struct DeviceGuard {
 };
 
 static void free_paths_arrays(pct_paths* P) {
-    cudaFree(P->N); cudaFree(P->start); cudaFree(P->end); cudaFree(P->ell); cudaFree(P->flags); cudaFree(P->code_off); cudaFree(P->codes);
+    cudaDeviceSynchronize();         // the buffers go back to the pool on the legacy stream: nothing may still use them
+    pool_free(P->N, 0); pool_free(P->start, 0); pool_free(P->end, 0); pool_free(P->ell, 0); pool_free(P->flags, 0); pool_free(P->code_off, 0); pool_free(P->codes, 0);
     if (P->plan) { free_solve_plan(P->plan); P->plan = nullptr; }
     P->N = nullptr; P->start = nullptr; P->end = nullptr; P->ell = nullptr; P->flags = nullptr; P->code_off = nullptr; P->codes = nullptr;
 }
@@ -81,7 +82,7 @@ static int ensure_codes(pct_ctx* ctx, pct_paths* P, int64_t need, cudaStream_t s
     if (P->chunks_used > 0)
         PCT_CUDA(ctx, cudaMemcpyAsync(fresh, P->codes, sizeof(ulonglong2) * (size_t)P->chunks_used, cudaMemcpyDeviceToDevice, st));
     PCT_CUDA(ctx, cudaStreamSynchronize(st));
-    if (P->codes) PCT_CUDA(ctx, cudaFree(P->codes));
+    if (P->codes) PCT_CUDA(ctx, pool_free(P->codes, st));
     P->codes = fresh;
     P->chunks_cap = cap;
     return PCT_OK;
@@ -234,7 +235,7 @@ int pct_generate_mlp(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hull, v
     ulonglong2* stage = nullptr;
     uint32_t* nchunks = nullptr;
     int rc = PCT_OK;
-    auto fail = [&](int code) { cudaFree(stage); cudaFree(nchunks); free_paths_arrays(P); delete P; return code; };
+    auto fail = [&](int code) { pool_free(stage, st); pool_free(nchunks, st); free_paths_arrays(P); delete P; return code; };
 #define GEN_CUDA(call)                                                                                          \
     do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { cudaGetLastError();                               \
         return fail(set_error(ctx, e__ == cudaErrorMemoryAllocation ? PCT_E_OOM : PCT_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e__))); } } while (0)
@@ -273,7 +274,7 @@ int pct_generate_mlp(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hull, v
     GEN_CUDA(cudaMemcpyAsync(&hs, ctx->d_stats, sizeof(hs), cudaMemcpyDeviceToHost, st));
     GEN_CUDA(cudaStreamSynchronize(st));
 #undef GEN_CUDA
-    cudaFree(stage); cudaFree(nchunks);
+    pool_free(stage, st); pool_free(nchunks, st);
     P->total_visits = (int64_t)hs.total_visits; P->n_rejected = (int64_t)hs.n_rejected; P->total_samples = (int64_t)hs.total_samples; P->n_ties = (int64_t)hs.n_ties;
     *out = P;
     return PCT_OK;
@@ -440,7 +441,7 @@ int pct_reconstruct_host(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hul
     auto cleanup = [&]() {
         ctx->batch_ready = nullptr; ctx->n_batch_ready = 0;
         if (cs) cudaStreamSynchronize(cs);
-        cudaFree(d_tr); cudaFree(d_b); cudaFree(d_x); cudaFree(d_hull);
+        pool_free(d_tr, st); pool_free(d_b, st); pool_free(d_x, st); pool_free(d_hull, st);
         if (P) pct_paths_free(P);
         for (auto& e : ev) if (e) cudaEventDestroy(e);
         for (auto& e : ready) if (e) cudaEventDestroy(e);

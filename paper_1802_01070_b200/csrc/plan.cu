@@ -333,8 +333,9 @@ __global__ void k_plan_work_keys(const PlanGroup* __restrict__ groups, const uin
 
 void free_solve_plan(SolvePlan* plan) {
     if (!plan) return;
-    cudaFree(plan->perm); cudaFree(plan->p0); cudaFree(plan->pflag); cudaFree(plan->cnt); cudaFree(plan->groups); cudaFree(plan->stream); cudaFree(plan->launch_order);
-    cudaFree(plan->direct_list); cudaFree(plan->d_direct_count);
+    cudaDeviceSynchronize();         // freed on the legacy stream: nothing may still use the plan
+    pool_free(plan->perm, 0); pool_free(plan->p0, 0); pool_free(plan->pflag, 0); pool_free(plan->cnt, 0); pool_free(plan->groups, 0); pool_free(plan->stream, 0); pool_free(plan->launch_order, 0);
+    pool_free(plan->direct_list, 0); pool_free(plan->d_direct_count, 0);
     delete plan;
 }
 
@@ -353,8 +354,8 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     void* tmp = nullptr;
     int64_t* d_group_begin = nullptr;
     auto fail = [&](int code) {
-        cudaFree(keysA); cudaFree(keysB); cudaFree(valsA); cudaFree(valsB); cudaFree(tmp); cudaFree(cnt_off); cudaFree(cnt_len);
-        cudaFree(d_group_begin);
+        pool_free(keysA, st); pool_free(keysB, st); pool_free(valsA, st); pool_free(valsB, st); pool_free(tmp, st); pool_free(cnt_off, st); pool_free(cnt_len, st);
+        pool_free(d_group_begin, st);
         free_solve_plan(plan);
         return code;
     };
@@ -368,7 +369,15 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
         if (!dbg) return;
         cudaStreamSynchronize(st);
         const auto now = std::chrono::steady_clock::now();
-        fprintf(stderr, "[plan] %-28s %8.2f ms\n", what, std::chrono::duration<double, std::milli>(now - t_last).count());
+        unsigned long long reserved = 0, used = 0, thr = 0;
+        cudaMemPool_t pool;
+        if (cudaDeviceGetMemPool(&pool, ctx->device) == cudaSuccess) {
+            cudaMemPoolGetAttribute(pool, cudaMemPoolAttrReservedMemCurrent, &reserved);
+            cudaMemPoolGetAttribute(pool, cudaMemPoolAttrUsedMemCurrent, &used);
+            cudaMemPoolGetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+        }
+        fprintf(stderr, "[plan] %-28s %8.2f ms   pool reserved %.2f GB used %.2f GB thr %.3g\n", what,
+                std::chrono::duration<double, std::milli>(now - t_last).count(), reserved / 1e9, used / 1e9, (double)thr);
         t_last = now;
     };
     PLAN_CUDA(cudaMallocAsync(&keysA, 8 * mm, st)); PLAN_CUDA(cudaMallocAsync(&keysB, 8 * mm, st));
@@ -418,7 +427,7 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     ++ctx->launches;
     // the sort buffers are no longer needed once the group table is complete
     PLAN_CUDA(cudaStreamSynchronize(st));
-    cudaFree(keysA); cudaFree(keysB); cudaFree(valsA); cudaFree(valsB); cudaFree(tmp);
+    pool_free(keysA, st); pool_free(keysB, st); pool_free(valsA, st); pool_free(valsB, st); pool_free(tmp, st);
     keysA = keysB = nullptr; valsA = valsB = nullptr; tmp = nullptr;
     lap("starts + params + cnt scan");
     PLAN_CUDA(cudaMallocAsync(&plan->cnt, cnt_bytes > 0 ? (size_t)cnt_bytes : 16, st));
@@ -456,7 +465,7 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
         uint32_t *wv0 = nullptr, *wv1 = nullptr;
         void* wtmp = nullptr;
         const size_t ng = (size_t)n_groups;
-        auto wfree = [&]() { cudaFree(wk0); cudaFree(wk1); cudaFree(wv0); cudaFree(wv1); cudaFree(wtmp); };
+        auto wfree = [&]() { pool_free(wk0, st); pool_free(wk1, st); pool_free(wv0, st); pool_free(wv1, st); pool_free(wtmp, st); };
 #define WORK_CUDA(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { cudaGetLastError(); wfree(); \
         return fail(set_error(ctx, e__ == cudaErrorMemoryAllocation ? PCT_E_OOM : PCT_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e__))); } } while (0)
         WORK_CUDA(cudaMallocAsync(&wk0, 8 * ng, st)); WORK_CUDA(cudaMallocAsync(&wk1, 8 * ng, st));
@@ -484,7 +493,7 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     PLAN_CUDA(cudaStreamSynchronize(st));
     plan->group_begin[(size_t)n_blocks] = (int64_t)n_groups;
     for (uint32_t c : plan->direct_count) plan->n_direct += c;
-    cudaFree(cnt_off); cudaFree(cnt_len); cudaFree(d_group_begin);
+    pool_free(cnt_off, st); pool_free(cnt_len, st); pool_free(d_group_begin, st);
 #undef PLAN_CUDA
     *out = plan;
     return PCT_OK;
