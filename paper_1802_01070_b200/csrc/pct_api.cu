@@ -372,7 +372,9 @@ int pct_solve(pct_ctx* ctx, const pct_paths* P, const float* b, const float* x0,
         if (Pm->plan && Pm->plan->block_size != block_size) { free_solve_plan(Pm->plan); Pm->plan = nullptr; }
         if (!Pm->plan) {
             ProfScope prof(ctx, 4, st);
-            if ((rc = build_solve_plan(ctx, P, block_size, st, &Pm->plan)) != PCT_OK) return rc;
+            rc = build_solve_plan(ctx, P, block_size, st, &Pm->plan);
+            if (rc == PCT_E_OOM) { Pm->plan = nullptr; cudaGetLastError(); }      // no room for the plan: direct kernels
+            else if (rc != PCT_OK) return rc;
         }
         plan = Pm->plan;
     }
