@@ -65,6 +65,8 @@ struct PlanGroup {
     // part of the window the verified members actually visit, as offsets from the row's window base (k_plan_verify):
     // n - nbase(r) in [dn_lo, dn_hi], z - zbase(r) in [dz_lo, dz_hi].  Only that part is staged and flushed.
     int32_t dn_lo, dn_hi, dz_lo, dz_hi;
+    int32_t max_cnt;     // largest number of visits one window slot of this group receives in a slab, measured by the first
+                         // (counting) sweep; 0 = not measured yet.  Bounds the additions per slot of the fixed-point Delta.
 };
 
 // thread -> rank of its history in the group's sorted order.  Transposed on purpose: the lanes of a warp take

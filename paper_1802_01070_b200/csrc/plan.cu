@@ -125,7 +125,7 @@ k_plan_params(const __grid_constant__ DevCfg g, const int32_t* __restrict__ star
     const uint32_t size = (uint32_t)(((gi + 1 < n_groups) ? (int64_t)groups[gi + 1].start : m) - (int64_t)G.start);
     if (G.cls == 7) {
         if (threadIdx.x == 0) { G.size = size; G.nslab = 0; G.m_first = 0; G.nb0 = G.zb0 = G.sn = G.sz = 0; G.wps = 0; G.cnt_off = G.stream_off = 0;
-                                G.dn_lo = G.dz_lo = 0; G.dn_hi = G.dz_hi = -1; groups[gi] = G; cnt_len[gi] = 0; }
+                                G.dn_lo = G.dz_lo = 0; G.dn_hi = G.dz_hi = -1; G.max_cnt = 0; groups[gi] = G; cnt_len[gi] = 0; }
         return;
     }
     const int dir = (G.cls & 1) ? -1 : 1;
@@ -167,6 +167,7 @@ k_plan_params(const __grid_constant__ DevCfg g, const int32_t* __restrict__ star
     G.wps = 0;               // k_plan_verify collects the largest visits-per-slab here
     G.cnt_off = G.stream_off = 0;
     G.dn_lo = WIN_N; G.dn_hi = -1; G.dz_lo = WIN_Z; G.dz_hi = -1;      // empty; k_plan_verify widens them
+    G.max_cnt = 0;
     groups[gi] = G;
     cnt_len[gi] = (uint32_t)G.nslab * GROUP;
 }

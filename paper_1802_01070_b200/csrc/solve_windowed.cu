@@ -20,7 +20,9 @@ namespace pct {
 // its upper bits (field arithmetic touches bits 2-14 only): no base addition per visit.
 constexpr int K2W_WIN = WIN_SLOTS * 8;
 constexpr int K2W_SMEM = K2W_WIN + 32768;
-constexpr int FIX_BITS = 17;                 // |c_i| 2^e < 2^17; <= MAX_ROW_VISITS * GROUP = 6144 additions per slot < 2^31
+// Fixed-point Delta (R21): |c_i| 2^e < 2^FIX and at most A additions per slot must satisfy A 2^FIX < 2^31.  The counting
+// sweep only knows A <= MAX_ROW_VISITS * GROUP = 6144 (FIX = 17) and measures the true maximum; later sweeps use it.
+constexpr int FIX_BITS = 17;
 
 __device__ __forceinline__ void red_add_v2_w(float2* p, float a, float b) {
     asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(a), "f"(b) : "memory");
@@ -114,7 +116,7 @@ __global__ void __launch_bounds__(GROUP, 2)
 k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, const float* __restrict__ ell,
                  const uint32_t* __restrict__ perm, const uint32_t* __restrict__ p0, const uint8_t* __restrict__ pflag,
                  const uint8_t* __restrict__ cnt, const unsigned long long* __restrict__ stream,
-                 const PlanGroup* __restrict__ groups, const uint32_t* __restrict__ launch_order, int64_t group0, const float* __restrict__ b, const float* __restrict__ x,
+                 PlanGroup* __restrict__ groups, const uint32_t* __restrict__ launch_order, int64_t group0, const float* __restrict__ b, const float* __restrict__ x,
                  float2* __restrict__ ds, float* __restrict__ dsum) {
     extern __shared__ __align__(16) unsigned char smem[];
     __shared__ unsigned tbl[8];
@@ -209,7 +211,10 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
     for (int k = 1; k < GROUP / 32; ++k) mx = fmaxf(mx, red[k]);
     int ex = 0;
     if (mx > 0.f && mx < INFINITY) frexpf(mx, &ex);              // mx < 2^ex
-    const float scale = exp2f((float)(FIX_BITS - ex)), inv_scale = exp2f((float)(ex - FIX_BITS));
+    int fix = FIX_BITS;
+    if (!COUNT && G.max_cnt > 0) fix = min(29, max(FIX_BITS, 30 - (32 - __clz(G.max_cnt))));     // max_cnt < 2^(32 - clz)
+    const float scale = exp2f((float)(fix - ex)), inv_scale = exp2f((float)(ex - fix));
+    unsigned my_max = 0u;
     const int cfix = __float2int_rn(ci * scale);
 
     // ---- pass 2: {Delta, s} += {c_i, 1} on every visit; flush per slab -------------------------------------------------
@@ -237,6 +242,7 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
                 unsigned* d1 = reinterpret_cast<unsigned*>(win + WIN_SLOTS * 4 + a);
                 if (COUNT) {
                     const unsigned cs = *d1;
+                    my_max = max(my_max, cs);
                     if (cs != 0u) {                   // a touched slot is a verified visit: it lies inside the grid
                         red_add_v2_w(ds + col.base + z * wg.stride_z, (float)*d0 * inv_scale, (float)cs);
                         *d0 = 0; *d1 = 0u;
@@ -251,6 +257,10 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
             });
         }
         __syncthreads();
+    }
+    if (COUNT) {        // remember the largest slot count for the sweeps that reuse the cached counts
+        my_max = __reduce_max_sync(0xffffffffu, my_max);
+        if ((tid & 31) == 0 && my_max > 0u) atomicMax(&groups[launch_order[group0 + blockIdx.x]].max_cnt, (int)my_max);
     }
 }
 
