@@ -326,3 +326,23 @@ def test_windowed_plan_head_blocks(binding, oracle):
     x_o = P.solve(pr["wepl"].cpu().numpy(), np.ones(cfg.n, np.float32), 2, cfg.block, cfg.lam)
     assert np.linalg.norm(x_g - x_o) / np.linalg.norm(x_o) <= REL_L2_TOL
     assert np.max(np.abs(x_g - x_o)) <= MAX_ABS_TOL
+
+
+def test_windowed_plan_outlier_residual(binding, oracle):
+    """One history with an absurd WEPL (an undetected nuclear interaction in real data, "data cleaning"): its
+    c_i is orders of magnitude above its neighbours' and sets the fixed-point scale of its group (R21).  The image must
+    still match the oracle within the north_star tolerance."""
+    cfg = synth.scaled(synth.CONFIGS["tiny"], 20000)
+    x_true, hull, shadow = synth.make_phantom(cfg)
+    pr = synth.generate_protons(cfg, x_true, shadow)
+    wepl = pr["wepl"].clone()
+    wepl[1234] = 3000.0
+    wepl[15000] = -500.0
+    g, p, pa, P = oracle_setup(oracle, cfg, pr, hull)
+    ctx, paths = gpu_paths(binding, cfg, pr, hull)
+    ctx.solve_config(2)
+    x0 = torch.ones(cfg.n, dtype=torch.float32, device="cuda")
+    x_w = ctx.solve(paths, wepl.cuda(), x0, 4, 5000, 0.1).cpu().numpy()
+    x_o = P.solve(wepl.numpy(), np.ones(cfg.n, np.float32), 4, 5000, 0.1)
+    assert np.linalg.norm(x_w - x_o) / np.linalg.norm(x_o) <= REL_L2_TOL
+    assert np.max(np.abs(x_w - x_o)) <= MAX_ABS_TOL
