@@ -383,7 +383,14 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const HullRec*
                 while ((d0 | d1 | d2) != 0) {
                     // lowest candidate axis with the smallest s (strict comparison: x before y before z on equality)
                     int best = d0 != 0 ? 0 : (d1 != 0 ? 1 : 2);
-                    if ((d0 != 0) + (d1 != 0) + (d2 != 0) > 1) {
+                    if (d0 != 0 && d1 != 0 && d2 == 0) {
+                        // the common two-candidate case of an oblique path: x and y faces in one segment
+                        const double nx_ = fabs((d0 > 0 ? f_hi[0] : f_lo[0]) - A[0]), dx_ = fabs(B[0] - A[0]);
+                        const double ny_ = fabs((d1 > 0 ? f_hi[1] : f_lo[1]) - A[1]), dy_ = fabs(B[1] - A[1]);
+                        const double lx = nx_ * dy_, ly = ny_ * dx_;           // s_x < s_y <=> lx < ly
+                        best = ly < lx ? 1 : 0;
+                        if (fabs(lx - ly) * seg_len < g.tie_eps * (dx_ * dy_)) tie = true;
+                    } else if ((d0 != 0) + (d1 != 0) + (d2 != 0) > 1) {
                         const int dir[3] = {d0, d1, d2};
                         double num[3], den[3];
 #pragma unroll
@@ -415,8 +422,8 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const HullRec*
                     else if (best == 1) PCT_MOVE_AXIS(1, d1, g.ny)
                     else PCT_MOVE_AXIS(2, d2, g.nz)
 #undef PCT_MOVE_AXIS
-                    if (!inside) { flags = PCT_REJ_LEFT_GRID; bad = true; break; }
-                    if (++n_vis > (unsigned)g.max_visits) { flags = PCT_REJ_CAPACITY; bad = true; break; }
+                    ++n_vis;
+                    if (!inside || n_vis > (unsigned)g.max_visits) { flags = !inside ? PCT_REJ_LEFT_GRID : PCT_REJ_CAPACITY; bad = true; break; }
                     cw.push(code);
                 }
                 A[0] = B[0]; A[1] = B[1]; A[2] = B[2];
