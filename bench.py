@@ -292,7 +292,8 @@ def main():
         b_h = torch.empty(cfg.m, dtype=torch.float32).pin_memory(); b_h.copy_(b)
         hull_h = torch.empty(cfg.n, dtype=torch.uint8).pin_memory(); hull_h.copy_(hull_flat)
         x_h = torch.empty(cfg.n, dtype=torch.float32).pin_memory()
-        ctx.reconstruct_host(host, -cfg.u_tracker, cfg.u_tracker, hull_h, b_h, None, cfg.iters, cfg.block, cfg.lam, x_h)
+        for _ in range(2):      # untimed: the stream-ordered pool needs two passes to settle on this allocation pattern
+            ctx.reconstruct_host(host, -cfg.u_tracker, cfg.u_tracker, hull_h, b_h, None, cfg.iters, cfg.block, cfg.lam, x_h)
         barrier()
         t0 = time.perf_counter()
         e_start, e_stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
