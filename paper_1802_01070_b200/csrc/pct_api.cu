@@ -4,11 +4,91 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
+#include <unordered_map>
 
 #include "pct_internal.cuh"
 
 namespace pct {
+
+// ---- size-keyed cache of device buffers --------------------------------------------------------------------------------
+// Paths, plans and their scratch are rebuilt for every reconstruction with exactly the same sizes.  cudaMalloc/cudaFree of
+// tens of GB costs hundreds of milliseconds, and the stream-ordered pool (cudaMallocAsync) reused such blocks erratically
+// (35-700 ms per allocation, profiles/r01e_final.md).  So: freed blocks are kept per device and handed out again on an
+// exact size match.  The cache is process-wide (buffers outlive contexts), trimmed when it exceeds half of the device
+// memory or when an allocation fails, and by cache_trim().  A reused block is only safe because all work of a
+// reconstruction is enqueued on one stream, in order.
+namespace {
+struct DevCache {
+    std::mutex mu;
+    std::unordered_map<void*, size_t> live;                    // blocks handed out
+    std::unordered_multimap<size_t, void*> idle;               // blocks waiting for reuse
+    size_t idle_bytes = 0;
+};
+DevCache& dev_cache(int device) {
+    static DevCache caches[64];
+    return caches[device >= 0 && device < 64 ? device : 0];
+}
+void trim_locked(DevCache& c) {
+    for (auto& kv : c.idle) cudaFree(kv.second);
+    c.idle.clear();
+    c.idle_bytes = 0;
+}
+}  // namespace
+
+cudaError_t cache_alloc(void** p, size_t bytes) {
+    *p = nullptr;
+    if (bytes == 0) bytes = 16;
+    int device = 0;
+    cudaGetDevice(&device);
+    DevCache& c = dev_cache(device);
+    std::lock_guard<std::mutex> lock(c.mu);
+    auto it = c.idle.find(bytes);
+    if (it != c.idle.end()) {
+        *p = it->second;
+        c.idle.erase(it);
+        c.idle_bytes -= bytes;
+        c.live[*p] = bytes;
+        return cudaSuccess;
+    }
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess) {                 // make room and try once more
+        cudaGetLastError();
+        cudaDeviceSynchronize();
+        trim_locked(c);
+        e = cudaMalloc(p, bytes);
+    }
+    if (e == cudaSuccess) c.live[*p] = bytes;
+    return e;
+}
+
+cudaError_t cache_free(void* p) {
+    if (!p) return cudaSuccess;
+    int device = 0;
+    cudaGetDevice(&device);
+    DevCache& c = dev_cache(device);
+    std::lock_guard<std::mutex> lock(c.mu);
+    auto it = c.live.find(p);
+    if (it == c.live.end()) return cudaFree(p);          // not ours
+    const size_t bytes = it->second;
+    c.live.erase(it);
+    size_t free_b = 0, total_b = 0;
+    if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && c.idle_bytes + bytes > total_b / 2) {
+        cudaDeviceSynchronize();
+        trim_locked(c);
+    }
+    c.idle.emplace(bytes, p);
+    c.idle_bytes += bytes;
+    return cudaSuccess;
+}
+
+void cache_trim(int device) {
+    DevCache& c = dev_cache(device);
+    std::lock_guard<std::mutex> lock(c.mu);
+    cudaDeviceSynchronize();
+    trim_locked(c);
+}
 
 int set_error(pct_ctx* ctx, int code, const char* fmt, ...) {
     if (ctx) {
@@ -52,7 +132,7 @@ struct DeviceGuard {
 
 static void free_paths_arrays(pct_paths* P) {
     cudaDeviceSynchronize();         // the buffers go back to the pool on the legacy stream: nothing may still use them
-    pool_free(P->N, 0); pool_free(P->start, 0); pool_free(P->end, 0); pool_free(P->ell, 0); pool_free(P->flags, 0); pool_free(P->code_off, 0); pool_free(P->codes, 0);
+    cache_free(P->N); cache_free(P->start); cache_free(P->end); cache_free(P->ell); cache_free(P->flags); cache_free(P->code_off); cache_free(P->codes);
     if (P->plan) { free_solve_plan(P->plan); P->plan = nullptr; }
     P->N = nullptr; P->start = nullptr; P->end = nullptr; P->ell = nullptr; P->flags = nullptr; P->code_off = nullptr; P->codes = nullptr;
 }
@@ -76,13 +156,13 @@ static int ensure_codes(pct_ctx* ctx, pct_paths* P, int64_t need, cudaStream_t s
     int64_t cap = P->chunks_cap + P->chunks_cap / 2;
     if (cap < need) cap = need;
     ulonglong2* fresh = nullptr;
-    cudaError_t e = cudaMallocAsync(&fresh, sizeof(ulonglong2) * (size_t)cap, st);
-    if (e != cudaSuccess && cap > need) { cudaGetLastError(); cap = need; e = cudaMallocAsync(&fresh, sizeof(ulonglong2) * (size_t)cap, st); }
+    cudaError_t e = cache_alloc((void**)&fresh, sizeof(ulonglong2) * (size_t)cap);
+    if (e != cudaSuccess && cap > need) { cudaGetLastError(); cap = need; e = cache_alloc((void**)&fresh, sizeof(ulonglong2) * (size_t)cap); }
     if (e != cudaSuccess) { cudaGetLastError(); return set_error(ctx, PCT_E_OOM, "code stream of %lld chunks does not fit", (long long)cap); }
     if (P->chunks_used > 0)
         PCT_CUDA(ctx, cudaMemcpyAsync(fresh, P->codes, sizeof(ulonglong2) * (size_t)P->chunks_used, cudaMemcpyDeviceToDevice, st));
     PCT_CUDA(ctx, cudaStreamSynchronize(st));
-    if (P->codes) PCT_CUDA(ctx, pool_free(P->codes, st));
+    if (P->codes) PCT_CUDA(ctx, cache_free(P->codes));
     P->codes = fresh;
     P->chunks_cap = cap;
     return PCT_OK;
@@ -150,15 +230,6 @@ int pct_create(const pct_geometry* geom, const pct_mlp_params* params, int devic
     }
     if (cudaMalloc(&ctx->d_stats, sizeof(GenStats)) != cudaSuccess || cudaMalloc(&ctx->d_total, sizeof(unsigned long long)) != cudaSuccess) {
         cudaGetLastError(); pct_destroy(ctx); return PCT_E_OOM;
-    }
-    {   // large buffers come from the device's stream-ordered pool; keep freed memory cached (paths and plans are
-        // rebuilt per reconstruction, and a multi-GB cudaMalloc/cudaFree pair costs tens of milliseconds)
-        cudaMemPool_t pool;
-        if (cudaDeviceGetDefaultMemPool(&pool, device) == cudaSuccess) {
-            unsigned long long keep = ~0ull;
-            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-        }
-        cudaGetLastError();
     }
     *out = ctx;
     return PCT_OK;
@@ -235,19 +306,19 @@ int pct_generate_mlp(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hull, v
     ulonglong2* stage = nullptr;
     uint32_t* nchunks = nullptr;
     int rc = PCT_OK;
-    auto fail = [&](int code) { pool_free(stage, st); pool_free(nchunks, st); free_paths_arrays(P); delete P; return code; };
+    auto fail = [&](int code) { cache_free(stage); cache_free(nchunks); free_paths_arrays(P); delete P; return code; };
 #define GEN_CUDA(call)                                                                                          \
     do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { cudaGetLastError();                               \
         return fail(set_error(ctx, e__ == cudaErrorMemoryAllocation ? PCT_E_OOM : PCT_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e__))); } } while (0)
-    GEN_CUDA(cudaMallocAsync(&P->N, sizeof(uint32_t) * mm, st));
-    GEN_CUDA(cudaMallocAsync(&P->start, sizeof(int32_t) * mm, st));
-    GEN_CUDA(cudaMallocAsync(&P->end, sizeof(int32_t) * mm, st));
-    GEN_CUDA(cudaMallocAsync(&P->ell, sizeof(float) * mm, st));
-    GEN_CUDA(cudaMallocAsync(&P->flags, sizeof(uint8_t) * mm, st));
-    GEN_CUDA(cudaMallocAsync(&P->code_off, sizeof(uint64_t) * mm, st));
+    GEN_CUDA(cache_alloc((void**)&P->N, sizeof(uint32_t) * mm));
+    GEN_CUDA(cache_alloc((void**)&P->start, sizeof(int32_t) * mm));
+    GEN_CUDA(cache_alloc((void**)&P->end, sizeof(int32_t) * mm));
+    GEN_CUDA(cache_alloc((void**)&P->ell, sizeof(float) * mm));
+    GEN_CUDA(cache_alloc((void**)&P->flags, sizeof(uint8_t) * mm));
+    GEN_CUDA(cache_alloc((void**)&P->code_off, sizeof(uint64_t) * mm));
     const int batch_max = (int)(m < GEN_BATCH ? (m > 0 ? m : 1) : GEN_BATCH);
-    GEN_CUDA(cudaMallocAsync(&stage, sizeof(ulonglong2) * (size_t)batch_max * (size_t)ctx->cfg.stage_chunks, st));
-    GEN_CUDA(cudaMallocAsync(&nchunks, sizeof(uint32_t) * (size_t)batch_max, st));
+    GEN_CUDA(cache_alloc((void**)&stage, sizeof(ulonglong2) * (size_t)batch_max * (size_t)ctx->cfg.stage_chunks));
+    GEN_CUDA(cache_alloc((void**)&nchunks, sizeof(uint32_t) * (size_t)batch_max));
     GEN_CUDA(cudaMemsetAsync(ctx->d_stats, 0, sizeof(GenStats), st));
     const ProtonPtrs pp = {pr->phi, pr->t_in, pr->v_in, pr->dt_in, pr->dv_in, pr->t_out, pr->v_out, pr->dt_out, pr->dv_out};
     for (int64_t i0 = 0; i0 < m; i0 += GEN_BATCH) {
@@ -260,9 +331,9 @@ int pct_generate_mlp(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hull, v
         GEN_CUDA(cudaStreamSynchronize(st));
         int64_t need = P->chunks_used + (int64_t)batch_chunks;
         if (need > P->chunks_cap) {
-            // first batch: extrapolate to all histories (+25 %); later: ensure_codes grows by 1.5x
+            // first batch: extrapolate to all histories (+60 %: oblique paths take up to sqrt(2) more steps); later: ensure_codes grows by 1.5x
             int64_t guess = need;
-            if (i0 == 0 && m > count) guess = (int64_t)((double)batch_chunks * ((double)m / (double)count) * 1.25) + 1024;
+            if (i0 == 0 && m > count) guess = (int64_t)((double)batch_chunks * ((double)m / (double)count) * 1.6) + 1024;   // the first batch may be the axis-aligned (shortest-code) one
             if ((rc = ensure_codes(ctx, P, guess > need ? guess : need, st)) != PCT_OK) {
                 if (guess > need && (rc = ensure_codes(ctx, P, need, st)) != PCT_OK) return fail(rc);
             }
@@ -274,7 +345,7 @@ int pct_generate_mlp(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hull, v
     GEN_CUDA(cudaMemcpyAsync(&hs, ctx->d_stats, sizeof(hs), cudaMemcpyDeviceToHost, st));
     GEN_CUDA(cudaStreamSynchronize(st));
 #undef GEN_CUDA
-    pool_free(stage, st); pool_free(nchunks, st);
+    cache_free(stage); cache_free(nchunks);
     P->total_visits = (int64_t)hs.total_visits; P->n_rejected = (int64_t)hs.n_rejected; P->total_samples = (int64_t)hs.total_samples; P->n_ties = (int64_t)hs.n_ties;
     *out = P;
     return PCT_OK;
@@ -443,7 +514,7 @@ int pct_reconstruct_host(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hul
     auto cleanup = [&]() {
         ctx->batch_ready = nullptr; ctx->n_batch_ready = 0;
         if (cs) cudaStreamSynchronize(cs);
-        pool_free(d_tr, st); pool_free(d_b, st); pool_free(d_x, st); pool_free(d_hull, st);
+        cache_free(d_tr); cache_free(d_b); cache_free(d_x); cache_free(d_hull);
         if (P) pct_paths_free(P);
         for (auto& e : ev) if (e) cudaEventDestroy(e);
         for (auto& e : ready) if (e) cudaEventDestroy(e);
@@ -456,10 +527,10 @@ int pct_reconstruct_host(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hul
     do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { cudaGetLastError(); cleanup();                    \
         return set_error(ctx, e__ == cudaErrorMemoryAllocation ? PCT_E_OOM : PCT_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e__)); } } while (0)
     for (auto& e : ev) REC_CUDA(cudaEventCreate(&e));
-    REC_CUDA(cudaMallocAsync(&d_tr, sizeof(double) * 9 * mm, st));
-    REC_CUDA(cudaMallocAsync(&d_b, sizeof(float) * mm, st));
-    REC_CUDA(cudaMallocAsync(&d_x, sizeof(float) * (size_t)n, st));
-    if (hull_host) REC_CUDA(cudaMallocAsync(&d_hull, (size_t)n, st));
+    REC_CUDA(cache_alloc((void**)&d_tr, sizeof(double) * 9 * mm));
+    REC_CUDA(cache_alloc((void**)&d_b, sizeof(float) * mm));
+    REC_CUDA(cache_alloc((void**)&d_x, sizeof(float) * (size_t)n));
+    if (hull_host) REC_CUDA(cache_alloc((void**)&d_hull, (size_t)n));
     REC_CUDA(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
     REC_CUDA(cudaEventCreateWithFlags(&ev_alloc, cudaEventDisableTiming));
     REC_CUDA(cudaEventCreate(&ev_c0));

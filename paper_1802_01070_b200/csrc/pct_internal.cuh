@@ -164,9 +164,10 @@ namespace pct {
 
 int set_error(pct_ctx* ctx, int code, const char* fmt, ...);
 
-// Large, short-lived buffers (paths, plans, sort scratch) come from the device's stream-ordered pool (cudaMallocAsync) and
-// go back to it with cudaFreeAsync; cudaFree on such a pointer works but leaves the pool's accounting and reuse erratic.
-inline cudaError_t pool_free(void* p, cudaStream_t st) { return p ? cudaFreeAsync(p, st) : cudaSuccess; }
+// Large, short-lived buffers (paths, plans, sort scratch) come from a size-keyed cache of device blocks (pct_api.cu).
+cudaError_t cache_alloc(void** p, size_t bytes);
+cudaError_t cache_free(void* p);
+void cache_trim(int device);
 
 // RAII bracket around one kernel launch when profiling is on (kinds: pct.h, pct_profile)
 struct ProfScope {

@@ -335,8 +335,8 @@ __global__ void k_plan_work_keys(const PlanGroup* __restrict__ groups, const uin
 void free_solve_plan(SolvePlan* plan) {
     if (!plan) return;
     cudaDeviceSynchronize();         // freed on the legacy stream: nothing may still use the plan
-    pool_free(plan->perm, 0); pool_free(plan->p0, 0); pool_free(plan->pflag, 0); pool_free(plan->cnt, 0); pool_free(plan->groups, 0); pool_free(plan->stream, 0); pool_free(plan->launch_order, 0);
-    pool_free(plan->direct_list, 0); pool_free(plan->d_direct_count, 0);
+    cache_free(plan->perm); cache_free(plan->p0); cache_free(plan->pflag); cache_free(plan->cnt); cache_free(plan->groups); cache_free(plan->stream); cache_free(plan->launch_order);
+    cache_free(plan->direct_list); cache_free(plan->d_direct_count);
     delete plan;
 }
 
@@ -355,8 +355,8 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     void* tmp = nullptr;
     int64_t* d_group_begin = nullptr;
     auto fail = [&](int code) {
-        pool_free(keysA, st); pool_free(keysB, st); pool_free(valsA, st); pool_free(valsB, st); pool_free(tmp, st); pool_free(cnt_off, st); pool_free(cnt_len, st);
-        pool_free(d_group_begin, st);
+        cache_free(keysA); cache_free(keysB); cache_free(valsA); cache_free(valsB); cache_free(tmp); cache_free(cnt_off); cache_free(cnt_len);
+        cache_free(d_group_begin);
         free_solve_plan(plan);
         return code;
     };
@@ -381,8 +381,8 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
                 std::chrono::duration<double, std::milli>(now - t_last).count(), reserved / 1e9, used / 1e9, (double)thr);
         t_last = now;
     };
-    PLAN_CUDA(cudaMallocAsync(&keysA, 8 * mm, st)); PLAN_CUDA(cudaMallocAsync(&keysB, 8 * mm, st));
-    PLAN_CUDA(cudaMallocAsync(&valsA, 4 * mm, st)); PLAN_CUDA(cudaMallocAsync(&valsB, 4 * mm, st));
+    PLAN_CUDA(cache_alloc((void**)&keysA, 8 * mm)); PLAN_CUDA(cache_alloc((void**)&keysB, 8 * mm));
+    PLAN_CUDA(cache_alloc((void**)&valsA, 4 * mm)); PLAN_CUDA(cache_alloc((void**)&valsB, 4 * mm));
     const unsigned nb256 = (unsigned)((m + 255) / 256);
     k_plan_keys<<<nb256, 256, 0, st>>>(ctx->cfg, P->N, P->start, P->end, m, block_size, keysA, valsA);
     ++ctx->launches;
@@ -393,7 +393,7 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     cub::DoubleBuffer<uint32_t> dv(valsA, valsB);
     size_t tmp_bytes = 0;
     PLAN_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, dk, dv, m, 0, KEY_BLOCK_SHIFT + block_bits, st));
-    PLAN_CUDA(cudaMallocAsync(&tmp, tmp_bytes > 0 ? tmp_bytes : 16, st));
+    PLAN_CUDA(cache_alloc((void**)&tmp, tmp_bytes > 0 ? tmp_bytes : 16));
     PLAN_CUDA(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, dk, dv, m, 0, KEY_BLOCK_SHIFT + block_bits, st));
     const uint64_t* keys = dk.Current();
     uint64_t* gid = dk.Alternate();            // reused: group id per sorted position
@@ -410,10 +410,10 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     PLAN_CUDA(cudaMemcpyAsync(&n_groups, ctx->d_total, sizeof(n_groups), cudaMemcpyDeviceToHost, st));
     PLAN_CUDA(cudaStreamSynchronize(st));
     plan->n_groups = (int64_t)n_groups;
-    PLAN_CUDA(cudaMallocAsync(&plan->groups, sizeof(PlanGroup) * (size_t)(n_groups + 1), st));
-    PLAN_CUDA(cudaMallocAsync(&d_group_begin, sizeof(int64_t) * (size_t)(n_blocks + 1), st));
-    PLAN_CUDA(cudaMallocAsync(&cnt_len, sizeof(uint32_t) * (size_t)n_groups, st));
-    PLAN_CUDA(cudaMallocAsync(&cnt_off, sizeof(uint64_t) * (size_t)n_groups, st));
+    PLAN_CUDA(cache_alloc((void**)&plan->groups, sizeof(PlanGroup) * (size_t)(n_groups + 1)));
+    PLAN_CUDA(cache_alloc((void**)&d_group_begin, sizeof(int64_t) * (size_t)(n_blocks + 1)));
+    PLAN_CUDA(cache_alloc((void**)&cnt_len, sizeof(uint32_t) * (size_t)n_groups));
+    PLAN_CUDA(cache_alloc((void**)&cnt_off, sizeof(uint64_t) * (size_t)n_groups));
     lap("heads + scan");
     k_plan_starts<<<nb256, 256, 0, st>>>(keys, head, gid, m, plan->groups, d_group_begin);
     k_plan_params<<<(unsigned)n_groups, 256, 0, st>>>(ctx->cfg, P->start, P->end, plan->perm, m, (int64_t)n_groups, plan->groups, cnt_len);
@@ -428,15 +428,15 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     ++ctx->launches;
     // the sort buffers are no longer needed once the group table is complete
     PLAN_CUDA(cudaStreamSynchronize(st));
-    pool_free(keysA, st); pool_free(keysB, st); pool_free(valsA, st); pool_free(valsB, st); pool_free(tmp, st);
+    cache_free(keysA); cache_free(keysB); cache_free(valsA); cache_free(valsB); cache_free(tmp);
     keysA = keysB = nullptr; valsA = valsB = nullptr; tmp = nullptr;
     lap("starts + params + cnt scan");
-    PLAN_CUDA(cudaMallocAsync(&plan->cnt, cnt_bytes > 0 ? (size_t)cnt_bytes : 16, st));
+    PLAN_CUDA(cache_alloc((void**)&plan->cnt, cnt_bytes > 0 ? (size_t)cnt_bytes : 16));
     PLAN_CUDA(cudaMemsetAsync(plan->cnt, 0, cnt_bytes > 0 ? (size_t)cnt_bytes : 16, st));
-    PLAN_CUDA(cudaMallocAsync(&plan->p0, 4 * mm, st));
-    PLAN_CUDA(cudaMallocAsync(&plan->pflag, mm, st));
-    PLAN_CUDA(cudaMallocAsync(&plan->direct_list, 4 * mm, st));
-    PLAN_CUDA(cudaMallocAsync(&plan->d_direct_count, sizeof(uint32_t) * (size_t)n_blocks, st));
+    PLAN_CUDA(cache_alloc((void**)&plan->p0, 4 * mm));
+    PLAN_CUDA(cache_alloc((void**)&plan->pflag, mm));
+    PLAN_CUDA(cache_alloc((void**)&plan->direct_list, 4 * mm));
+    PLAN_CUDA(cache_alloc((void**)&plan->d_direct_count, sizeof(uint32_t) * (size_t)n_blocks));
     PLAN_CUDA(cudaMemsetAsync(plan->d_direct_count, 0, sizeof(uint32_t) * (size_t)n_blocks, st));
     lap("allocs before verify");
     k_plan_verify<<<(unsigned)n_groups, GROUP, 0, st>>>(ctx->cfg, P->N, P->start, P->code_off, P->codes, plan->perm, plan->groups,
@@ -452,7 +452,7 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     PLAN_CUDA(cudaMemcpyAsync(&stream_words, ctx->d_total, sizeof(stream_words), cudaMemcpyDeviceToHost, st));
     PLAN_CUDA(cudaStreamSynchronize(st));
     plan->stream_words = (int64_t)stream_words;
-    PLAN_CUDA(cudaMallocAsync(&plan->stream, stream_words > 0 ? 8 * (size_t)stream_words : 16, st));
+    PLAN_CUDA(cache_alloc((void**)&plan->stream, stream_words > 0 ? 8 * (size_t)stream_words : 16));
     PLAN_CUDA(cudaMemsetAsync(plan->stream, 0xFF, stream_words > 0 ? 8 * (size_t)stream_words : 16, st));
     k_plan_stream_off<<<(unsigned)((n_groups + 255) / 256), 256, 0, st>>>(cnt_off, (int64_t)n_groups, plan->groups);
     lap("stream alloc + memset");
@@ -466,17 +466,17 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
         uint32_t *wv0 = nullptr, *wv1 = nullptr;
         void* wtmp = nullptr;
         const size_t ng = (size_t)n_groups;
-        auto wfree = [&]() { pool_free(wk0, st); pool_free(wk1, st); pool_free(wv0, st); pool_free(wv1, st); pool_free(wtmp, st); };
+        auto wfree = [&]() { cache_free(wk0); cache_free(wk1); cache_free(wv0); cache_free(wv1); cache_free(wtmp); };
 #define WORK_CUDA(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { cudaGetLastError(); wfree(); \
         return fail(set_error(ctx, e__ == cudaErrorMemoryAllocation ? PCT_E_OOM : PCT_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e__))); } } while (0)
-        WORK_CUDA(cudaMallocAsync(&wk0, 8 * ng, st)); WORK_CUDA(cudaMallocAsync(&wk1, 8 * ng, st));
-        WORK_CUDA(cudaMallocAsync(&wv0, 4 * ng, st)); WORK_CUDA(cudaMallocAsync(&wv1, 4 * ng, st));
+        WORK_CUDA(cache_alloc((void**)&wk0, 8 * ng)); WORK_CUDA(cache_alloc((void**)&wk1, 8 * ng));
+        WORK_CUDA(cache_alloc((void**)&wv0, 4 * ng)); WORK_CUDA(cache_alloc((void**)&wv1, 4 * ng));
         k_plan_work_keys<<<(unsigned)((n_groups + 255) / 256), 256, 0, st>>>(plan->groups, plan->perm, (int64_t)n_groups, block_size, wk0, wv0);
         cub::DoubleBuffer<uint64_t> wk(wk0, wk1);
         cub::DoubleBuffer<uint32_t> wv(wv0, wv1);
         size_t wbytes = 0;
         WORK_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, wbytes, wk, wv, (int64_t)n_groups, 0, 32 + block_bits, st));
-        WORK_CUDA(cudaMallocAsync(&wtmp, wbytes > 0 ? wbytes : 16, st));
+        WORK_CUDA(cache_alloc((void**)&wtmp, wbytes > 0 ? wbytes : 16));
         WORK_CUDA(cub::DeviceRadixSort::SortPairs(wtmp, wbytes, wk, wv, (int64_t)n_groups, 0, 32 + block_bits, st));
         WORK_CUDA(cudaStreamSynchronize(st));
         plan->launch_order = wv.Current();
@@ -494,7 +494,7 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     PLAN_CUDA(cudaStreamSynchronize(st));
     plan->group_begin[(size_t)n_blocks] = (int64_t)n_groups;
     for (uint32_t c : plan->direct_count) plan->n_direct += c;
-    pool_free(cnt_off, st); pool_free(cnt_len, st); pool_free(d_group_begin, st);
+    cache_free(cnt_off); cache_free(cnt_len); cache_free(d_group_begin);
 #undef PLAN_CUDA
     *out = plan;
     return PCT_OK;
