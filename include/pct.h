@@ -15,6 +15,9 @@
  *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Work is enqueued on it; device
  *     results are valid once the caller has synchronised the stream.  pct_generate_mlp and the *_host calls
  *     synchronise the stream themselves (they need sizes on the host).
+ *   - Device memory: paths, plans and scratch come from a process-wide cache of device blocks that are reused on an exact
+ *     size match (rebuilding the same reconstruction costs no allocation); pct_trim_cache releases the idle blocks.  All
+ *     calls on one context must be issued on one stream at a time (a reused block relies on stream order).
  *   - Return value: PCT_OK (0) or a negative PCT_E_* code; never throws, never aborts.  pct_last_error(ctx)
  *     gives a human-readable message for the last failure on that context.
  *   - Frames (R1): grid frame (x,y,z), z = rotation axis, voxel (ix,iy,iz) = origin + [i, i+1]*h per axis,
@@ -121,6 +124,9 @@ int pct_solve(pct_ctx* ctx, const pct_paths* paths, const float* b, const float*
 int pct_reconstruct_host(pct_ctx* ctx, const pct_protons* protons, const uint8_t* hull_host, const float* b_host,
                          const float* x0_host, int iters, int64_t block_size, float lambda, float* x_out_host,
                          pct_recon_stats* stats, void* stream);
+
+/* Releases the idle blocks of the device-buffer cache of ctx's device (synchronises the device). */
+int pct_trim_cache(pct_ctx* ctx);
 
 /* Number of kernel launches issued by this context so far (bench.py reports it as gpu_launches). */
 int64_t pct_launch_count(const pct_ctx* ctx);

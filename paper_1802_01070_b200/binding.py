@@ -21,7 +21,7 @@ REJECT_MASK = REJ_MISS | REJ_ORDER | REJ_DEPTH | REJ_LEFT_GRID | REJ_CAPACITY | 
 EXPORTS = ("pct_create", "pct_destroy", "pct_last_error", "pct_generate_mlp", "pct_paths_info", "pct_paths_free",
            "pct_paths_decode", "pct_forward_project", "pct_column_counts", "pct_solve", "pct_reconstruct_host",
            "pct_launch_count", "pct_profile_enable", "pct_profile_read", "pct_measure_peaks", "pct_solve_config",
-           "pct_plan_info")
+           "pct_plan_info", "pct_trim_cache")
 
 
 class Geometry(C.Structure):
@@ -108,6 +108,7 @@ def load_library(path: Optional[str] = None):
     L.pct_measure_peaks.argtypes = [vp, C.POINTER(Peaks)]
     L.pct_solve_config.argtypes = [vp, C.c_int, i64]
     L.pct_plan_info.argtypes = [vp, C.POINTER(PlanStats)]
+    L.pct_trim_cache.argtypes = [vp]
     if path == _build.LIB:
         _lib = L
     return L
@@ -209,6 +210,10 @@ class Context:
         pr = Profile()
         self._check(self._L.pct_profile_read(self._h, C.byref(pr)))
         return {k: (pr.ms[i], pr.launches[i]) for i, k in enumerate(PROFILE_KINDS)}
+
+    def trim_cache(self):
+        """pct_trim_cache: give the idle device blocks of the library's buffer cache back to the driver."""
+        self._check(self._L.pct_trim_cache(self._h))
 
     def solve_config(self, mode: int = 0, min_block: int = 0):
         """pct_solve_config: 0 = automatic, 1 = direct kernel only, 2 = windowed plan whenever possible."""

@@ -268,6 +268,13 @@ int pct_profile_read(pct_ctx* ctx, pct_profile* out) {
 }
 
 const char* pct_last_error(const pct_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+int pct_trim_cache(pct_ctx* ctx) {
+    if (!ctx) return PCT_E_INVALID_ARG;
+    DeviceGuard guard(ctx->device);
+    cache_trim(ctx->device);
+    return PCT_OK;
+}
+
 int64_t pct_launch_count(const pct_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
 int pct_generate_mlp(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hull, void* stream, pct_paths** out) {
