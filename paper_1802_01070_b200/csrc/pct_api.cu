@@ -1,8 +1,10 @@
 // pct_api.cu -- the extern "C" boundary of libpct.so (include/pct.h) and the iteration driver (A8).
 #include <algorithm>
+#include <chrono>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <new>
@@ -533,11 +535,17 @@ int pct_reconstruct_host(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hul
 #define REC_CUDA(call)                                                                                          \
     do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { cudaGetLastError(); cleanup();                    \
         return set_error(ctx, e__ == cudaErrorMemoryAllocation ? PCT_E_OOM : PCT_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e__)); } } while (0)
+    const bool dbg = getenv("PCT_PLAN_DEBUG") != nullptr;
+    const auto t_begin = std::chrono::steady_clock::now();
+    auto stamp = [&](const char* what) {
+        if (dbg) fprintf(stderr, "[recon] %-22s at %8.2f ms\n", what, std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t_begin).count());
+    };
     for (auto& e : ev) REC_CUDA(cudaEventCreate(&e));
     REC_CUDA(cache_alloc((void**)&d_tr, sizeof(double) * 9 * mm));
     REC_CUDA(cache_alloc((void**)&d_b, sizeof(float) * mm));
     REC_CUDA(cache_alloc((void**)&d_x, sizeof(float) * (size_t)n));
     if (hull_host) REC_CUDA(cache_alloc((void**)&d_hull, (size_t)n));
+    stamp("allocated");
     REC_CUDA(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
     REC_CUDA(cudaEventCreateWithFlags(&ev_alloc, cudaEventDisableTiming));
     REC_CUDA(cudaEventCreate(&ev_c0));
@@ -564,18 +572,22 @@ int pct_reconstruct_host(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hul
     pct_protons dev = *pr;
     dev.phi = d_tr; dev.t_in = d_tr + mm; dev.v_in = d_tr + 2 * mm; dev.dt_in = d_tr + 3 * mm; dev.dv_in = d_tr + 4 * mm;
     dev.t_out = d_tr + 5 * mm; dev.v_out = d_tr + 6 * mm; dev.dt_out = d_tr + 7 * mm; dev.dv_out = d_tr + 8 * mm;
+    stamp("copies enqueued");
     ctx->batch_ready = ready.data(); ctx->n_batch_ready = n_batches;
     rc = pct_generate_mlp(ctx, &dev, d_hull, stream, &P);
     ctx->batch_ready = nullptr; ctx->n_batch_ready = 0;
     if (rc != PCT_OK) { cleanup(); return rc; }
     REC_CUDA(cudaEventRecord(ev[2], st));
+    stamp("generate returned");
     REC_CUDA(cudaStreamWaitEvent(st, ev_c1, 0));              // b has arrived
     if (!x0_host && (rc = launch_fill(ctx, d_x, n, 1.0f, st)) != PCT_OK) { cleanup(); return rc; }   // x0 = 1 (BASELINE.json configs)
     if ((rc = pct_solve(ctx, P, d_b, d_x, iters, block_size, lambda, d_x, stream)) != PCT_OK) { cleanup(); return rc; }
     REC_CUDA(cudaEventRecord(ev[3], st));
     REC_CUDA(cudaMemcpyAsync(x_out_host, d_x, sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost, st));
     REC_CUDA(cudaEventRecord(ev[4], st));
+    stamp("solve enqueued");
     REC_CUDA(cudaStreamSynchronize(st));
+    stamp("stream drained");
     if (stats) {
         stats->m = m; stats->total_visits = P->total_visits; stats->n_rejected = P->n_rejected; stats->n_ties = P->n_ties;
         float ms[4] = {0, 0, 0, 0};
@@ -585,6 +597,7 @@ int pct_reconstruct_host(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hul
     }
 #undef REC_CUDA
     cleanup();
+    stamp("cleaned up");
     return PCT_OK;
 }
 
