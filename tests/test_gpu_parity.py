@@ -346,3 +346,35 @@ def test_windowed_plan_outlier_residual(binding, oracle):
     x_o = P.solve(wepl.numpy(), np.ones(cfg.n, np.float32), 4, 5000, 0.1)
     assert np.linalg.norm(x_w - x_o) / np.linalg.norm(x_o) <= REL_L2_TOL
     assert np.max(np.abs(x_w - x_o)) <= MAX_ABS_TOL
+
+
+def test_count_cache_ownership_between_plans(binding, oracle):
+    """Two sets of rows solved alternately on ONE context: the context's count cache (R23) changes owner every call and
+    must be refilled, never reused across plans; repeated calls on the same rows must reuse it.  Each result equals the
+    oracle's for its own rows."""
+    cfg = synth.scaled(synth.CONFIGS["tiny"], 12000)
+    x_true, hull, shadow = synth.make_phantom(cfg)
+    pr_a = synth.generate_protons(cfg, x_true, shadow)
+    pr_b = synth.generate_protons(dataclasses.replace(cfg, seed=7), x_true, shadow)
+    kw = synth.mlp_params(cfg)
+    ctx = binding.Context(synth.geometry(cfg), kw, 0)
+    ctx.solve_config(2)
+    hull_d = hull.reshape(-1).cuda()
+    paths, refs = [], []
+    for pr in (pr_a, pr_b):
+        dev = {k: pr[k].cuda() for k in binding.PROTON_KEYS}
+        paths.append(ctx.generate_mlp(dev, -cfg.u_tracker, cfg.u_tracker, hull_d))
+        g, p, pa, P = oracle_setup(oracle, cfg, pr, hull)
+        refs.append(P.solve(pr["wepl"].numpy(), np.ones(cfg.n, np.float32), 3, 4000, 0.1))
+    x0 = torch.ones(cfg.n, dtype=torch.float32, device="cuda")
+    for which in (0, 1, 1, 0, 0, 1):
+        pr = (pr_a, pr_b)[which]
+        x_g = ctx.solve(paths[which], pr["wepl"].cuda(), x0, 3, 4000, 0.1).cpu().numpy()
+        assert np.linalg.norm(x_g - refs[which]) / np.linalg.norm(refs[which]) <= REL_L2_TOL
+        assert np.max(np.abs(x_g - refs[which])) <= MAX_ABS_TOL
+    # a different block size on the same rows rebuilds the plan (and the counts)
+    x_g = ctx.solve(paths[0], pr_a["wepl"].cuda(), x0, 2, 2500, 0.1).cpu().numpy()
+    g, p, pa, P = oracle_setup(oracle, cfg, pr_a, hull)
+    x_o = P.solve(pr_a["wepl"].numpy(), np.ones(cfg.n, np.float32), 2, 2500, 0.1)
+    assert np.max(np.abs(x_g - x_o)) <= MAX_ABS_TOL
+    ctx.trim_cache()
