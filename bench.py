@@ -23,7 +23,7 @@ if ROOT not in sys.path:
 import numpy as np
 import torch
 
-from paper_1802_01070_b200 import synth
+import synth
 
 METRIC = "path-voxel updates/s per solver iteration; end-to-end recon s at 116M/261M"
 UNIT = "path-voxel updates/s"

@@ -105,6 +105,12 @@ void pct_paths_free(pct_paths* paths);
 int pct_paths_decode(pct_ctx* ctx, const pct_paths* paths, int64_t i0, int64_t i1, int64_t* row_ptr, int32_t* voxels,
                      int64_t cap, float* ell, uint8_t* flags, void* stream);
 
+/* The tie log (R9; north_star: "logged boundary ties"): indices, ascending, of the histories whose flags intersect
+ * `mask` (e.g. PCT_TIE).  idx_out: HOST int64[cap] (may be NULL if cap == 0); *n_out (HOST) = how many histories match.
+ * If more than cap match, an arbitrary cap of them are returned.  m < 2^32.  Synchronises `stream`. */
+int pct_paths_flagged(pct_ctx* ctx, const pct_paths* paths, uint32_t mask, int64_t* idx_out, int64_t cap, int64_t* n_out,
+                      void* stream);
+
 /* A9 (R19): b_out[i] = l_i * sum over visits of x[j].  x: DEVICE float32[n]; b_out: DEVICE float32[m]. */
 int pct_forward_project(pct_ctx* ctx, const pct_paths* paths, const float* x, float* b_out, void* stream);
 

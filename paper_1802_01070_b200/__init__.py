@@ -1,8 +1,7 @@
 """pct-b200: single-B200 proton-CT hot path (MLP -> rows of A -> block-iterative DROP).
 
 Sub-modules
-  synth    seeded synthetic inputs (shared by oracle tests and CUDA tests; no method arithmetic)
   binding  thin ctypes binding of the C-ABI in include/pct.h (libpct.so; fails loudly if missing)
   build    in-tree nvcc build of csrc/ for sm_100a
 """
-__all__ = ["synth", "binding", "build"]
+__all__ = ["binding", "build"]

@@ -21,7 +21,7 @@ REJECT_MASK = REJ_MISS | REJ_ORDER | REJ_DEPTH | REJ_LEFT_GRID | REJ_CAPACITY | 
 EXPORTS = ("pct_create", "pct_destroy", "pct_last_error", "pct_generate_mlp", "pct_paths_info", "pct_paths_free",
            "pct_paths_decode", "pct_forward_project", "pct_column_counts", "pct_solve", "pct_reconstruct_host",
            "pct_launch_count", "pct_profile_enable", "pct_profile_read", "pct_measure_peaks", "pct_solve_config",
-           "pct_plan_info", "pct_trim_cache")
+           "pct_plan_info", "pct_trim_cache", "pct_paths_flagged")
 
 
 class Geometry(C.Structure):
@@ -96,6 +96,7 @@ def load_library(path: Optional[str] = None):
     L.pct_paths_free.argtypes = [vp]
     L.pct_paths_free.restype = None
     L.pct_paths_decode.argtypes = [vp, vp, i64, i64, vp, vp, i64, vp, vp, vp]
+    L.pct_paths_flagged.argtypes = [vp, vp, C.c_uint32, vp, i64, C.POINTER(i64), vp]
     L.pct_forward_project.argtypes = [vp, vp, vp, vp, vp]
     L.pct_column_counts.argtypes = [vp, vp, i64, i64, vp, vp]
     L.pct_solve.argtypes = [vp, vp, vp, vp, C.c_int, i64, C.c_float, vp, vp]
@@ -250,6 +251,15 @@ class Context:
         self._check(self._L.pct_paths_decode(self._h, paths._h, i0, i1, row_ptr.data_ptr(), vox.data_ptr(), total, None,
                                              None, st))
         return row_ptr, vox[:total], ell, flags
+
+    def paths_flagged(self, paths: Paths, mask: int = TIE, cap: int = 1 << 20):
+        """pct_paths_flagged: (ascending history indices whose flags intersect mask [at most cap], total matching)."""
+        import numpy as np
+        idx = np.zeros(max(cap, 1), dtype=np.int64)
+        n = C.c_int64()
+        self._check(self._L.pct_paths_flagged(self._h, paths._h, int(mask), idx.ctypes.data, int(cap), C.byref(n),
+                                              _stream_ptr(self.device)))
+        return idx[:min(n.value, cap)].copy(), n.value
 
     def forward_project(self, paths: Paths, x: torch.Tensor, out: Optional[torch.Tensor] = None) -> torch.Tensor:
         b = out if out is not None else torch.empty(paths.m, dtype=torch.float32, device=self.device)

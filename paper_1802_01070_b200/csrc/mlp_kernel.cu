@@ -14,143 +14,103 @@ namespace pct {
 
 __device__ __forceinline__ double face_coord(const DevCfg& g, int a, int i) { return fma((double)i, g.h, g.lo[a]); }
 
-struct Step { int axis, dir; double s; bool tie; };
-
-// R9 closed-voxel lazy stepping.  0: B inside closed box(c), 1: stepped, 2: stepped out of the grid.
-__device__ __forceinline__ int lazy_step(const DevCfg& g, const double (&A)[3], const double (&B)[3], double seg_len,
-                                         int (&c)[3], Step& st) {
-    double s[3];
-    int dir[3];
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        const double f_lo = face_coord(g, a, c[a]), f_hi = face_coord(g, a, c[a] + 1);
-        dir[a] = 0; s[a] = 0.0;
-        if (B[a] > f_hi) { dir[a] = 1; s[a] = (f_hi - A[a]) / (B[a] - A[a]); }
-        else if (B[a] < f_lo) { dir[a] = -1; s[a] = (f_lo - A[a]) / (B[a] - A[a]); }
-    }
-    int best = -1;
-    double sb = 0.0;
-#pragma unroll
-    for (int a = 0; a < 3; ++a)
-        if (dir[a] != 0 && (best < 0 || s[a] < sb)) { best = a; sb = s[a]; }
-    if (best < 0) return 0;
-    bool tie = false;
-    int db = 0;
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        if (a != best && dir[a] != 0 && (s[a] - sb) * seg_len < g.tie_eps) tie = true;
-        if (a == best) { c[a] += dir[a]; db = dir[a]; }
-    }
-    st.axis = best; st.dir = db; st.s = sb; st.tie = tie;
-    const bool in = c[0] >= 0 && c[0] < g.nx && c[1] >= 0 && c[1] < g.ny && c[2] >= 0 && c[2] < g.nz;
-    return in ? 1 : 2;
-}
-
 struct Hit { bool ok, tie; int c[3]; double P[3]; };
 
-// A1 / R3-R4: slab-clip the ray {T + s d, s >= 0} to the grid box, then walk the chord to the first hull voxel.
-// The clip box is the bounding box of the hull voxels (g.bmin..g.bmax; the whole grid if hull == NULL): a straight
-// chord visits the same voxels wherever the walk starts, so the air between the grid faces and that box is skipped.
-// Crossing parameters inside the loop use one reciprocal per axis instead of a division per step; a decision that
-// this could change is a tie far below tie_eps and is flagged as such; the entry point P_0 itself is recomputed with
-// the exact quotient of the last crossing.
+// A1 / R3-R4: from the tracker point T along d (not normalised) to the first hull voxel V_s and the point P_0 where the
+// ray enters it.  Written as a ray-parameter traversal (Amanatides & Woo): the point is T + s d, s >= 0, and everything
+// is expressed in s -- the interval [s_in, s_out] in which the ray is inside the search box, and per axis the parameter
+// s_next[a] of the next voxel face.  The search box is the bounding box of the hull voxels (g.bmin..g.bmax; the whole
+// grid if hull == NULL): a straight ray visits the same voxels wherever the traversal starts, so the air between the
+// grid faces and that box is skipped.  Decisions (which face comes first) are those of rule R9 applied to the chord of
+// the ray in the box; two faces closer than tie_eps along the ray set the tie flag.  Inside the loop s_next uses one
+// reciprocal per axis; P_0 is computed from the exact quotient of the face that was crossed last.
 __device__ __noinline__ void find_hull(const DevCfg& g, const uint8_t* __restrict__ hull, const double (&T)[3],
                                        const double (&d)[3], Hit& hit) {
     hit.ok = false; hit.tie = false;
-    double blo[3], bhi[3];
-#pragma unroll
-    for (int a = 0; a < 3; ++a) { blo[a] = face_coord(g, a, g.bmin[a]); bhi[a] = face_coord(g, a, g.bmax[a] + 1); }
-    double s_min = 0.0, s_max = INFINITY, near_s[3];
-    int enter_axis = -1;
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        near_s[a] = -INFINITY;
-        if (d[a] != 0.0) {
-            const double s1 = (blo[a] - T[a]) / d[a], s2 = (bhi[a] - T[a]) / d[a];
-            near_s[a] = fmin(s1, s2);
-            if (near_s[a] > s_min) { s_min = near_s[a]; enter_axis = a; }
-            s_max = fmin(s_max, fmax(s1, s2));
-        } else if (T[a] < blo[a] || T[a] > bhi[a]) return;
-    }
-    if (!(s_min < s_max)) return;
     const double d_len = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
-    double A[3], B[3];
-    int c[3];
+    const double tie_s = d_len > 0.0 ? g.tie_eps / d_len : 0.0;        // tie_eps (mm along the ray) as a parameter difference
+    // per axis: the parameter interval in which the ray is between the box's two faces
+    double s_in = 0.0, s_out = INFINITY, s_enter[3];
+    int ax_in = -1;                                                    // axis through whose face the ray enters (-1: T is inside)
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-        A[a] = T[a] + s_min * d[a];
-        B[a] = T[a] + s_max * d[a];
-        if (a == enter_axis) {
-            A[a] = d[a] > 0 ? blo[a] : bhi[a];
-            c[a] = d[a] > 0 ? g.bmin[a] : g.bmax[a];
-        } else {
-            if (enter_axis >= 0 && (s_min - near_s[a]) * d_len < g.tie_eps) hit.tie = true;
-            const int i = (int)floor((A[a] - g.lo[a]) / g.h);
-            c[a] = min(max(i, g.bmin[a]), g.bmax[a]);
-        }
+        const double b_lo = face_coord(g, a, g.bmin[a]), b_hi = face_coord(g, a, g.bmax[a] + 1);
+        s_enter[a] = -INFINITY;
+        if (d[a] > 0.0) { s_enter[a] = (b_lo - T[a]) / d[a]; s_out = fmin(s_out, (b_hi - T[a]) / d[a]); }
+        else if (d[a] < 0.0) { s_enter[a] = (b_hi - T[a]) / d[a]; s_out = fmin(s_out, (b_lo - T[a]) / d[a]); }
+        else if (T[a] < b_lo || T[a] > b_hi) return;                   // parallel to this slab and outside it
+        if (s_enter[a] > s_in) { s_in = s_enter[a]; ax_in = a; }
     }
-    const double dx = B[0] - A[0], dy = B[1] - A[1], dz = B[2] - A[2];
-    const double seg_len = sqrt(dx * dx + dy * dy + dz * dz);
-    Step last; last.axis = -1; last.dir = 0; last.s = 0.0; last.tie = false;
+    if (!(s_in < s_out)) return;                                       // the ray passes beside the box (or only touches it)
+    // entry voxel: the boundary index on the entering axis, the voxel containing the entry point on the other two
+    int c[3], step[3], left[3], dlin[3];
+    double inv[3], s_next[3], P[3];
+    const int stride[3] = {1, g.nx, g.nx * g.ny};
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        step[a] = d[a] > 0.0 ? 1 : (d[a] < 0.0 ? -1 : 0);
+        if (a == ax_in) {
+            c[a] = step[a] > 0 ? g.bmin[a] : g.bmax[a];
+            P[a] = face_coord(g, a, step[a] > 0 ? g.bmin[a] : g.bmax[a] + 1);         // on the face, exactly
+        } else {
+            if (ax_in >= 0 && s_in - s_enter[a] < tie_s) hit.tie = true;             // enters through an edge of the box
+            P[a] = fma(s_in, d[a], T[a]);
+            c[a] = min(max((int)floor((P[a] - g.lo[a]) / g.h), g.bmin[a]), g.bmax[a]);
+        }
+        left[a] = step[a] > 0 ? g.bmax[a] - c[a] : c[a] - g.bmin[a];                  // steps this axis may still take in the box
+        dlin[a] = step[a] * stride[a];
+        inv[a] = step[a] != 0 ? 1.0 / d[a] : 0.0;
+    }
+    int crossed = -1;                                                   // axis of the face crossed last (-1: none yet)
     if (hull != nullptr) {
-        // incremental form of the R9 rule along one chord: per axis the next face in the direction of travel, its
-        // crossing parameter s = (face - A) * 1/(B - A), refreshed only on the axis that was stepped
-        // se[a] = s of the next crossing on axis a, or +inf if B does not lie strictly beyond that face (not a candidate);
-        // left[a] = steps the axis may still take inside the hull's bounding box
-        double inv[3], se[3];
-        int dir[3], left[3], dlin[3];
-        const int stride[3] = {1, g.nx, g.nx * g.ny};
+        // a face is a candidate while the ray's exit point of the box lies strictly beyond it (rule R9 on the chord);
+        // s_next[a] = +inf marks "no further face on this axis"
+        double E[3];
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
-            const double dd = B[a] - A[a];
-            dir[a] = dd > 0.0 ? 1 : (dd < 0.0 ? -1 : 0);
-            inv[a] = dir[a] != 0 ? 1.0 / dd : 0.0;
-            const double fnext = face_coord(g, a, c[a] + (dir[a] > 0 ? 1 : 0));
-            const bool cand = dir[a] > 0 ? B[a] > fnext : (dir[a] < 0 ? B[a] < fnext : false);
-            se[a] = cand ? (fnext - A[a]) * inv[a] : INFINITY;
-            left[a] = dir[a] > 0 ? g.bmax[a] - c[a] : c[a] - g.bmin[a];
-            dlin[a] = dir[a] * stride[a];
+            E[a] = fma(s_out, d[a], T[a]);
+            const double f = face_coord(g, a, c[a] + (step[a] > 0 ? 1 : 0));
+            const bool cand = step[a] > 0 ? E[a] > f : (step[a] < 0 ? E[a] < f : false);
+            s_next[a] = cand ? (f - T[a]) * inv[a] : INFINITY;
         }
-        const double tie_thr = seg_len > 0.0 ? g.tie_eps / seg_len : 0.0;
         int lin = c[0] + g.nx * (c[1] + g.ny * c[2]);
         while (hull[lin] == 0) {
-            int best = 0;
-            double sb = se[0];
-            if (se[1] < sb) { best = 1; sb = se[1]; }                       // strict: x before y before z on equality
-            if (se[2] < sb) { best = 2; sb = se[2]; }
-            if (sb == INFINITY) return;                                     // chord ends without meeting the hull
-            if ((best != 0 && se[0] - sb < tie_thr) || (best != 1 && se[1] - sb < tie_thr) || (best != 2 && se[2] - sb < tie_thr)) hit.tie = true;
-#define PCT_HULL_MOVE(a)                                                                                       \
+            int ax = 0;
+            double sb = s_next[0];
+            if (s_next[1] < sb) { ax = 1; sb = s_next[1]; }                 // strict: x before y before z on equality
+            if (s_next[2] < sb) { ax = 2; sb = s_next[2]; }
+            if (sb == INFINITY) return;                                     // the chord ends without meeting the hull
+            if ((ax != 0 && s_next[0] - sb < tie_s) || (ax != 1 && s_next[1] - sb < tie_s) || (ax != 2 && s_next[2] - sb < tie_s)) hit.tie = true;
+#define PCT_HULL_ADVANCE(a)                                                                                    \
             {                                                                                                  \
-                c[a] += dir[a];                                                                                \
+                c[a] += step[a];                                                                               \
                 if (--left[a] < 0) return;                     /* left the hull's bounding box: miss */         \
                 lin += dlin[a];                                                                                \
-                const double fnext = face_coord(g, a, c[a] + (dir[a] > 0 ? 1 : 0));                            \
-                const bool cand = dir[a] > 0 ? B[a] > fnext : B[a] < fnext;                                    \
-                se[a] = cand ? (fnext - A[a]) * inv[a] : INFINITY;                                             \
-                last.axis = a; last.dir = dir[a];                                                              \
+                const double f = face_coord(g, a, c[a] + (step[a] > 0 ? 1 : 0));                               \
+                const bool cand = step[a] > 0 ? E[a] > f : E[a] < f;                                           \
+                s_next[a] = cand ? (f - T[a]) * inv[a] : INFINITY;                                             \
             }
-            if (best == 0) PCT_HULL_MOVE(0)
-            else if (best == 1) PCT_HULL_MOVE(1)
-            else PCT_HULL_MOVE(2)
-#undef PCT_HULL_MOVE
-        }
-        if (last.axis >= 0) {
-#pragma unroll
-            for (int a = 0; a < 3; ++a)
-                if (a == last.axis) {
-                    const double face = last.dir > 0 ? face_coord(g, a, c[a]) : face_coord(g, a, c[a] + 1);
-                    last.s = (face - A[a]) / (B[a] - A[a]);
-                }
+            if (ax == 0) PCT_HULL_ADVANCE(0)
+            else if (ax == 1) PCT_HULL_ADVANCE(1)
+            else PCT_HULL_ADVANCE(2)
+#undef PCT_HULL_ADVANCE
+            crossed = ax;
         }
     }
+    if (crossed >= 0) {
+        // P_0 = the point of the ray on the face through which V_s was entered: exact quotient, exact face coordinate
+        double face = 0.0, s_hit = 0.0;
 #pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        hit.c[a] = c[a];
-        double p = last.axis < 0 ? A[a] : A[a] + last.s * (B[a] - A[a]);
-        if (a == last.axis) p = last.dir > 0 ? face_coord(g, a, c[a]) : face_coord(g, a, c[a] + 1);
-        hit.P[a] = p;
+        for (int a = 0; a < 3; ++a)
+            if (a == crossed) { face = face_coord(g, a, c[a] + (step[a] > 0 ? 0 : 1)); s_hit = (face - T[a]) / d[a]; }
+#pragma unroll
+        for (int a = 0; a < 3; ++a) P[a] = a == crossed ? face : fma(s_hit, d[a], T[a]);
+    } else if (ax_in < 0) {
+#pragma unroll
+        for (int a = 0; a < 3; ++a) P[a] = T[a];                            // the tracker point itself lies in a hull voxel
     }
+#pragma unroll
+    for (int a = 0; a < 3; ++a) { hit.c[a] = c[a]; hit.P[a] = P[a]; }
     hit.ok = true;
 }
 
@@ -674,6 +634,27 @@ __global__ void __launch_bounds__(128) k_decode(const __grid_constant__ DevCfg g
         v += (code & 1) ? -mag : mag;
         out[k] = v;
     }
+}
+
+// ---- indices of the histories whose flags intersect `mask` (the tie log, R9) ------------------------------------------
+__global__ void __launch_bounds__(256) k_collect_flagged(const uint8_t* __restrict__ flags, int64_t m, unsigned mask,
+                                                         uint32_t* __restrict__ idx, int64_t cap, unsigned long long* __restrict__ count) {
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < m; i += stride) {
+        if (flags[i] & mask) {
+            const unsigned long long slot = atomicAdd(count, 1ull);
+            if ((int64_t)slot < cap) idx[slot] = (uint32_t)i;
+        }
+    }
+}
+
+int launch_collect_flagged(pct_ctx* ctx, const pct_paths* P, unsigned mask, uint32_t* idx, int64_t cap, unsigned long long* d_count, cudaStream_t st) {
+    PCT_CUDA(ctx, cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), st));
+    const int64_t want = (P->m + 255) / 256, lim = (int64_t)ctx->num_sms * 16;
+    k_collect_flagged<<<(unsigned)(want < lim ? want : lim), 256, 0, st>>>(P->flags, P->m, mask, idx, cap, d_count);
+    ++ctx->launches;
+    PCT_CUDA(ctx, cudaGetLastError());
+    return PCT_OK;
 }
 
 int launch_decode(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, const uint64_t* row_ptr, int32_t* voxels,

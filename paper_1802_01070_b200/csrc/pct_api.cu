@@ -132,6 +132,11 @@ struct DeviceGuard {
     ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
 };
 
+// rows are only meaningful on the grid and device they were generated for
+static bool same_grid(const pct_ctx* ctx, const pct_paths* P) {
+    return P->device == ctx->device && P->nx == ctx->geom.nx && P->ny == ctx->geom.ny && P->nz == ctx->geom.nz && P->n_vox == ctx->n_vox;
+}
+
 static void free_paths_arrays(pct_paths* P) {
     cudaDeviceSynchronize();         // the buffers go back to the pool on the legacy stream: nothing may still use them
     cache_free(P->N); cache_free(P->start); cache_free(P->end); cache_free(P->ell); cache_free(P->flags); cache_free(P->code_off); cache_free(P->codes);
@@ -310,12 +315,14 @@ int pct_generate_mlp(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hull, v
     if (!P) return set_error(ctx, PCT_E_OOM, "host allocation");
     std::memset(P, 0, sizeof(*P));
     P->device = ctx->device; P->m = pr->m; P->n_vox = ctx->n_vox;
+    P->nx = ctx->geom.nx; P->ny = ctx->geom.ny; P->nz = ctx->geom.nz;
     const int64_t m = pr->m;
     const size_t mm = (size_t)(m > 0 ? m : 1);
     ulonglong2* stage = nullptr;
     uint32_t* nchunks = nullptr;
     int rc = PCT_OK;
-    auto fail = [&](int code) { cache_free(stage); cache_free(nchunks); free_paths_arrays(P); delete P; return code; };
+    // kernels of this call may still be running on `st`: drain it before any block goes back to the (process-wide) cache
+    auto fail = [&](int code) { cudaStreamSynchronize(st); cudaGetLastError(); cache_free(stage); cache_free(nchunks); free_paths_arrays(P); delete P; return code; };
 #define GEN_CUDA(call)                                                                                          \
     do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { cudaGetLastError();                               \
         return fail(set_error(ctx, e__ == cudaErrorMemoryAllocation ? PCT_E_OOM : PCT_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e__))); } } while (0)
@@ -398,6 +405,7 @@ int pct_paths_decode(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, i
                      float* ell, uint8_t* flags, void* stream) {
     if (!ctx) return PCT_E_INVALID_ARG;
     if (!P || !row_ptr || i0 < 0 || i1 > P->m || i0 > i1) return set_error(ctx, PCT_E_INVALID_ARG, "bad decode range");
+    if (!same_grid(ctx, P)) return set_error(ctx, PCT_E_INVALID_ARG, "paths were generated on another grid or device");
     DeviceGuard guard(ctx->device);
     cudaStream_t st = (cudaStream_t)stream;
     const int64_t cnt = i1 - i0;
@@ -417,16 +425,46 @@ int pct_paths_decode(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, i
     return PCT_OK;
 }
 
+int pct_paths_flagged(pct_ctx* ctx, const pct_paths* P, uint32_t mask, int64_t* idx_out, int64_t cap, int64_t* n_out, void* stream) {
+    if (!ctx) return PCT_E_INVALID_ARG;
+    if (!P || !n_out || cap < 0 || (cap > 0 && !idx_out)) return set_error(ctx, PCT_E_INVALID_ARG, "bad flagged-list arguments");
+    if (!same_grid(ctx, P)) return set_error(ctx, PCT_E_INVALID_ARG, "paths were generated on another grid or device");
+    DeviceGuard guard(ctx->device);
+    cudaStream_t st = (cudaStream_t)stream;
+    *n_out = 0;
+    if (P->m == 0) return PCT_OK;
+    uint32_t* d_idx = nullptr;
+    const int64_t keep = cap < P->m ? cap : P->m;
+    PCT_CUDA(ctx, cache_alloc((void**)&d_idx, sizeof(uint32_t) * (size_t)(keep > 0 ? keep : 1)));
+    int rc = launch_collect_flagged(ctx, P, mask, d_idx, keep, ctx->d_total, st);
+    unsigned long long n = 0;
+    std::vector<uint32_t> host((size_t)keep);
+    cudaError_t e = rc == PCT_OK ? cudaMemcpyAsync(&n, ctx->d_total, sizeof(n), cudaMemcpyDeviceToHost, st) : cudaSuccess;
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    const int64_t got = (int64_t)n < keep ? (int64_t)n : keep;
+    if (e == cudaSuccess && got > 0) e = cudaMemcpy(host.data(), d_idx, sizeof(uint32_t) * (size_t)got, cudaMemcpyDeviceToHost);
+    cudaStreamSynchronize(st);
+    cache_free(d_idx);
+    if (rc != PCT_OK) return rc;
+    if (e != cudaSuccess) { cudaGetLastError(); return set_error(ctx, PCT_E_CUDA, "flagged list: %s", cudaGetErrorString(e)); }
+    std::sort(host.begin(), host.begin() + got);
+    for (int64_t k = 0; k < got; ++k) idx_out[k] = (int64_t)host[(size_t)k];
+    *n_out = (int64_t)n;
+    return PCT_OK;
+}
+
 int pct_forward_project(pct_ctx* ctx, const pct_paths* P, const float* x, float* b_out, void* stream) {
     if (!ctx) return PCT_E_INVALID_ARG;
-    if (!P || !x || (!b_out && P->m > 0) || P->n_vox != ctx->n_vox) return set_error(ctx, PCT_E_INVALID_ARG, "bad forward_project arguments");
+    if (!P || !x || (!b_out && P->m > 0)) return set_error(ctx, PCT_E_INVALID_ARG, "bad forward_project arguments");
+    if (!same_grid(ctx, P)) return set_error(ctx, PCT_E_INVALID_ARG, "paths were generated on another grid or device");
     DeviceGuard guard(ctx->device);
     return launch_forward_project(ctx, P, x, b_out, (cudaStream_t)stream);
 }
 
 int pct_column_counts(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, uint32_t* counts, void* stream) {
     if (!ctx) return PCT_E_INVALID_ARG;
-    if (!P || !counts || i0 < 0 || i1 > P->m || i0 > i1 || P->n_vox != ctx->n_vox) return set_error(ctx, PCT_E_INVALID_ARG, "bad column_counts arguments");
+    if (!P || !counts || i0 < 0 || i1 > P->m || i0 > i1) return set_error(ctx, PCT_E_INVALID_ARG, "bad column_counts arguments");
+    if (!same_grid(ctx, P)) return set_error(ctx, PCT_E_INVALID_ARG, "paths were generated on another grid or device");
     DeviceGuard guard(ctx->device);
     return launch_column_counts(ctx, P, i0, i1, counts, (cudaStream_t)stream);
 }
@@ -435,8 +473,9 @@ int pct_column_counts(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, 
 int pct_solve(pct_ctx* ctx, const pct_paths* P, const float* b, const float* x0, int iters, int64_t block_size, float lambda,
               float* x_out, void* stream) {
     if (!ctx) return PCT_E_INVALID_ARG;
-    if (!P || (!b && P->m > 0) || !x0 || !x_out || iters < 0 || block_size < 1 || P->n_vox != ctx->n_vox || !std::isfinite(lambda))
+    if (!P || (!b && P->m > 0) || !x0 || !x_out || iters < 0 || block_size < 1 || !std::isfinite(lambda))
         return set_error(ctx, PCT_E_INVALID_ARG, "bad solve arguments");
+    if (!same_grid(ctx, P)) return set_error(ctx, PCT_E_INVALID_ARG, "paths were generated on another grid or device");
     DeviceGuard guard(ctx->device);
     cudaStream_t st = (cudaStream_t)stream;
     int rc;
@@ -522,7 +561,10 @@ int pct_reconstruct_host(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hul
     int rc = PCT_OK;
     auto cleanup = [&]() {
         ctx->batch_ready = nullptr; ctx->n_batch_ready = 0;
+        // on the error paths kernels and copies may still be in flight: nothing returns to the cache before both streams drain
+        cudaStreamSynchronize(st);
         if (cs) cudaStreamSynchronize(cs);
+        cudaGetLastError();
         cache_free(d_tr); cache_free(d_b); cache_free(d_x); cache_free(d_hull);
         if (P) pct_paths_free(P);
         for (auto& e : ev) if (e) cudaEventDestroy(e);
@@ -553,7 +595,7 @@ int pct_reconstruct_host(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hul
     for (auto& e : ready) REC_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     REC_CUDA(cudaEventRecord(ev[0], st));
     REC_CUDA(cudaEventRecord(ev_alloc, st));
-    REC_CUDA(cudaStreamWaitEvent(cs, ev_alloc, 0));          // the stream-ordered allocations above
+    REC_CUDA(cudaStreamWaitEvent(cs, ev_alloc, 0));          // the copy stream starts behind whatever `st` still runs on these (reused) blocks
     // small inputs first: the copy engine serves requests in issue order, and K1 needs the hull before its first batch
     if (hull_host) REC_CUDA(cudaMemcpyAsync(d_hull, hull_host, (size_t)n, cudaMemcpyHostToDevice, st));
     if (x0_host) REC_CUDA(cudaMemcpyAsync(d_x, x0_host, sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, st));

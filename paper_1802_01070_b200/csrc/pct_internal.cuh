@@ -147,6 +147,7 @@ struct pct_ctx {
 
 struct pct_paths {
     int device;
+    int nx, ny, nz;      // grid the rows were generated on: every later call checks its context against them
     int64_t m, n_vox;
     uint32_t* N;         // path entries per history
     int32_t* start;      // start voxel
@@ -204,5 +205,6 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
 void free_solve_plan(SolvePlan* plan);
 int launch_block_update(pct_ctx* ctx, float* x, float2* ds, float* dsum, uint32_t* counts, bool store, float lambda, cudaStream_t st);
 int launch_fill(pct_ctx* ctx, float* p, int64_t n, float value, cudaStream_t st);
+int launch_collect_flagged(pct_ctx* ctx, const pct_paths* P, unsigned mask, uint32_t* idx, int64_t cap, unsigned long long* d_count, cudaStream_t st);
 
 }  // namespace pct

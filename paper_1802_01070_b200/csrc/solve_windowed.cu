@@ -114,6 +114,7 @@ __device__ __forceinline__ void walk_slab(const unsigned long long* __restrict__
 template <bool COUNT>
 __global__ void __launch_bounds__(GROUP, 2)
 k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, const float* __restrict__ ell,
+                 const int32_t* __restrict__ start, const uint64_t* __restrict__ code_off, const ulonglong2* __restrict__ codes,
                  const uint32_t* __restrict__ perm, const uint32_t* __restrict__ p0, const uint8_t* __restrict__ pflag,
                  const uint8_t* __restrict__ cnt, const unsigned long long* __restrict__ stream,
                  PlanGroup* __restrict__ groups, const uint32_t* __restrict__ launch_order, int64_t group0, const float* __restrict__ b, const float* __restrict__ x,
@@ -121,8 +122,11 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
     extern __shared__ __align__(16) unsigned char smem[];
     __shared__ unsigned tbl[8];
     __shared__ float red[GROUP / 32];
+    __shared__ unsigned ehist[256];               // members per binade of |c_i| (R21: robust fixed-point scale)
+    __shared__ int e_med;
     __shared__ PlanGroup Gs;
     if (threadIdx.x == 0) Gs = groups[launch_order[group0 + blockIdx.x]];
+    if (threadIdx.x < 256) ehist[threadIdx.x] = 0u;
     __syncthreads();
     const PlanGroup& G = Gs;
     if (G.cls == 7 || G.nslab == 0 || G.wps == 0) return;
@@ -192,30 +196,63 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
         walk_slab(my_stream + (size_t)s * G.wps * GROUP, w0, cmax, tbl_s, p, [&](unsigned q) { S += lds_f32(win_addr(q)); });
     }
     // ---- c_i and the CTA's fixed-point scale (R17, R21) -----------------------------------------------------------------
+    // The scale must not be set by an outlier (an absurd WEPL makes |c_i| orders of magnitude larger than its neighbours'
+    // and would coarsen the quantum of all 1024 members) nor by a non-finite value.  So: the CTA takes the MEDIAN binade
+    // of the finite |c_i| (histogram of the FP32 exponents), caps the scale at 64 x that binade, and every member whose
+    // c_i is not finite or lies beyond the cap is "late": it adds nothing to the fixed-point window and instead walks its
+    // row once with red.global.add.f32, exactly as the direct kernel does (Inf / NaN propagate the same way).
     float ci = 0.f;
-    if (active && n_vis > 0) {
+    const bool has = active && n_vis > 0;
+    if (has) {
         const float l = ell[i];
         ci = (b[i] - l * S) / ((float)n_vis * l);
     }
-    float mx = fabsf(ci);
+    const float aci = fabsf(ci);
+    const bool finite = aci < INFINITY;                                  // false for Inf and NaN
+    {
+        const unsigned e = (has && finite && aci > 0.f) ? (__float_as_uint(aci) >> 23) : 0xFFFFFFFFu;
+        const unsigned peers = __match_any_sync(0xffffffffu, e);
+        if (e != 0xFFFFFFFFu && (tid & 31) == __ffs(peers) - 1) atomicAdd(&ehist[e], (unsigned)__popc(peers));
+    }
+    float mx = finite ? aci : 0.f;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-    __syncthreads();                              // all walkers done with xs
+    __syncthreads();                              // all walkers done with xs; ehist complete
     if ((tid & 31) == 0) red[tid >> 5] = mx;
     int* dl = reinterpret_cast<int*>(win);
 #pragma unroll
     for (int k = 0; k < 2 * WIN_SLOTS / GROUP; ++k) dl[tid + k * GROUP] = 0;      // clears Delta and s
+    if (tid < 32) {                               // median binade: lane l owns bins 8l .. 8l+7
+        unsigned mine = 0u;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) mine += ehist[tid * 8 + k];
+        unsigned incl = mine;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const unsigned y = __shfl_up_sync(0xffffffffu, incl, o); if (tid >= o) incl += y; }
+        const unsigned total = __shfl_sync(0xffffffffu, incl, 31), half = (total + 1u) >> 1;
+        const unsigned at = __ballot_sync(0xffffffffu, incl >= half && total > 0u);
+        if (total == 0u) { if (tid == 0) e_med = -1; }
+        else if (tid == __ffs(at) - 1) {
+            unsigned cum = incl - mine;
+            int bin = tid * 8;
+            for (int k = 0; k < 8; ++k) { cum += ehist[tid * 8 + k]; if (cum >= half) { bin = tid * 8 + k; break; } }
+            e_med = bin;
+        }
+    }
     __syncthreads();
     mx = red[0];
 #pragma unroll
     for (int k = 1; k < GROUP / 32; ++k) mx = fmaxf(mx, red[k]);
-    int ex = 0;
-    if (mx > 0.f && mx < INFINITY) frexpf(mx, &ex);              // mx < 2^ex
     int fix = FIX_BITS;
     if (!COUNT && G.max_cnt > 0) fix = min(29, max(FIX_BITS, 30 - (32 - __clz(G.max_cnt))));     // max_cnt < 2^(32 - clz)
+    int ex = 0;
+    if (mx > 0.f) frexpf(mx, &ex);                               // every finite |c_i| < 2^ex
+    if (e_med >= 0) ex = min(ex, e_med - 120);                   // 64 x the median's binade [2^(e-127), 2^(e-126))
+    ex = max(ex, fix - 126);                                     // keeps both scales normal FP32 numbers
     const float scale = exp2f((float)(fix - ex)), inv_scale = exp2f((float)(ex - fix));
+    const bool late = has && !(aci < ldexpf(1.f, ex));           // beyond the cap, Inf or NaN
     unsigned my_max = 0u;
-    const int cfix = __float2int_rn(ci * scale);
+    const int cfix = late ? 0 : __float2int_rn(ci * scale);
 
     // ---- pass 2: {Delta, s} += {c_i, 1} on every visit; flush per slab -------------------------------------------------
     p = win_s + p_init + (COUNT ? 0u : (unsigned)(tid & 1) * (WIN_SLOTS * 4));     // odd lanes: second Delta copy
@@ -258,6 +295,22 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
         }
         __syncthreads();
     }
+    if (late) {
+        // this member's Delta contributions go straight to the global accumulator (its visits were counted in the window)
+        const unsigned long long* cp = reinterpret_cast<const unsigned long long*>(codes + code_off[i]);
+        int v = start[i];
+        unsigned long long w = 0ull;
+        for (uint32_t k = 0; k < n_vis; ++k) {
+            if (k > 0) {
+                const uint32_t f = (k - 1) % CODES_PER_WORD;
+                if (f == 0) w = __ldg(cp++);
+                const int code = (int)((w >> (3 * f)) & 7ull);
+                const int mag = (code >> 1) == 0 ? g.sx : ((code >> 1) == 1 ? g.sy : g.sz);
+                v += (code & 1) ? -mag : mag;
+            }
+            red_add_f32(COUNT ? &ds[v].x : dsum + v, ci);
+        }
+    }
     if (COUNT) {        // remember the largest slot count for the sweeps that reuse the cached counts
         my_max = __reduce_max_sync(0xffffffffu, my_max);
         if ((tid & 31) == 0 && my_max > 0u) atomicMax(&groups[launch_order[group0 + blockIdx.x]].max_cnt, (int)my_max);
@@ -275,10 +328,10 @@ int launch_block_windowed(pct_ctx* ctx, const pct_paths* P, const SolvePlan* pla
     }
     ProfScope prof(ctx, 1, st);
     if (count)
-        k_block_windowed<true><<<(unsigned)(g1 - g0), GROUP, K2W_SMEM, st>>>(ctx->cfg, P->N, P->ell, plan->perm, plan->p0, plan->pflag,
+        k_block_windowed<true><<<(unsigned)(g1 - g0), GROUP, K2W_SMEM, st>>>(ctx->cfg, P->N, P->ell, P->start, P->code_off, P->codes, plan->perm, plan->p0, plan->pflag,
                                                                             plan->cnt, plan->stream, plan->groups, plan->launch_order, g0, b, x, ds, dsum);
     else
-        k_block_windowed<false><<<(unsigned)(g1 - g0), GROUP, K2W_SMEM, st>>>(ctx->cfg, P->N, P->ell, plan->perm, plan->p0, plan->pflag,
+        k_block_windowed<false><<<(unsigned)(g1 - g0), GROUP, K2W_SMEM, st>>>(ctx->cfg, P->N, P->ell, P->start, P->code_off, P->codes, plan->perm, plan->p0, plan->pflag,
                                                                              plan->cnt, plan->stream, plan->groups, plan->launch_order, g0, b, x, ds, dsum);
     ++ctx->launches;
     PCT_CUDA(ctx, cudaGetLastError());

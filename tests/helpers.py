@@ -1,7 +1,7 @@
 """Shared test helpers (input marshalling only; no method arithmetic)."""
 import numpy as np
 
-from paper_1802_01070_b200 import synth
+import synth
 
 
 def oracle_setup(pcto, cfg, protons, hull=None, params_override=None, nthreads=0):

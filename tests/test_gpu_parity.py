@@ -10,7 +10,7 @@ import numpy as np
 import pytest
 import torch
 
-from paper_1802_01070_b200 import synth
+import synth
 from helpers import oracle_setup, split_rows
 
 pytestmark = pytest.mark.gpu
@@ -227,6 +227,14 @@ def test_full_size_sampled(binding, oracle, name):
                 assert (flags_g[r] | flags_o[r]) & binding.TIE
                 total_mis += 1
     assert total_mis <= 1
+    # the tie log (north_star: ties are logged, fraction < 1e-6): every tie-flagged history by index
+    tie_idx, n_tie = ctx.paths_flagged(paths, binding.TIE)
+    assert n_tie == paths.n_ties == len(tie_idx) and n_tie <= max(1, int(1e-6 * m)) + 24
+    print(f"[tie log] {name}: {n_tie} tie-flagged histories of {m}: {tie_idx.tolist()}")
+    log_dir = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+    if os.path.isdir(log_dir):
+        with open(os.path.join(log_dir, f"tie_log_{name}.txt"), "w") as f:
+            f.write(f"# {name}: {n_tie} tie-flagged histories (PCT_TIE, R9) of {m}; indices:\n" + "\n".join(map(str, tie_idx.tolist())) + "\n")
     # properties that hold at any size: forward_project(1) = L_i = N_i * l_i; sum of counts = sum of N
     row_ptr, _, ell, flags = ctx.paths_decode(paths, 0, 200_000)
     N = torch.diff(row_ptr).to(torch.float64)
@@ -236,14 +244,22 @@ def test_full_size_sampled(binding, oracle, name):
     counts = ctx.column_counts(paths, 0, m)
     assert int(counts.to(torch.int64).sum().item()) == paths.total_visits
     del counts, L, N, row_ptr, ell, flags
-    # two blocks of the configured solve (B = 200 k / 1 M) against the oracle on the same histories
+    # the first blocks of the configured solve (B = 200 k / 1 M / 2 M) against the oracle on the same histories, TWO
+    # sweeps: the first runs the counting kernels (k_block_windowed<true>, k_block_update_store), the second the
+    # cached-count kernels (k_block_windowed<false>, k_block_update_cached4) that do 11 of the 12 timed sweeps of bench.py
     sub_m = min(m, (1 if name == "paperB" else 2) * cfg.block)      # config 3: one block of 2 M (oracle time)
     if os.environ.get("PCT_TEST_SKIP_BLOCKS", "0") != "1":
         sub = {k: v[:sub_m].contiguous() for k, v in pr.items()}
         ctx2, paths2 = gpu_paths(binding, cfg, sub, hull)
-        x_g = ctx2.solve(paths2, sub["wepl"], ones, 1, cfg.block, cfg.lam).cpu().numpy()
+        ctx2.profile_enable(True)
+        x_g = ctx2.solve(paths2, sub["wepl"], ones, 2, cfg.block, cfg.lam).cpu().numpy()
+        prof = ctx2.profile_read()
+        n_blk = -(-sub_m // cfg.block)
+        assert prof["project_windowed"][1] == 2 * n_blk, prof         # plan path, both sweeps
+        info = paths2.plan_info()
+        assert info["n_direct"] < 0.02 * sub_m, info
         g, p, pa, P = oracle_setup(oracle, cfg, {k: v.cpu() for k, v in sub.items()}, hull.cpu())
-        x_o = P.solve(sub["wepl"].cpu().numpy(), np.ones(cfg.n, np.float32), 1, cfg.block, cfg.lam)
+        x_o = P.solve(sub["wepl"].cpu().numpy(), np.ones(cfg.n, np.float32), 2, cfg.block, cfg.lam)
         assert np.linalg.norm(x_g - x_o) / np.linalg.norm(x_o) <= REL_L2_TOL
         assert np.max(np.abs(x_g - x_o)) <= MAX_ABS_TOL
 
@@ -378,3 +394,101 @@ def test_count_cache_ownership_between_plans(binding, oracle):
     x_o = P.solve(pr_a["wepl"].numpy(), np.ones(cfg.n, np.float32), 2, 2500, 0.1)
     assert np.max(np.abs(x_g - x_o)) <= MAX_ABS_TOL
     ctx.trim_cache()
+
+
+# ---- config 4 (BASELINE.json): block-size / relaxation corners on the config-1 phantom ---------------------------------
+def test_config4_corners_on_head_phantom(binding, oracle):
+    """B in {1 k, 10 k, 100 k} x lambda in {0.05, 0.2} on 400 k histories of config 1, two sweeps each: B <= 10 k runs the
+    direct kernels (blocks too sparse for windows), B = 100 k the plan path; each against the oracle."""
+    cfg = synth.CONFIGS["head"]
+    m = 400_000
+    x_true, hull, shadow = synth.make_phantom(cfg, "cuda")
+    pr = synth.generate_protons(cfg, x_true, shadow, device="cuda", i0=0, i1=m)
+    ctx, paths = gpu_paths(binding, cfg, pr, hull)
+    g, p, pa, P = oracle_setup(oracle, cfg, {k: v.cpu() for k, v in pr.items()}, hull.cpu())
+    assert compare_lists(binding, oracle, ctx, paths, P, 0, 20000)[0] <= 1
+    x0 = torch.ones(cfg.n, dtype=torch.float32, device="cuda")
+    b_h = pr["wepl"].cpu().numpy()
+    for B, lam in ((1000, 0.05), (1000, 0.2), (10_000, 0.05), (10_000, 0.2), (100_000, 0.05), (100_000, 0.2)):
+        ctx.profile_enable(True)
+        x_g = ctx.solve(paths, pr["wepl"], x0, 2, B, lam).cpu().numpy()
+        prof = ctx.profile_read()
+        ctx.profile_enable(False)
+        if B >= 100_000:
+            assert prof["project_windowed"][1] == 2 * (m // B), (B, prof)
+        else:
+            assert prof["project_windowed"][1] == 0 and prof["project_direct"][1] == 2 * (m // B), (B, prof)
+        x_o = P.solve(b_h, np.ones(cfg.n, np.float32), 2, B, lam)
+        rel, mx = np.linalg.norm(x_g - x_o) / np.linalg.norm(x_o), np.max(np.abs(x_g - x_o))
+        assert rel <= REL_L2_TOL and mx <= MAX_ABS_TOL, (B, lam, rel, mx)
+
+
+# ---- the fixed-point window against outliers and non-finite data (R21) --------------------------------------------------
+def test_windowed_plan_extreme_outlier_and_nonfinite(binding, oracle):
+    """A 1e6-fold outlier must not coarsen the fixed-point quantum of its group (it is sent through the FP32 global
+    atomics instead), and Inf / NaN in b must propagate exactly as in the direct kernel: same voxels non-finite, all
+    others equal within the tolerance -- whichever path a history takes."""
+    cfg = synth.scaled(synth.CONFIGS["tiny"], 20000)
+    x_true, hull, shadow = synth.make_phantom(cfg)
+    pr = synth.generate_protons(cfg, x_true, shadow)
+    g, p, pa, P = oracle_setup(oracle, cfg, pr, hull)
+    ctx, paths = gpu_paths(binding, cfg, pr, hull)
+    x0 = torch.ones(cfg.n, dtype=torch.float32, device="cuda")
+    wepl = pr["wepl"].clone()
+    wepl[777] = 3.0e7            # |c_i| ~ 1e6 x its neighbours'
+    wepl[9000] = -1.0e7
+    ctx.solve_config(2)
+    x_w = ctx.solve(paths, wepl.cuda(), x0, 3, 5000, 0.1).cpu().numpy()
+    ctx.solve_config(1)
+    x_d = ctx.solve(paths, wepl.cuda(), x0, 3, 5000, 0.1).cpu().numpy()
+    x_o = P.solve(wepl.numpy(), np.ones(cfg.n, np.float32), 3, 5000, 0.1)
+    # the image now holds values ~1e4: the tolerance is relative to them where they are (FP32 atomics, north_star)
+    for x_g in (x_w, x_d):
+        assert np.linalg.norm(x_g - x_o) / np.linalg.norm(x_o) <= REL_L2_TOL
+    # and where the outliers never went, the windowed path is as exact as without them
+    far = np.abs(x_o) < 10.0
+    assert far.sum() > 0.5 * cfg.n
+    assert np.max(np.abs(x_w[far] - x_o[far])) <= MAX_ABS_TOL
+    # Inf and NaN
+    for bad in (np.inf, -np.inf, np.nan):
+        wepl = pr["wepl"].clone()
+        wepl[4321] = bad
+        ctx.solve_config(2)
+        x_w = ctx.solve(paths, wepl.cuda(), x0, 2, 5000, 0.1).cpu().numpy()
+        ctx.solve_config(1)
+        x_d = ctx.solve(paths, wepl.cuda(), x0, 2, 5000, 0.1).cpu().numpy()
+        x_o = P.solve(wepl.numpy(), np.ones(cfg.n, np.float32), 2, 5000, 0.1)
+        nf = ~np.isfinite(x_o)
+        assert nf.sum() > 0
+        assert np.array_equal(~np.isfinite(x_w), nf) and np.array_equal(~np.isfinite(x_d), nf)
+        assert np.max(np.abs(x_w[~nf] - x_o[~nf])) <= MAX_ABS_TOL and np.max(np.abs(x_d[~nf] - x_o[~nf])) <= MAX_ABS_TOL
+    # tiny residuals (scale clamp): b = A x0 exactly representable -> c_i ~ 1e-8 relative noise, result stays x0
+    b_fit = ctx.forward_project(paths, x0)
+    ctx.solve_config(2)
+    x_w = ctx.solve(paths, b_fit, x0, 2, 5000, 0.1).cpu().numpy()
+    assert np.all(np.isfinite(x_w)) and np.max(np.abs(x_w - 1.0)) < 1e-5
+
+
+def test_tie_log_and_grid_mismatch(binding, oracle):
+    """pct_paths_flagged lists exactly the flagged histories; rows generated on one grid are refused by a context of
+    another grid with the same voxel count."""
+    cfg = synth.scaled(synth.CONFIGS["tiny"], 30000)
+    x_true, hull, shadow = synth.make_phantom(cfg)
+    pr = synth.generate_protons(cfg, x_true, shadow)
+    ctx, paths = gpu_paths(binding, cfg, pr, hull)
+    flags = ctx.paths_decode(paths)[3].cpu().numpy()
+    for mask in (binding.TIE, binding.REJECT_MASK, binding.END_MISMATCH | binding.TIE):
+        idx, n = ctx.paths_flagged(paths, mask)
+        assert n == len(idx) and np.array_equal(idx, np.nonzero(flags & mask)[0])
+    idx, n = ctx.paths_flagged(paths, binding.REJECT_MASK, cap=5)
+    assert n == paths.n_rejected and len(idx) == min(5, n) and np.all(flags[idx] & binding.REJECT_MASK)
+    geom = synth.geometry(cfg)
+    other = dict(geom, nx=geom["ny"] // 2, ny=geom["nx"] * 2)          # 16 x 64 x 8: same n, different strides
+    ctx2 = binding.Context(other, synth.mlp_params(cfg), 0)
+    x0 = torch.ones(cfg.n, dtype=torch.float32, device="cuda")
+    with pytest.raises(binding.PctError):
+        ctx2.solve(paths, pr["wepl"].cuda(), x0, 1, 5000, 0.1)
+    with pytest.raises(binding.PctError):
+        ctx2.forward_project(paths, x0)
+    with pytest.raises(binding.PctError):
+        ctx2.column_counts(paths, 0, 10)

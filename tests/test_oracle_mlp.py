@@ -10,7 +10,7 @@ import numpy as np
 import pytest
 from scipy import integrate, interpolate, optimize
 
-from paper_1802_01070_b200 import synth
+import synth
 
 GOLD = os.path.join(os.path.dirname(__file__), "golden", "mlp_survey_values.txt")
 POLY = synth.poly_mm(200.0, 200.0)

@@ -8,7 +8,7 @@ import dataclasses
 import numpy as np
 import pytest
 
-from paper_1802_01070_b200 import synth
+import synth
 from helpers import oracle_setup, split_rows
 
 SMALL = dataclasses.replace(synth.CONFIGS["tiny"], name="tiny-small", nx=8, ny=8, nz=2, u_tracker=8.0, m=160)

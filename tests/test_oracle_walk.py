@@ -9,7 +9,7 @@ import dataclasses
 import numpy as np
 import pytest
 
-from paper_1802_01070_b200 import synth
+import synth
 from helpers import oracle_setup, split_rows
 
 
