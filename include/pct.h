@@ -147,6 +147,11 @@ int pct_solve_config(pct_ctx* ctx, int mode, int64_t min_block);
 /* Statistics of the solve plan cached in `paths` by the last pct_solve that used one (all zero if none). */
 typedef struct {
     int64_t block_size, n_blocks, n_groups, n_direct, plan_bytes;
+    /* what one sweep of the windowed kernel moves (bench.py's roofline): bytes of the slab-aligned code stream and of the
+     * per-(slab, thread) visit counts (HBM, read once per pass), window slots staged from x / flushed to the
+     * accumulator per sweep (L2 gathers / reductions that remain after the shared-memory aggregation), and the
+     * histories and visits that take the windowed kernel */
+    int64_t stream_bytes, cnt_bytes, staged_slots, windowed_histories, windowed_visits;
 } pct_plan_stats;
 int pct_plan_info(const pct_paths* paths, pct_plan_stats* out /* HOST */);
 
@@ -166,11 +171,13 @@ int pct_profile_read(pct_ctx* ctx, pct_profile* out);
 /* Roofline denominators MEASURED_PEAKS.json lacks, measured on ctx's device with register /
  * L2 / shared-memory resident microbenchmarks (best of three launches, CUDA events; ~0.3 s in total):
  * plain FP64 FMA/s (K1), random 4-byte L2 gathers/s over a 64 MiB array, red.global.add.f32/s and .v2.f32/s
- * (random and warp-contiguous addresses), shared-memory 32-bit atomic adds/s and loads/s (random slots).
+ * (random and warp-contiguous addresses), shared-memory 32-bit atomic adds/s and loads/s (random slots, and
+ * conflict-free).
  * out: HOST.  Blocking; uses the legacy default stream. */
 typedef struct {
     double fp64_fma_per_s, l2_gather_per_s, l2_red_f32_per_s, l2_red_v2_per_s, l2_red_v2_coalesced_per_s,
-        smem_atomic_per_s, smem_load_per_s;
+        smem_atomic_per_s, smem_load_per_s;          /* random slots: the bank conflicts of an arbitrary address stream */
+    double smem_atomic_cf_per_s, smem_load_cf_per_s; /* conflict-free (lane l -> bank l): the pipe's own ceiling        */
     int32_t num_sms;
 } pct_peaks;
 int pct_measure_peaks(pct_ctx* ctx, pct_peaks* out);

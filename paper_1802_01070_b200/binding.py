@@ -59,12 +59,14 @@ class Profile(C.Structure):
 
 
 class PlanStats(C.Structure):
-    _fields_ = [(k, C.c_int64) for k in ("block_size", "n_blocks", "n_groups", "n_direct", "plan_bytes")]
+    _fields_ = [(k, C.c_int64) for k in ("block_size", "n_blocks", "n_groups", "n_direct", "plan_bytes", "stream_bytes",
+                                          "cnt_bytes", "staged_slots", "windowed_histories", "windowed_visits")]
 
 
 class Peaks(C.Structure):
     _fields_ = [(k, C.c_double) for k in ("fp64_fma_per_s", "l2_gather_per_s", "l2_red_f32_per_s", "l2_red_v2_per_s",
-                                          "l2_red_v2_coalesced_per_s", "smem_atomic_per_s", "smem_load_per_s")] + [
+                                          "l2_red_v2_coalesced_per_s", "smem_atomic_per_s", "smem_load_per_s",
+                                          "smem_atomic_cf_per_s", "smem_load_cf_per_s")] + [
         ("num_sms", C.c_int32)]
 
 

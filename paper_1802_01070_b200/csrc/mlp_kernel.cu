@@ -2,10 +2,13 @@
 // step codes (A3).  PAPER.md:7 ("calculating the individual proton's most likely path [3]" gives the rows of A),
 // PAPER.md:26 ("each proton as an individual thread").  FP64 throughout; readings R1-R12 of DESIGN.md.
 //
-// One thread per history.  The kernel is bound by the FP64 pipe (a few hundred flop per MLP sample, K ~ 2*depth
-// samples) and by divergence in the walk, not by memory: 72 B in, ~60-170 B out per history.
-// Codes go to a staging buffer laid out [chunk][history-in-batch] (so that a warp's k-th chunks are contiguous)
-// and are compacted to their final 16-byte-aligned position once the batch's sizes are known.
+// Three kernels per batch of 2^20 histories: k_hull (one thread per history: hull entry/exit and the per-history part of
+// the MLP), k_mlp_walk_warp (one WARP per history, lane = MLP sample: the bulk of the FP64 work, all lanes converged) and
+// k_mlp_walk (one thread per history, the sequential rule R9 step by step: the few histories the warp kernel hands over).
+// Bound by the FP64 pipe (~100 FP64 instructions per MLP sample, K ~ 2*depth samples), not by memory: 72 B in, ~60-170 B
+// out per history.  Rows are written straight to the code stream; their place comes from an atomic chunk counter.
+#include <cstdlib>
+
 #include <cub/device/device_radix_sort.cuh>
 
 #include "pct_internal.cuh"
@@ -121,22 +124,20 @@ __device__ __forceinline__ double horner6(const double (&c)[6], double x) {
     return r;
 }
 
-// 16-byte chunk writer: 42 codes, field k at bits 3(k%21) of word k/21; unused fields stay 7 (pad).
 // 16-byte chunk writer: 42 codes, field k at bits 3(k%21) of word k/21; unused fields are 7 (pad).  A code is inserted
 // at the top of the word being filled and the word shifted down by one field per push, so that after 21 pushes the first
 // code sits in field 0 (one funnel shift and one OR per code, no variable shifts).
 struct CodeWriter {
     unsigned long long acc, w0;   // word being filled; finished first word of the chunk
     int nc, chunk;                // codes in the current chunk (0..41); chunks written
-    ulonglong2* stage;            // stage[chunk * stride + p]
-    size_t stride;
-    __device__ __forceinline__ void init(ulonglong2* s, size_t str) { acc = 0ull; w0 = 0ull; nc = 0; chunk = 0; stage = s; stride = str; }
+    ulonglong2* stage;            // stage[chunk]
+    __device__ __forceinline__ void init(ulonglong2* s) { acc = 0ull; w0 = 0ull; nc = 0; chunk = 0; stage = s; }
     __device__ __forceinline__ void push(int code) {
         acc = (acc >> 3) | ((unsigned long long)code << 60);
         ++nc;
         if (nc == CODES_PER_WORD) { w0 = acc; acc = 0ull; }
         else if (nc == CODES_PER_CHUNK) {
-            stage[(size_t)chunk * stride] = make_ulonglong2(w0, acc);
+            stage[chunk] = make_ulonglong2(w0, acc);
             acc = 0ull; nc = 0; ++chunk;
         }
     }
@@ -146,24 +147,31 @@ struct CodeWriter {
     }
     __device__ __forceinline__ int finish() {
         if (nc > 0) {
-            stage[(size_t)chunk * stride] = nc >= CODES_PER_WORD ? make_ulonglong2(w0, partial(acc, nc - CODES_PER_WORD))
-                                                                 : make_ulonglong2(partial(acc, nc), ~0ull);
+            stage[chunk] = nc >= CODES_PER_WORD ? make_ulonglong2(w0, partial(acc, nc - CODES_PER_WORD))
+                                                : make_ulonglong2(partial(acc, nc), ~0ull);
             ++chunk;
         }
         return chunk;
     }
 };
 
-// Hull record of one history (A1): what k_hull hands to k_mlp_walk.  K = number of MLP segments (R8); K = 0: rejected.
-struct alignas(16) HullRec {
-    double pin[3], pout[3];      // P_0, P_K (grid frame)
-    int32_t vin, vout;           // V_s, V_e (linear voxel index)
+// What k_hull (A1) hands to the walk kernels, per history: hull entry/exit, the MLP end states in the gantry frame (R5),
+// the number of MLP segments K (R8; K = 0: rejected) and everything of the MLP that depends on the history only.
+struct alignas(16) HistRec {
+    double pin[3], pout[3];           // P_0, P_K (grid frame, mm)
+    double cph, sph;                  // gantry angle
+    double u0, t0, v0, t2, v2, D;     // end states; D = u2 - u0
+    double du;                        // D / K
+    double dt_in, dv_in, nu_t, nu_v;  // entry slopes; exit minus entry slopes
+    double log_du;                    // ln(du / X0): ln(k du / X0) = ln k + log_du, ln k tabulated (one log per history)
+    double cq[3][6];                  // Sigma2 moments: J_q(d2) = int_0^d2 r^q f(D - r) dr = d2^(q+1) sum_j cq[q][j] d2^j
+    int32_t vin, vout;                // V_s, V_e (linear voxel index)
     uint32_t K, flags;
 };
 
 // Spatial sort key of a history inside its batch: 2 mm cell of the entry tracker hit, v-major.  Neighbouring threads
-// of k_hull then shoot neighbouring, near-parallel rays: the hull search and (through the stable K sort) the voxel walk
-// of a warp take nearly the same steps.  The key only orders the work; it has no influence on any result.
+// of k_hull then shoot neighbouring, near-parallel rays: the hull search of a warp takes nearly the same steps.  The key
+// only orders the work; it has no influence on any result.
 __global__ void __launch_bounds__(256)
 k_hull_keys(const ProtonPtrs pr, int64_t i_base, int count, double t_lo, double v_lo, double inv_cell, int nt, int nv,
             uint32_t* __restrict__ keys, uint32_t* __restrict__ vals) {
@@ -179,26 +187,24 @@ k_hull_keys(const ProtonPtrs pr, int64_t i_base, int count, double t_lo, double 
     vals[p] = (uint32_t)p;
 }
 
-// A1 / R3-R5: tracker record -> hull entry/exit.  Thread q takes history p = order[q] (spatial order, k_hull_keys).
-// Also emits, in that order, the sort key K: k_mlp_walk runs the batch in order of K so that the lanes of a warp have the
-// same trip count (the sample loop is the whole cost); the K sort is stable, so equal-K neighbours stay neighbours in space.
+// A1 / R3-R5: tracker record -> hull entry/exit and the per-history part of the MLP.  Thread q takes history
+// p = order[q] (spatial order, k_hull_keys).  Also emits, in that order, the sort key K: the walk kernels run the batch in
+// order of K (longest first), so that concurrently running warps have the same trip count.
 __global__ void __launch_bounds__(128)
 k_hull(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const uint8_t* __restrict__ hull, int64_t i_base, int count,
-       const uint32_t* __restrict__ order, HullRec* __restrict__ recs, uint32_t* __restrict__ keys, uint32_t* __restrict__ vals) {
+       const uint32_t* __restrict__ order, HistRec* __restrict__ recs, uint32_t* __restrict__ keys, uint32_t* __restrict__ vals) {
     const int q = blockIdx.x * blockDim.x + threadIdx.x;
     if (q >= count) return;
     const int p = (int)order[q];
     const int64_t i = i_base + p;
     const double phi = pr.phi[i], t_in = pr.t_in[i], v_in = pr.v_in[i], dt_in = pr.dt_in[i], dv_in = pr.dv_in[i];
     const double t_out = pr.t_out[i], v_out = pr.v_out[i], dt_out = pr.dt_out[i], dv_out = pr.dv_out[i];
-    HullRec r;
-    r.K = 0; r.flags = 0; r.vin = r.vout = -1;
-#pragma unroll
-    for (int a = 0; a < 3; ++a) { r.pin[a] = 0.0; r.pout[a] = 0.0; }
+    HistRec* r = recs + p;
+    uint32_t K = 0, flags = 0;
     do {
         if (!(isfinite(phi) && isfinite(t_in) && isfinite(v_in) && isfinite(dt_in) && isfinite(dv_in) &&
               isfinite(t_out) && isfinite(v_out) && isfinite(dt_out) && isfinite(dv_out))) {
-            r.flags = PCT_REJ_NONFINITE; break;
+            flags = PCT_REJ_NONFINITE; break;
         }
         double sph, cph;
         sincos(phi, &sph, &cph);
@@ -214,87 +220,127 @@ k_hull(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const uint8_t* __r
             const double d[3] = {-(cph - dt_out * sph), -(sph + dt_out * cph), -dv_out};
             find_hull(g, hull, T, d, h_out);
         }
-        if (!h_in.ok || !h_out.ok) { r.flags = PCT_REJ_MISS; break; }
-        if (h_in.tie || h_out.tie) r.flags |= PCT_TIE;
+        if (!h_in.ok || !h_out.ok) { flags = PCT_REJ_MISS; break; }
+        if (h_in.tie || h_out.tie) flags |= PCT_TIE;
+        // R5: MLP end states in the gantry frame
         const double u0 = h_in.P[0] * cph + h_in.P[1] * sph, u2 = h_out.P[0] * cph + h_out.P[1] * sph;
         const double D = u2 - u0;
-        if (!(D > 0.0)) { r.flags = PCT_REJ_ORDER; break; }
-        if (D > g.max_depth) { r.flags = PCT_REJ_DEPTH; break; }
-        r.K = (uint32_t)max(1, (int)ceil(D / (g.step_frac * g.h) - 1e-9));     // R8
+        if (!(D > 0.0)) { flags = PCT_REJ_ORDER; break; }
+        if (D > g.max_depth) { flags = PCT_REJ_DEPTH; break; }
+        K = (uint32_t)max(1, (int)ceil(D / (g.step_frac * g.h) - 1e-9));     // R8
+        const double du = D / (double)K;
 #pragma unroll
-        for (int a = 0; a < 3; ++a) { r.pin[a] = h_in.P[a]; r.pout[a] = h_out.P[a]; }
-        r.vin = h_in.c[0] + g.nx * (h_in.c[1] + g.ny * h_in.c[2]);
-        r.vout = h_out.c[0] + g.nx * (h_out.c[1] + g.ny * h_out.c[2]);
+        for (int a = 0; a < 3; ++a) { r->pin[a] = h_in.P[a]; r->pout[a] = h_out.P[a]; }
+        r->cph = cph; r->sph = sph;
+        r->u0 = u0; r->t0 = -h_in.P[0] * sph + h_in.P[1] * cph; r->v0 = h_in.P[2];
+        r->t2 = -h_out.P[0] * sph + h_out.P[1] * cph; r->v2 = h_out.P[2];
+        r->D = D; r->du = du;
+        r->dt_in = dt_in; r->dv_in = dv_in; r->nu_t = dt_out - dt_in; r->nu_v = dv_out - dv_in;
+        r->log_du = log(du / g.X0);
+        {   // f(D - r) = sum_j c_j r^j (Taylor shift of the polynomial about the exit depth D); cq[q][j] = c_j / (j + q + 1)
+            const double binom[6][6] = {{1, 0, 0, 0, 0, 0}, {1, 1, 0, 0, 0, 0}, {1, 2, 1, 0, 0, 0},
+                                        {1, 3, 3, 1, 0, 0}, {1, 4, 6, 4, 1, 0}, {1, 5, 10, 10, 5, 1}};
+            double Dp[6];
+            Dp[0] = 1.0;
+#pragma unroll
+            for (int e = 1; e < 6; ++e) Dp[e] = Dp[e - 1] * D;
+#pragma unroll
+            for (int j = 0; j < 6; ++j) {
+                double cj = 0.0;
+#pragma unroll
+                for (int ii = j; ii < 6; ++ii) cj += g.a[ii] * binom[ii][j] * Dp[ii - j];
+                if (j & 1) cj = -cj;
+#pragma unroll
+                for (int qq = 0; qq < 3; ++qq) r->cq[qq][j] = cj / (double)(j + qq + 1);
+            }
+        }
+        r->vin = h_in.c[0] + g.nx * (h_in.c[1] + g.ny * h_in.c[2]);
+        r->vout = h_out.c[0] + g.nx * (h_out.c[1] + g.ny * h_out.c[2]);
     } while (false);
-    recs[p] = r;
-    keys[q] = r.K;
+    r->K = K; r->flags = flags;
+    keys[q] = K;
     vals[q] = (uint32_t)p;
 }
 
-// A2 + A3.  Thread q of the batch takes history p = order[q] (the batch sorted by K, see k_hull).
+// The per-history constants of the MLP in registers (both walk kernels)
+struct MlpHist {
+    double u0, t0, v0, t2, v2, D, du, dt_in, dv_in, nu_t, nu_v, log_du;
+    double cq[3][6];
+    __device__ __forceinline__ void load(const HistRec* __restrict__ r) {
+        u0 = r->u0; t0 = r->t0; v0 = r->v0; t2 = r->t2; v2 = r->v2; D = r->D; du = r->du;
+        dt_in = r->dt_in; dv_in = r->dv_in; nu_t = r->nu_t; nu_v = r->nu_v; log_du = r->log_du;
+#pragma unroll
+        for (int q = 0; q < 3; ++q)
+#pragma unroll
+            for (int j = 0; j < 6; ++j) cq[q][j] = r->cq[q][j];
+    }
+};
+
+// A2 / R7: most likely lateral positions (t, v) at depth w1 = k du, 0 < k < K -- the Gaussian-conditioning form of the MLP
+// of ref [3] (positions only):  y = mu + Sigma1 R1^T (R1 Sigma1 R1^T + Sigma2)^-1 (y2 - R1 mu),  mu = R0 y0.
+// Sigma1 moments are Horner polynomials in w1 (DevCfg::s1c), Sigma2 moments in d2 = D - w1 (MlpHist::cq); the two log terms
+// are ln(w1 / X0) = ln k + ln(du / X0) and ln(d2 / X0) = ln(K - k) + ln(du / X0).
+__device__ __forceinline__ void mlp_sample(const DevCfg& g, const MlpHist& H, const double* __restrict__ logk, int k, int K,
+                                           double& w1, double& tk, double& vk) {
+    w1 = (double)k * H.du;
+    const double d2 = H.D - w1;
+    const double l1 = fma(g.log_coeff, __ldg(logk + k) + H.log_du, 1.0), l2 = fma(g.log_coeff, __ldg(logk + (K - k)) + H.log_du, 1.0);
+    const double g1 = l1 * l1, g2 = l2 * l2;
+    const double w1_2 = w1 * w1, d2_2 = d2 * d2;
+    const double C1 = g1 * w1 * horner6(g.s1c[0], w1);
+    const double B1 = g1 * w1_2 * horner6(g.s1c[1], w1);
+    const double A1 = g1 * w1_2 * w1 * horner6(g.s1c[2], w1);
+    const double C2 = g2 * d2 * horner6(H.cq[0], d2);
+    const double B2 = g2 * d2_2 * horner6(H.cq[1], d2);
+    const double A2 = g2 * d2_2 * d2 * horner6(H.cq[2], d2);
+    const double P0 = fma(d2, B1, A1), P1 = fma(d2, C1, B1);      // first row / col of Sigma1 R1^T
+    const double S00 = fma(d2, P1, P0) + A2, S01 = P1 + B2, S11 = C1 + C2;
+    const double inv_det = 1.0 / (S00 * S11 - S01 * S01);
+    const double G00 = (P0 * S11 - B1 * S01) * inv_det, G01 = (B1 * S00 - P0 * S01) * inv_det;
+    const double mu_t = fma(w1, H.dt_in, H.t0), mu_v = fma(w1, H.dv_in, H.v0);
+    tk = mu_t + G00 * (H.t2 - fma(d2, H.dt_in, mu_t)) + G01 * H.nu_t;
+    vk = mu_v + G00 * (H.v2 - fma(d2, H.dv_in, mu_v)) + G01 * H.nu_v;
+}
+
+// ---- A2 + A3, sequential form: one thread per history, rule R9 applied step by step --------------------------------------
+// The general routine: it handles every case (vertices that lie exactly on voxel faces, segments longer than a voxel,
+// paths that leave the grid or exceed the row capacity).  k_mlp_walk_warp does the bulk of the work and sends the histories
+// it cannot decide lane-locally here (list / list_count); with list == NULL it walks all `count` histories of the batch
+// (order[]), which is how PCT_K1_SEQUENTIAL=1 runs K1.  Codes go to a staging row per thread and are copied to the code
+// stream once the row's length is known (chunk_counter allocates its place).
 __global__ void __launch_bounds__(128, 4)
-k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const HullRec* __restrict__ recs, const uint32_t* __restrict__ order,
-           const double* __restrict__ logk, int64_t i_base,
-           int count, int stage_stride, ulonglong2* __restrict__ stage, uint32_t* __restrict__ nchunks, uint32_t* __restrict__ Nout,
-           int32_t* __restrict__ start_out, int32_t* __restrict__ end_out, float* __restrict__ ell_out,
-           uint8_t* __restrict__ flags_out, GenStats* __restrict__ stats) {
+k_mlp_walk(const __grid_constant__ DevCfg g, const HistRec* __restrict__ recs, const uint32_t* __restrict__ order,
+           const uint32_t* __restrict__ list, const unsigned* __restrict__ list_count, const double* __restrict__ logk, int64_t i_base,
+           int count, ulonglong2* __restrict__ stage, ulonglong2* __restrict__ codes, unsigned long long* __restrict__ chunk_counter,
+           uint64_t* __restrict__ code_off, uint32_t* __restrict__ Nout, int32_t* __restrict__ start_out, int32_t* __restrict__ end_out,
+           float* __restrict__ ell_out, uint8_t* __restrict__ flags_out, GenStats* __restrict__ stats) {
     const int q = blockIdx.x * blockDim.x + threadIdx.x;
-    const bool active = q < count;
+    const int total = list ? (int)min(*list_count, (unsigned)count) : count;
+    const bool active = q < total;
     unsigned flags = 0;
     unsigned N = 0, n_samples = 0;
-    int n_chunks = 0;
     if (active) {
-        const int p = (int)order[count - 1 - q];      // longest first: the CTAs launched last are the cheapest (short tail)
+        const int p = list ? (int)list[q] : (int)order[count - 1 - q];      // longest first: the CTAs launched last are the cheapest
         const int64_t i = i_base + p;
-        const HullRec rec = recs[p];
-        flags = rec.flags;
+        const HistRec* rec = recs + p;
+        flags = rec->flags;
         int32_t start_v = -1, end_v = -1;
         float ell = 0.f;
-        if (rec.K > 0) do {
-            const double phi = pr.phi[i], dt_in = pr.dt_in[i], dv_in = pr.dv_in[i], dt_out = pr.dt_out[i], dv_out = pr.dv_out[i];
-            double sph, cph;
-            sincos(phi, &sph, &cph);
-            struct { double P[3]; int c[3]; } h_in, h_out;
-#pragma unroll
-            for (int a = 0; a < 3; ++a) { h_in.P[a] = rec.pin[a]; h_out.P[a] = rec.pout[a]; }
-            h_in.c[0] = rec.vin % g.nx; h_in.c[1] = (rec.vin / g.nx) % g.ny; h_in.c[2] = rec.vin / (g.nx * g.ny);
-            h_out.c[0] = rec.vout % g.nx; h_out.c[1] = (rec.vout / g.nx) % g.ny; h_out.c[2] = rec.vout / (g.nx * g.ny);
-            // R5: MLP end states in the gantry frame
-            const double u0 = h_in.P[0] * cph + h_in.P[1] * sph, t0 = -h_in.P[0] * sph + h_in.P[1] * cph, v0 = h_in.P[2];
-            const double u2 = h_out.P[0] * cph + h_out.P[1] * sph, t2 = -h_out.P[0] * sph + h_out.P[1] * cph, v2 = h_out.P[2];
-            const double D = u2 - u0;
-            const int K = (int)rec.K;                                             // R8 (k_hull)
-
-            const double du = D / (double)K;
-            // Sigma2 moments: J_q(d2) = int_0^d2 r^q f(D-r) dr = d2^(q+1) sum_j cq[q][j] d2^j,
-            // f(D-r) = sum_j c_j r^j (Taylor shift of the polynomial about the exit depth D)
-            double cq[3][6];
-            {
-                const double binom[6][6] = {{1, 0, 0, 0, 0, 0}, {1, 1, 0, 0, 0, 0}, {1, 2, 1, 0, 0, 0},
-                                            {1, 3, 3, 1, 0, 0}, {1, 4, 6, 4, 1, 0}, {1, 5, 10, 10, 5, 1}};
-                double Dp[6];
-                Dp[0] = 1.0;
-#pragma unroll
-                for (int e = 1; e < 6; ++e) Dp[e] = Dp[e - 1] * D;
-#pragma unroll
-                for (int j = 0; j < 6; ++j) {
-                    double cj = 0.0;
-#pragma unroll
-                    for (int ii = j; ii < 6; ++ii) cj += g.a[ii] * binom[ii][j] * Dp[ii - j];
-                    if (j & 1) cj = -cj;
-#pragma unroll
-                    for (int q = 0; q < 3; ++q) cq[q][j] = cj / (double)(j + q + 1);
-                }
-            }
-            const double nu_t1 = dt_out - dt_in, nu_v1 = dv_out - dv_in;
-            // ln(w1 / X0) = ln k + ln(du / X0) and ln(d2 / X0) = ln(K - k) + ln(du / X0): one log per history, ln k tabulated
-            const double log_du = log(du / g.X0);
+        int n_chunks = 0;
+        ulonglong2* my_stage = stage + (size_t)q * (size_t)g.stage_chunks;
+        const int K = (int)rec->K;
+        if (K > 0) do {
+            MlpHist H;
+            H.load(rec);
+            const double cph = rec->cph, sph = rec->sph;
+            const double pout[3] = {rec->pout[0], rec->pout[1], rec->pout[2]};
+            const int vin = rec->vin, vout = rec->vout;
             // R9-R11 walk state
-            int c[3] = {h_in.c[0], h_in.c[1], h_in.c[2]};
-            start_v = c[0] + g.nx * (c[1] + g.ny * c[2]);
+            int c[3] = {vin % g.nx, (vin / g.nx) % g.ny, vin / (g.nx * g.ny)};
+            start_v = vin;
             CodeWriter cw;
-            cw.init(stage + p, (size_t)stage_stride);
-            double A[3] = {h_in.P[0], h_in.P[1], h_in.P[2]};
+            cw.init(my_stage);
+            double A[3] = {rec->pin[0], rec->pin[1], rec->pin[2]};
             double f_lo[3], f_hi[3];
 #pragma unroll
             for (int a = 0; a < 3; ++a) { f_lo[a] = face_coord(g, a, c[a]); f_hi[a] = face_coord(g, a, c[a] + 1); }
@@ -304,29 +350,12 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const HullRec*
             for (int k = 1; k <= K && !bad; ++k) {
                 double B[3];
                 if (k < K) {
-                    // A2 / R7: Gaussian-conditioning form of the MLP of ref [3] (positions only):
-                    // y = mu + Sigma1 R1^T (R1 Sigma1 R1^T + Sigma2)^-1 (y2 - R1 mu), mu = R0 y0
-                    const double w1 = (double)k * du, d2 = D - w1;
-                    const double l1 = fma(g.log_coeff, __ldg(logk + k) + log_du, 1.0), l2 = fma(g.log_coeff, __ldg(logk + (K - k)) + log_du, 1.0);
-                    const double g1 = l1 * l1, g2 = l2 * l2;
-                    const double w1_2 = w1 * w1, d2_2 = d2 * d2;
-                    const double C1 = g1 * w1 * horner6(g.s1c[0], w1);
-                    const double B1 = g1 * w1_2 * horner6(g.s1c[1], w1);
-                    const double A1 = g1 * w1_2 * w1 * horner6(g.s1c[2], w1);
-                    const double C2 = g2 * d2 * horner6(cq[0], d2);
-                    const double B2 = g2 * d2_2 * horner6(cq[1], d2);
-                    const double A2 = g2 * d2_2 * d2 * horner6(cq[2], d2);
-                    const double P0 = fma(d2, B1, A1), P1 = fma(d2, C1, B1);      // first row / col of Sigma1 R1^T
-                    const double S00 = fma(d2, P1, P0) + A2, S01 = P1 + B2, S11 = C1 + C2;
-                    const double inv_det = 1.0 / (S00 * S11 - S01 * S01);
-                    const double G00 = (P0 * S11 - B1 * S01) * inv_det, G01 = (B1 * S00 - P0 * S01) * inv_det;
-                    const double mu_t = fma(w1, dt_in, t0), mu_v = fma(w1, dv_in, v0);
-                    const double tk = mu_t + G00 * (t2 - fma(d2, dt_in, mu_t)) + G01 * nu_t1;
-                    const double vk = mu_v + G00 * (v2 - fma(d2, dv_in, mu_v)) + G01 * nu_v1;
-                    const double uk = u0 + w1;
+                    double w1, tk, vk;
+                    mlp_sample(g, H, logk, k, K, w1, tk, vk);
+                    const double uk = H.u0 + w1;
                     B[0] = uk * cph - tk * sph; B[1] = uk * sph + tk * cph; B[2] = vk;
                 } else {
-                    B[0] = h_out.P[0]; B[1] = h_out.P[1]; B[2] = h_out.P[2];
+                    B[0] = pout[0]; B[1] = pout[1]; B[2] = pout[2];
                 }
                 const double dx = B[0] - A[0], dy = B[1] - A[1], dz = B[2] - A[2];
                 const double seg_len = sqrt(dx * dx + dy * dy + dz * dz);
@@ -343,14 +372,7 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const HullRec*
                 while ((d0 | d1 | d2) != 0) {
                     // lowest candidate axis with the smallest s (strict comparison: x before y before z on equality)
                     int best = d0 != 0 ? 0 : (d1 != 0 ? 1 : 2);
-                    if (d0 != 0 && d1 != 0 && d2 == 0) {
-                        // the common two-candidate case of an oblique path: x and y faces in one segment
-                        const double nx_ = fabs((d0 > 0 ? f_hi[0] : f_lo[0]) - A[0]), dx_ = fabs(B[0] - A[0]);
-                        const double ny_ = fabs((d1 > 0 ? f_hi[1] : f_lo[1]) - A[1]), dy_ = fabs(B[1] - A[1]);
-                        const double lx = nx_ * dy_, ly = ny_ * dx_;           // s_x < s_y <=> lx < ly
-                        best = ly < lx ? 1 : 0;
-                        if (fabs(lx - ly) * seg_len < g.tie_eps * (dx_ * dy_)) tie = true;
-                    } else if ((d0 != 0) + (d1 != 0) + (d2 != 0) > 1) {
+                    if ((d0 != 0) + (d1 != 0) + (d2 != 0) > 1) {
                         const int dir[3] = {d0, d1, d2};
                         double num[3], den[3];
 #pragma unroll
@@ -365,8 +387,6 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const HullRec*
                         for (int a = 0; a < 3; ++a)
                             if (a != best && dir[a] != 0 && (num[a] * db_ - nb * den[a]) * seg_len < g.tie_eps * (den[a] * db_)) tie = true;
                     }
-                    // move across the face of axis `best`; neighbouring lanes follow neighbouring paths and mostly take the
-                    // same branch
                     int code;
                     bool inside;
 #define PCT_MOVE_AXIS(a, d, n_a)                                                                            \
@@ -393,13 +413,18 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const HullRec*
             N = n_vis;
             n_samples = (unsigned)K;
             if (tie) flags |= PCT_TIE;
-            if (c[0] != h_out.c[0] || c[1] != h_out.c[1] || c[2] != h_out.c[2]) flags |= PCT_END_MISMATCH;   // R10
-            ell = (float)(L / (double)N);                                                                    // R11
             end_v = c[0] + g.nx * (c[1] + g.ny * c[2]);
+            if (end_v != vout) flags |= PCT_END_MISMATCH;                                                    // R10
+            ell = (float)(L / (double)N);                                                                    // R11
         } while (false);
         if (N == 0) { n_chunks = 0; start_v = -1; end_v = -1; ell = 0.f; }
         flags &= 0xffu;
-        nchunks[p] = (uint32_t)n_chunks;
+        unsigned long long off = 0ull;
+        if (n_chunks > 0) {
+            off = atomicAdd(chunk_counter, (unsigned long long)n_chunks);
+            for (int k = 0; k < n_chunks; ++k) codes[off + k] = my_stage[k];
+        }
+        code_off[i] = off;
         Nout[i] = N;
         start_out[i] = start_v;
         end_out[i] = end_v;
@@ -419,11 +444,192 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const HullRec*
     }
 }
 
-int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, int64_t i_base, int count, int stage_stride,
-                     ulonglong2* stage, uint32_t* nchunks, pct_paths* P, cudaStream_t st) {
+// ---- A2 + A3, warp-cooperative form: one warp per history, lane = MLP sample -----------------------------------------------
+// PAPER.md:26 maps "each proton [to] an individual thread"; on a 32-wide machine the voxel stepping between the samples
+// then diverges (0-3 steps per sample and lane) and half of the lanes idle.  Here the 32 lanes of a warp take 32
+// CONSECUTIVE SAMPLES of one history:
+//   * lane l evaluates the MLP at depth k = k0 + l (all lanes converged, FP64) and maps the vertex straight to voxel index
+//     coordinates X = (P - lo) / h (one FMA pair per axis from (u, t, v));
+//   * the voxel of an interior vertex is round(X - 1/2).  A vertex is handled here only if it lies at least 1e-9 voxel
+//     widths away from every face: then that voxel is the only closed voxel containing it, so it IS the state the
+//     sequential rule R9 reaches there, whatever happened before.  The segment's steps follow from the voxels of its two
+//     ends (shuffle from lane l-1): at most one per axis; two or three are ordered by their crossing parameters with the
+//     same cross-multiplied comparison and tie rule as the sequential form;
+//   * the last segment ends in P_K, which lies exactly on a face of V_e by construction: its steps are decided as R9 states
+//     it, by comparing P_K (mm) with the faces of the voxel the segment starts in;
+//   * a warp scan of the step counts gives every code its place in the row, the codes are collected in shared memory,
+//     packed 21 per word and written to the code stream at a place taken from chunk_counter.
+// Anything else -- a vertex within 1e-9 of a face, a segment that spans more than one voxel, a voxel outside the grid, a
+// row beyond the capacity -- sends the whole history to the sequential kernel (fb_list), which decides it exactly as
+// before.  On the synthetic workloads that is ~1e-6 of the histories.
+constexpr int WK_WARPS = 4;
+constexpr double ROUND_MAGIC = 6755399441055744.0;      // 2^52 + 2^51: (x + M) - M = x rounded to the nearest integer
+constexpr double FACE_GUARD = 1e-9;                     // in voxel widths
+
+__global__ void __launch_bounds__(WK_WARPS * 32, 4)
+k_mlp_walk_warp(const __grid_constant__ DevCfg g, const HistRec* __restrict__ recs, const uint32_t* __restrict__ order,
+                const double* __restrict__ logk, int64_t i_base, int count, int row_cap, ulonglong2* __restrict__ codes,
+                unsigned long long* __restrict__ chunk_counter, uint64_t* __restrict__ code_off, uint32_t* __restrict__ Nout,
+                int32_t* __restrict__ start_out, int32_t* __restrict__ end_out, float* __restrict__ ell_out,
+                uint8_t* __restrict__ flags_out, uint32_t* __restrict__ fb_list, unsigned* __restrict__ fb_count,
+                GenStats* __restrict__ stats) {
+    extern __shared__ unsigned char row_codes[];            // WK_WARPS rows of row_cap bytes: one step code per byte
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    unsigned char* my_row = row_codes + (size_t)w * row_cap;
+    unsigned long long st_vis = 0, st_smp = 0;
+    unsigned st_rej = 0, st_tie = 0;
+    const double o0 = -g.lo[0] * g.inv_h - 0.5, o1 = -g.lo[1] * g.inv_h - 0.5, o2 = -g.lo[2] * g.inv_h - 0.5;
+    for (int q = blockIdx.x * WK_WARPS + w; q < count; q += gridDim.x * WK_WARPS) {
+        const int p = (int)order[count - 1 - q];          // longest first
+        const int64_t i = i_base + p;
+        const HistRec* rec = recs + p;
+        const int K = (int)rec->K;
+        unsigned flags = rec->flags;
+        if (K == 0) {
+            if (lane == 0) {
+                code_off[i] = 0ull; Nout[i] = 0u; start_out[i] = -1; end_out[i] = -1; ell_out[i] = 0.f; flags_out[i] = (uint8_t)flags;
+                ++st_rej;
+            }
+            continue;
+        }
+        MlpHist H;
+        H.load(rec);
+        const double cxh = rec->cph * g.inv_h, sxh = rec->sph * g.inv_h;
+        const int vin = rec->vin, vout = rec->vout;
+        // carried from round to round: voxel and index coordinates of the vertex before lane 0's
+        int cP0 = vin % g.nx, cP1 = (vin / g.nx) % g.ny, cP2 = vin / (g.nx * g.ny);
+        double XP0 = fma(rec->pin[0], g.inv_h, o0), XP1 = fma(rec->pin[1], g.inv_h, o1), XP2 = fma(rec->pin[2], g.inv_h, o2);
+        double Lsum = 0.0;
+        int steps = 0;                                      // codes written so far
+        bool tie = false, give_up = false;
+        int cE0 = cP0, cE1 = cP1, cE2 = cP2;                // voxel the walk ends in
+        for (int k0 = 1; k0 <= K; k0 += 32) {
+            const int k = k0 + lane;
+            const bool valid = k <= K, last = k == K;
+            double X0, X1, X2;
+            int cB0 = 0, cB1 = 0, cB2 = 0;
+            bool odd = false;                               // this lane cannot decide its segment locally
+            if (k < K) {
+                double w1, tk, vk;
+                mlp_sample(g, H, logk, k, K, w1, tk, vk);
+                const double uk = H.u0 + w1;
+                X0 = fma(uk, cxh, fma(tk, -sxh, o0)); X1 = fma(uk, sxh, fma(tk, cxh, o1)); X2 = fma(vk, g.inv_h, o2);
+                const double s0 = X0 + ROUND_MAGIC, s1 = X1 + ROUND_MAGIC, s2 = X2 + ROUND_MAGIC;
+                cB0 = __double2loint(s0); cB1 = __double2loint(s1); cB2 = __double2loint(s2);
+                odd = fabs(X0 - (s0 - ROUND_MAGIC)) > 0.5 - FACE_GUARD || fabs(X1 - (s1 - ROUND_MAGIC)) > 0.5 - FACE_GUARD ||
+                      fabs(X2 - (s2 - ROUND_MAGIC)) > 0.5 - FACE_GUARD;
+            } else {
+                X0 = fma(rec->pout[0], g.inv_h, o0); X1 = fma(rec->pout[1], g.inv_h, o1); X2 = fma(rec->pout[2], g.inv_h, o2);
+            }
+            int cA0 = __shfl_up_sync(0xffffffffu, cB0, 1), cA1 = __shfl_up_sync(0xffffffffu, cB1, 1), cA2 = __shfl_up_sync(0xffffffffu, cB2, 1);
+            double XA0 = __shfl_up_sync(0xffffffffu, X0, 1), XA1 = __shfl_up_sync(0xffffffffu, X1, 1), XA2 = __shfl_up_sync(0xffffffffu, X2, 1);
+            if (lane == 0) { cA0 = cP0; cA1 = cP1; cA2 = cP2; XA0 = XP0; XA1 = XP1; XA2 = XP2; }
+            if (last) {
+                // R9 on the segment into P_K: step across the axes on which P_K lies strictly outside the closed start voxel
+                const double b0 = rec->pout[0], b1 = rec->pout[1], b2 = rec->pout[2];
+                cB0 = cA0 + (b0 > face_coord(g, 0, cA0 + 1) ? 1 : (b0 < face_coord(g, 0, cA0) ? -1 : 0));
+                cB1 = cA1 + (b1 > face_coord(g, 1, cA1 + 1) ? 1 : (b1 < face_coord(g, 1, cA1) ? -1 : 0));
+                cB2 = cA2 + (b2 > face_coord(g, 2, cA2 + 1) ? 1 : (b2 < face_coord(g, 2, cA2) ? -1 : 0));
+                odd = b0 > face_coord(g, 0, cB0 + 1) || b0 < face_coord(g, 0, cB0) || b1 > face_coord(g, 1, cB1 + 1) || b1 < face_coord(g, 1, cB1) ||
+                      b2 > face_coord(g, 2, cB2 + 1) || b2 < face_coord(g, 2, cB2);              // more than one voxel away
+            }
+            const int d0 = valid ? cB0 - cA0 : 0, d1 = valid ? cB1 - cA1 : 0, d2 = valid ? cB2 - cA2 : 0;
+            if (valid) odd = odd || (unsigned)(d0 + 1) > 2u || (unsigned)(d1 + 1) > 2u || (unsigned)(d2 + 1) > 2u ||
+                             (unsigned)cB0 >= (unsigned)g.nx || (unsigned)cB1 >= (unsigned)g.ny || (unsigned)cB2 >= (unsigned)g.nz;
+            else odd = false;
+            if (__any_sync(0xffffffffu, odd)) { give_up = true; break; }
+            const int n = (d0 != 0) + (d1 != 0) + (d2 != 0);
+            // segment length: h |X_B - X_A| (the index map is a rotation scaled by 1/h)
+            const double e0 = X0 - XA0, e1 = X1 - XA1, e2 = X2 - XA2;
+            const double seg_len = valid ? g.h * sqrt(fma(e0, e0, fma(e1, e1, e2 * e2))) : 0.0;
+            Lsum += seg_len;
+            int r0 = 0, r1 = 0, r2 = 0;                     // place of each axis' step among this segment's steps
+            if (n >= 2) {
+                // crossing parameter of axis a: s_a = num_a / den_a, num_a = distance of A from the face, den_a = |B_a - A_a|
+                const double n0 = fabs((double)(cA0 + (d0 > 0 ? 1 : 0)) - 0.5 - XA0), n1 = fabs((double)(cA1 + (d1 > 0 ? 1 : 0)) - 0.5 - XA1),
+                             n2 = fabs((double)(cA2 + (d2 > 0 ? 1 : 0)) - 0.5 - XA2);
+                const double a0 = fabs(e0), a1 = fabs(e1), a2 = fabs(e2);
+                const double l01 = n0 * a1, l10 = n1 * a0, l02 = n0 * a2, l20 = n2 * a0, l12 = n1 * a2, l21 = n2 * a1;
+                const bool p01 = d0 != 0 && d1 != 0, p02 = d0 != 0 && d2 != 0, p12 = d1 != 0 && d2 != 0;
+                // s_a < s_b <=> l_ab < l_ba; on equality the lower axis goes first
+                r0 = (p01 && l10 < l01) + (p02 && l20 < l02);
+                r1 = (p01 && !(l10 < l01)) + (p12 && l21 < l12);
+                r2 = (p02 && !(l20 < l02)) + (p12 && !(l21 < l12));
+                const double te = g.tie_eps;
+                if ((p01 && fabs(l01 - l10) * seg_len < te * (a0 * a1)) || (p02 && fabs(l02 - l20) * seg_len < te * (a0 * a2)) ||
+                    (p12 && fabs(l12 - l21) * seg_len < te * (a1 * a2))) tie = true;
+            }
+            int incl = n;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += y; }
+            const int total = __shfl_sync(0xffffffffu, incl, 31);
+            if (steps + total + 1 > g.max_visits) { give_up = true; break; }      // the sequential kernel flags the capacity
+            const int at = steps + incl - n;
+            if (d0 != 0) my_row[at + r0] = (unsigned char)(d0 < 0 ? 1 : 0);
+            if (d1 != 0) my_row[at + r1] = (unsigned char)(d1 < 0 ? 3 : 2);
+            if (d2 != 0) my_row[at + r2] = (unsigned char)(d2 < 0 ? 5 : 4);
+            steps += total;
+            const int src = min(31, K - k0);                // lane of the last valid vertex of this round
+            cP0 = __shfl_sync(0xffffffffu, cB0, 31); cP1 = __shfl_sync(0xffffffffu, cB1, 31); cP2 = __shfl_sync(0xffffffffu, cB2, 31);
+            XP0 = __shfl_sync(0xffffffffu, X0, 31); XP1 = __shfl_sync(0xffffffffu, X1, 31); XP2 = __shfl_sync(0xffffffffu, X2, 31);
+            cE0 = __shfl_sync(0xffffffffu, cB0, src); cE1 = __shfl_sync(0xffffffffu, cB1, src); cE2 = __shfl_sync(0xffffffffu, cB2, src);
+        }
+        if (give_up) {
+            if (lane == 0) fb_list[atomicAdd(fb_count, 1u)] = (uint32_t)p;
+            continue;
+        }
+        if (__any_sync(0xffffffffu, tie)) flags |= PCT_TIE;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) Lsum += __shfl_xor_sync(0xffffffffu, Lsum, o);
+        const int N = steps + 1;
+        const int end_v = cE0 + g.nx * (cE1 + g.ny * cE2);
+        if (end_v != vout) flags |= PCT_END_MISMATCH;                                                        // R10
+        const int n_chunks = (steps + CODES_PER_CHUNK - 1) / CODES_PER_CHUNK;
+        unsigned long long off = 0ull;
+        if (lane == 0 && n_chunks > 0) off = atomicAdd(chunk_counter, (unsigned long long)n_chunks);
+        off = __shfl_sync(0xffffffffu, off, 0);
+        __syncwarp();
+        unsigned long long* out = reinterpret_cast<unsigned long long*>(codes + off);
+        for (int wd = lane; wd < 2 * n_chunks; wd += 32) {
+            unsigned long long word = 0ull;
+            const int base = wd * CODES_PER_WORD;
+#pragma unroll
+            for (int j = 0; j < CODES_PER_WORD; ++j) {
+                const unsigned long long c = base + j < steps ? (unsigned long long)my_row[base + j] : 7ull;
+                word |= c << (3 * j);
+            }
+            if (base + CODES_PER_WORD > steps) word |= 1ull << 63;     // bit 63 is no code field; set in partial words like the sequential writer's
+            out[wd] = word;
+        }
+        __syncwarp();
+        if (lane == 0) {
+            code_off[i] = off; Nout[i] = (uint32_t)N; start_out[i] = vin; end_out[i] = end_v;
+            ell_out[i] = (float)(Lsum / (double)N);                                                          // R11
+            flags_out[i] = (uint8_t)(flags & 0xffu);
+            st_vis += (unsigned long long)N; st_smp += (unsigned long long)K; st_tie += (flags & PCT_TIE) ? 1u : 0u;
+        }
+    }
+    if (lane == 0) {
+        if (st_smp) atomicAdd(&stats->total_samples, st_smp);
+        if (st_vis) atomicAdd(&stats->total_visits, st_vis);
+        if (st_rej) atomicAdd(&stats->n_rejected, (unsigned long long)st_rej);
+        if (st_tie) atomicAdd(&stats->n_ties, (unsigned long long)st_tie);
+    }
+}
+
+static bool k1_sequential() {
+    static const bool v = [] { const char* e = getenv("PCT_K1_SEQUENTIAL"); return e && e[0] == '1'; }();
+    return v;
+}
+
+// One batch of K1: spatial sort -> k_hull -> sort by K -> k_mlp_walk_warp -> k_mlp_walk on the histories it handed over.
+// `stage` holds count rows of stage_chunks chunks (used by the sequential kernel only); the code stream must have room for
+// count * stage_chunks more chunks behind *chunk_counter.
+int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, int64_t i_base, int count, ulonglong2* stage,
+                     unsigned long long* chunk_counter, pct_paths* P, cudaStream_t st) {
     const int threads = 128;
     const int blocks = (count + threads - 1) / threads;
-    // scratch: hull records, sort keys/values (double buffered), cub temporary storage
+    // scratch: history records, sort keys/values (double buffered), fallback list + counter, cub temporary storage
     size_t sort_tmp = 0;
     {
         cub::DoubleBuffer<uint32_t> dk(nullptr, nullptr), dv(nullptr, nullptr);
@@ -431,8 +637,9 @@ int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, in
     }
     auto up = [](size_t v) { return (v + 255) & ~(size_t)255; };
     const size_t arr = up(4 * (size_t)count);
-    const size_t o_rec = 0, o_k0 = up(sizeof(HullRec) * (size_t)count), o_k1 = o_k0 + arr, o_v0 = o_k1 + arr, o_v1 = o_v0 + arr,
-                 o_k2 = o_v1 + arr, o_k3 = o_k2 + arr, o_v2 = o_k3 + arr, o_v3 = o_v2 + arr, o_tmp = o_v3 + arr, total = o_tmp + up(sort_tmp);
+    const size_t o_rec = 0, o_k0 = up(sizeof(HistRec) * (size_t)count), o_k1 = o_k0 + arr, o_v0 = o_k1 + arr, o_v1 = o_v0 + arr,
+                 o_k2 = o_v1 + arr, o_k3 = o_k2 + arr, o_v2 = o_k3 + arr, o_v3 = o_v2 + arr, o_fb = o_v3 + arr, o_fbc = o_fb + arr,
+                 o_tmp = o_fbc + 256, total = o_tmp + up(sort_tmp);
     if (total > ctx->gen_scratch_bytes) {
         if (ctx->gen_scratch) PCT_CUDA(ctx, cudaFree(ctx->gen_scratch));
         ctx->gen_scratch = nullptr; ctx->gen_scratch_bytes = 0;
@@ -440,10 +647,13 @@ int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, in
         ctx->gen_scratch_bytes = total;
     }
     char* base = (char*)ctx->gen_scratch;
-    HullRec* recs = (HullRec*)(base + o_rec);
+    HistRec* recs = (HistRec*)(base + o_rec);
+    uint32_t* fb_list = (uint32_t*)(base + o_fb);
+    unsigned* fb_count = (unsigned*)(base + o_fbc);
     cub::DoubleBuffer<uint32_t> dk((uint32_t*)(base + o_k0), (uint32_t*)(base + o_k1)), dv((uint32_t*)(base + o_v0), (uint32_t*)(base + o_v1));
     cub::DoubleBuffer<uint32_t> sk((uint32_t*)(base + o_k2), (uint32_t*)(base + o_k3)), sv((uint32_t*)(base + o_v2), (uint32_t*)(base + o_v3));
     ProfScope prof(ctx, 0, st);
+    PCT_CUDA(ctx, cudaMemsetAsync(fb_count, 0, sizeof(unsigned), st));
     {   // spatial order of the batch: 2 mm cells of the entry tracker plane
         const DevCfg& c = ctx->cfg;
         const double ex = fmax(fabs(c.lo[0]), fabs(c.hi[0])), ey = fmax(fabs(c.lo[1]), fabs(c.hi[1]));
@@ -459,9 +669,23 @@ int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, in
     while ((1 << key_bits) < ctx->logk_n) ++key_bits;                  // K < logk_n
     PCT_CUDA(ctx, cub::DeviceRadixSort::SortPairs(base + o_tmp, sort_tmp, dk, dv, count, 0, key_bits, st));
     ctx->launches += 4;
-    k_mlp_walk<<<blocks, threads, 0, st>>>(ctx->cfg, pr, recs, dv.Current(), ctx->logk, i_base, count, stage_stride, stage, nchunks, P->N, P->start, P->end,
-                                           P->ell, P->flags, ctx->d_stats);
-    ++ctx->launches;
+    const uint32_t* order = dv.Current();
+    if (!k1_sequential()) {
+        const int row_cap = (ctx->cfg.max_visits + 15) & ~15;
+        const size_t smem = (size_t)WK_WARPS * (size_t)row_cap;
+        const int want = (count + WK_WARPS - 1) / WK_WARPS, cap = ctx->num_sms * 16;
+        k_mlp_walk_warp<<<want < cap ? want : cap, WK_WARPS * 32, smem, st>>>(ctx->cfg, recs, order, ctx->logk, i_base, count, row_cap, P->codes,
+                                                                             chunk_counter, P->code_off, P->N, P->start, P->end, P->ell, P->flags,
+                                                                             fb_list, fb_count, ctx->d_stats);
+        // the histories the warp kernel handed over (normally a handful; the grid covers the worst case and exits at once)
+        k_mlp_walk<<<blocks, threads, 0, st>>>(ctx->cfg, recs, order, fb_list, fb_count, ctx->logk, i_base, count, stage, P->codes, chunk_counter,
+                                               P->code_off, P->N, P->start, P->end, P->ell, P->flags, ctx->d_stats);
+        ctx->launches += 2;
+    } else {
+        k_mlp_walk<<<blocks, threads, 0, st>>>(ctx->cfg, recs, order, nullptr, nullptr, ctx->logk, i_base, count, stage, P->codes, chunk_counter,
+                                               P->code_off, P->N, P->start, P->end, P->ell, P->flags, ctx->d_stats);
+        ++ctx->launches;
+    }
     PCT_CUDA(ctx, cudaGetLastError());
     return PCT_OK;
 }
@@ -587,26 +811,6 @@ int launch_scan_u32(pct_ctx* ctx, const uint32_t* in, uint64_t* out, int64_t n, 
     k_scan_sums<<<1, SCAN_THREADS, 0, st>>>(sums, nb, base, d_total);
     k_scan_finish<<<(unsigned)nb, SCAN_THREADS, 0, st>>>(in, n, sums, out);
     ctx->launches += 3;
-    PCT_CUDA(ctx, cudaGetLastError());
-    return PCT_OK;
-}
-
-// ---- compaction: staging [chunk][history] -> final stream at 16-byte granularity ---------------------------------
-__global__ void __launch_bounds__(256) k_compact(const ulonglong2* __restrict__ stage, const uint32_t* __restrict__ nchunks,
-                                                 const uint64_t* __restrict__ off, int count, int stage_stride,
-                                                 ulonglong2* __restrict__ codes) {
-    const int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= count) return;
-    const uint32_t nc = nchunks[p];
-    const uint64_t o = off[p];
-    for (uint32_t k = 0; k < nc; ++k) codes[o + k] = stage[(size_t)k * stage_stride + p];
-}
-
-int launch_compact(pct_ctx* ctx, const ulonglong2* stage, const uint32_t* nchunks, const uint64_t* off, int count,
-                   int stage_stride, ulonglong2* codes, cudaStream_t st) {
-    if (count <= 0) return PCT_OK;
-    k_compact<<<(count + 255) / 256, 256, 0, st>>>(stage, nchunks, off, count, stage_stride, codes);
-    ++ctx->launches;
     PCT_CUDA(ctx, cudaGetLastError());
     return PCT_OK;
 }

@@ -319,10 +319,9 @@ int pct_generate_mlp(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hull, v
     const int64_t m = pr->m;
     const size_t mm = (size_t)(m > 0 ? m : 1);
     ulonglong2* stage = nullptr;
-    uint32_t* nchunks = nullptr;
     int rc = PCT_OK;
     // kernels of this call may still be running on `st`: drain it before any block goes back to the (process-wide) cache
-    auto fail = [&](int code) { cudaStreamSynchronize(st); cudaGetLastError(); cache_free(stage); cache_free(nchunks); free_paths_arrays(P); delete P; return code; };
+    auto fail = [&](int code) { cudaStreamSynchronize(st); cudaGetLastError(); cache_free(stage); free_paths_arrays(P); delete P; return code; };
 #define GEN_CUDA(call)                                                                                          \
     do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { cudaGetLastError();                               \
         return fail(set_error(ctx, e__ == cudaErrorMemoryAllocation ? PCT_E_OOM : PCT_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e__))); } } while (0)
@@ -333,35 +332,35 @@ int pct_generate_mlp(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hull, v
     GEN_CUDA(cache_alloc((void**)&P->flags, sizeof(uint8_t) * mm));
     GEN_CUDA(cache_alloc((void**)&P->code_off, sizeof(uint64_t) * mm));
     const int batch_max = (int)(m < GEN_BATCH ? (m > 0 ? m : 1) : GEN_BATCH);
+    // rows of the sequential walk kernel (the histories the warp kernel hands over; all of them with PCT_K1_SEQUENTIAL=1)
     GEN_CUDA(cache_alloc((void**)&stage, sizeof(ulonglong2) * (size_t)batch_max * (size_t)ctx->cfg.stage_chunks));
-    GEN_CUDA(cache_alloc((void**)&nchunks, sizeof(uint32_t) * (size_t)batch_max));
     GEN_CUDA(cudaMemsetAsync(ctx->d_stats, 0, sizeof(GenStats), st));
+    // rows are appended to the code stream at places handed out by a device counter (chunks), read back after every batch
+    GEN_CUDA(cudaMemsetAsync(ctx->d_total, 0, sizeof(unsigned long long), st));
     const ProtonPtrs pp = {pr->phi, pr->t_in, pr->v_in, pr->dt_in, pr->dv_in, pr->t_out, pr->v_out, pr->dt_out, pr->dv_out};
     for (int64_t i0 = 0; i0 < m; i0 += GEN_BATCH) {
         const int count = (int)((m - i0) < GEN_BATCH ? (m - i0) : GEN_BATCH);
-        if (ctx->batch_ready && i0 / GEN_BATCH < ctx->n_batch_ready) GEN_CUDA(cudaStreamWaitEvent(st, ctx->batch_ready[i0 / GEN_BATCH], 0));
-        if ((rc = launch_mlp_batch(ctx, pp, hull, i0, count, batch_max, stage, nchunks, P, st)) != PCT_OK) return fail(rc);
-        if ((rc = launch_scan_u32(ctx, nchunks, P->code_off + i0, count, (uint64_t)P->chunks_used, ctx->d_total, st)) != PCT_OK) return fail(rc);
-        unsigned long long batch_chunks = 0;
-        GEN_CUDA(cudaMemcpyAsync(&batch_chunks, ctx->d_total, sizeof(batch_chunks), cudaMemcpyDeviceToHost, st));
-        GEN_CUDA(cudaStreamSynchronize(st));
-        int64_t need = P->chunks_used + (int64_t)batch_chunks;
-        if (need > P->chunks_cap) {
-            // first batch: extrapolate to all histories (+60 %: oblique paths take up to sqrt(2) more steps); later: ensure_codes grows by 1.5x
-            int64_t guess = need;
-            if (i0 == 0 && m > count) guess = (int64_t)((double)batch_chunks * ((double)m / (double)count) * 1.6) + 1024;   // the first batch may be the axis-aligned (shortest-code) one
-            if ((rc = ensure_codes(ctx, P, guess > need ? guess : need, st)) != PCT_OK) {
-                if (guess > need && (rc = ensure_codes(ctx, P, need, st)) != PCT_OK) return fail(rc);
+        // room for the worst case of this batch; the first growth extrapolates what the batches so far needed to all histories
+        const int64_t reserve = P->chunks_used + (int64_t)count * ctx->cfg.stage_chunks;
+        if (reserve > P->chunks_cap) {
+            int64_t guess = reserve;
+            if (i0 > 0) guess = (int64_t)((double)P->chunks_used * ((double)m / (double)i0) * 1.45) + (int64_t)GEN_BATCH * ctx->cfg.stage_chunks;
+            if ((rc = ensure_codes(ctx, P, guess > reserve ? guess : reserve, st)) != PCT_OK) {
+                if (!(guess > reserve) || (rc = ensure_codes(ctx, P, reserve, st)) != PCT_OK) return fail(rc);
             }
         }
-        if ((rc = launch_compact(ctx, stage, nchunks, P->code_off + i0, count, batch_max, P->codes, st)) != PCT_OK) return fail(rc);
-        P->chunks_used = need;
+        if (ctx->batch_ready && i0 / GEN_BATCH < ctx->n_batch_ready) GEN_CUDA(cudaStreamWaitEvent(st, ctx->batch_ready[i0 / GEN_BATCH], 0));
+        if ((rc = launch_mlp_batch(ctx, pp, hull, i0, count, stage, ctx->d_total, P, st)) != PCT_OK) return fail(rc);
+        unsigned long long used = 0;
+        GEN_CUDA(cudaMemcpyAsync(&used, ctx->d_total, sizeof(used), cudaMemcpyDeviceToHost, st));
+        GEN_CUDA(cudaStreamSynchronize(st));
+        P->chunks_used = (int64_t)used;
     }
     GenStats hs;
     GEN_CUDA(cudaMemcpyAsync(&hs, ctx->d_stats, sizeof(hs), cudaMemcpyDeviceToHost, st));
     GEN_CUDA(cudaStreamSynchronize(st));
 #undef GEN_CUDA
-    cache_free(stage); cache_free(nchunks);
+    cache_free(stage);
     P->total_visits = (int64_t)hs.total_visits; P->n_rejected = (int64_t)hs.n_rejected; P->total_samples = (int64_t)hs.total_samples; P->n_ties = (int64_t)hs.n_ties;
     *out = P;
     return PCT_OK;
@@ -381,7 +380,11 @@ int pct_plan_info(const pct_paths* P, pct_plan_stats* out) {
     const SolvePlan* pl = P->plan;
     if (!pl) return PCT_OK;
     out->block_size = pl->block_size; out->n_blocks = pl->n_blocks; out->n_groups = pl->n_groups; out->n_direct = pl->n_direct;
-    out->plan_bytes = pl->cnt_bytes + 8 * pl->stream_words + P->m * 13 + (pl->n_groups + 1) * (int64_t)sizeof(PlanGroup) + pl->n_blocks * 4;
+    // everything the plan keeps resident: visit counts, code stream, perm + p0 + pflag + direct list (13 bytes per history),
+    // group table, launch order, per-block direct counts
+    out->plan_bytes = pl->cnt_bytes + 8 * pl->stream_words + P->m * 13 + (pl->n_groups + 1) * (int64_t)sizeof(PlanGroup) + pl->n_groups * 4 + pl->n_blocks * 4;
+    out->stream_bytes = 8 * pl->stream_words; out->cnt_bytes = pl->cnt_bytes;
+    out->staged_slots = pl->staged_slots; out->windowed_histories = pl->windowed_histories; out->windowed_visits = pl->windowed_visits;
     return PCT_OK;
 }
 

@@ -28,7 +28,7 @@ struct DevCfg {
     double s1c[3][6];          // Sigma1 moments: I_q(w) = w^(q+1) * sum_i s1c[q][i] w^i,  s1c[q][i] = a_i q! i!/(i+q+1)!
     double X0, log_coeff, step_frac, tie_eps, max_depth;
     int max_visits;
-    int stage_chunks;          // chunks per history in the staging buffer
+    int stage_chunks;          // chunks of the longest possible row (max_visits)
     double u_in, u_out;
     int bmin[3], bmax[3];      // bounding box of the hull voxels (inclusive); the whole grid if hull == NULL
 };
@@ -93,6 +93,7 @@ __host__ __device__ __forceinline__ unsigned win_addr(unsigned p) { return p ^ (
 
 struct SolvePlan {
     int64_t block_size, n_blocks, n_groups, n_direct, cnt_bytes;
+    int64_t staged_slots, windowed_histories, windowed_visits;   // per sweep (pct_plan_info)
     uint32_t* perm;          // sorted position -> history index (m)
     uint32_t* p0;            // packed window coordinate of the first visit, per sorted position
     uint8_t* pflag;          // per sorted position: 1 = windowed, 0 = not (rejected, or listed in direct_list)
@@ -186,13 +187,11 @@ struct ProfScope {
     } while (0)
 
 // launchers implemented in the .cu files (all enqueue on `st`, none synchronises unless stated)
-int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, int64_t i_base, int count, int stage_stride,
-                     ulonglong2* stage, uint32_t* nchunks, pct_paths* P, cudaStream_t st);
+int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, int64_t i_base, int count, ulonglong2* stage,
+                     unsigned long long* chunk_counter, pct_paths* P, cudaStream_t st);
 int launch_hull_bbox(pct_ctx* ctx, const uint8_t* hull, int* d_box6, cudaStream_t st);
 int launch_scan_u32(pct_ctx* ctx, const uint32_t* in, uint64_t* out, int64_t n, uint64_t base,
                     unsigned long long* d_total, cudaStream_t st);
-int launch_compact(pct_ctx* ctx, const ulonglong2* stage, const uint32_t* nchunks, const uint64_t* off, int count,
-                   int stage_stride, ulonglong2* codes, cudaStream_t st);
 int launch_decode(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, const uint64_t* row_ptr, int32_t* voxels,
                   cudaStream_t st);
 int launch_forward_project(pct_ctx* ctx, const pct_paths* P, const float* x, float* b_out, cudaStream_t st);

@@ -53,19 +53,22 @@ __global__ void __launch_bounds__(PK_THREADS) k_peak_red(float* __restrict__ d, 
     }
 }
 
-// shared-memory integer atomics (mode 0) or loads (mode 1) on `slots` 4-byte slots, random addresses
+// shared-memory integer atomics (mode 0, 2) or loads (mode 1, 3) on `slots` 4-byte slots; modes 0/1: random addresses,
+// modes 2/3: conflict-free (a random row of 32 slots per warp, lane l -> bank l)
 __global__ void __launch_bounds__(1024) k_peak_smem(int slots_mask, int iters, int mode, int* out) {
     extern __shared__ int sm[];
     for (int i = threadIdx.x; i <= slots_mask; i += blockDim.x) sm[i] = 0;
     __syncthreads();
-    unsigned s = (blockIdx.x * blockDim.x + threadIdx.x) * 2654435761u + 77u;
+    // modes 2/3: the sequence depends on the warp only, so all lanes draw the same row and differ in the bank
+    unsigned s = (mode >= 2 ? (blockIdx.x * blockDim.x + threadIdx.x) >> 5 : blockIdx.x * blockDim.x + threadIdx.x) * 2654435761u + 77u;
+    const int lane_or = mode >= 2 ? (int)(threadIdx.x & 31u) : 0, row_mask = mode >= 2 ? slots_mask & ~31 : slots_mask;
     int acc = 0;
     for (int i = 0; i < iters; ++i) {
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
             s = lcg(s);
-            const int idx = (int)((s >> 8) & (unsigned)slots_mask);
-            if (mode == 0) atomicAdd(&sm[idx], 1); else acc += sm[idx];
+            const int idx = (int)((s >> 8) & (unsigned)row_mask) | lane_or;
+            if ((mode & 1) == 0) atomicAdd(&sm[idx], 1); else acc += sm[idx];
         }
     }
     __syncthreads();
@@ -126,11 +129,12 @@ extern "C" int pct_measure_peaks(pct_ctx* ctx, pct_peaks* out) {
         const double rate = (double)blocks * PK_THREADS * iters / (ms * 1e-3);
         if (mode == 0) out->l2_red_f32_per_s = rate; else if (mode == 1) out->l2_red_v2_per_s = rate; else out->l2_red_v2_coalesced_per_s = rate;
     }
-    for (int mode = 0; mode < 2; ++mode) {            // shared memory: 8192 slots, 1024 threads, 2 CTAs / SM
+    for (int mode = 0; mode < 4; ++mode) {            // shared memory: 8192 slots, 1024 threads, 2 CTAs / SM
         const int blocks = sms * 2, iters = 2048, slots = 8192;
         if ((rc = time_best(ctx, [&] { k_peak_smem<<<blocks, 1024, slots * sizeof(int)>>>(slots - 1, iters, mode, (int*)buf); }, &ms)) != PCT_OK) return done(rc);
         const double rate = (double)blocks * 1024.0 * iters * 4.0 / (ms * 1e-3);
-        if (mode == 0) out->smem_atomic_per_s = rate; else out->smem_load_per_s = rate;
+        if (mode == 0) out->smem_atomic_per_s = rate; else if (mode == 1) out->smem_load_per_s = rate;
+        else if (mode == 2) out->smem_atomic_cf_per_s = rate; else out->smem_load_cf_per_s = rate;
     }
     out->num_sms = sms;
     return done(PCT_OK);

@@ -332,6 +332,42 @@ __global__ void k_plan_work_keys(const PlanGroup* __restrict__ groups, const uin
     vals[gi] = (uint32_t)gi;
 }
 
+// totals of one sweep for pct_plan_info: window slots staged (= the visited extent of every slab row that lies inside the
+// grid; an upper bound of the flushed slots), windowed histories and their visits.  tot = {slots, histories, visits}.
+__global__ void __launch_bounds__(256)
+k_plan_totals(const __grid_constant__ DevCfg g, const PlanGroup* __restrict__ groups, int64_t n_groups, const uint32_t* __restrict__ perm,
+              const uint8_t* __restrict__ pflag, const uint32_t* __restrict__ N, int64_t m, unsigned long long* __restrict__ tot) {
+    __shared__ unsigned long long sh[3][8];
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x, span = m > n_groups ? m : n_groups;
+    unsigned long long slots = 0, hist = 0, vis = 0;
+    for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < span; j += stride) {
+        if (j < n_groups) {
+            const PlanGroup G = groups[j];
+            if (G.cls != 7 && G.wps > 0 && G.dn_hi >= G.dn_lo && G.dz_hi >= G.dz_lo) {
+                const int dim_m = G.cls < 2 ? g.nx : g.ny, dir = (G.cls & 1) ? -1 : 1;
+                int rows = 0;
+                for (int r = 0; r < G.nslab * SLAB; ++r) rows += (unsigned)(G.m_first + dir * r) < (unsigned)dim_m;
+                slots += (unsigned long long)rows * (unsigned)(G.dn_hi - G.dn_lo + 1) * (unsigned)(G.dz_hi - G.dz_lo + 1);
+            }
+        }
+        if (j < m && pflag[j]) { ++hist; vis += N[perm[j]]; }
+    }
+    // one atomic per CTA and counter (same-address atomics serialise in L2)
+    unsigned long long v[3] = {slots, hist, vis};
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[k] += __shfl_xor_sync(0xffffffffu, v[k], o);
+        if ((threadIdx.x & 31) == 0) sh[k][threadIdx.x >> 5] = v[k];
+    }
+    __syncthreads();
+    if (threadIdx.x < 3) {
+        unsigned long long a = 0;
+        for (int w = 0; w < 8; ++w) a += sh[threadIdx.x][w];
+        if (a) atomicAdd(tot + threadIdx.x, a);
+    }
+}
+
 void free_solve_plan(SolvePlan* plan) {
     if (!plan) return;
     cudaDeviceSynchronize();         // freed on the legacy stream: nothing may still use the plan
@@ -348,6 +384,7 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     SolvePlan* plan = new (std::nothrow) SolvePlan();
     if (!plan) return set_error(ctx, PCT_E_OOM, "host allocation");
     plan->block_size = block_size; plan->n_blocks = n_blocks; plan->n_groups = 0; plan->n_direct = 0; plan->cnt_bytes = 0;
+    plan->staged_slots = plan->windowed_histories = plan->windowed_visits = 0;
     plan->perm = nullptr; plan->p0 = nullptr; plan->pflag = nullptr; plan->cnt = nullptr; plan->groups = nullptr;
     plan->direct_list = nullptr; plan->d_direct_count = nullptr; plan->stream = nullptr; plan->stream_words = 0; plan->launch_order = nullptr;
     uint64_t *keysA = nullptr, *keysB = nullptr, *cnt_off = nullptr;
@@ -486,6 +523,21 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
         ++ctx->launches;
     }
     lap("launch order");
+    {   // per-sweep totals for the roofline report
+        unsigned long long* d_tot = nullptr;
+        unsigned long long h_tot[3] = {0, 0, 0};
+        PLAN_CUDA(cache_alloc((void**)&d_tot, sizeof(h_tot)));
+        cudaError_t e = cudaMemsetAsync(d_tot, 0, sizeof(h_tot), st);
+        if (e == cudaSuccess) {
+            k_plan_totals<<<(unsigned)(ctx->num_sms * 8), 256, 0, st>>>(ctx->cfg, plan->groups, (int64_t)n_groups, plan->perm, plan->pflag, P->N, m, d_tot);
+            ++ctx->launches;
+            e = cudaMemcpyAsync(h_tot, d_tot, sizeof(h_tot), cudaMemcpyDeviceToHost, st);
+        }
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        cache_free(d_tot);
+        PLAN_CUDA(e);
+        plan->staged_slots = (int64_t)h_tot[0]; plan->windowed_histories = (int64_t)h_tot[1]; plan->windowed_visits = (int64_t)h_tot[2];
+    }
     plan->counts_ready.assign((size_t)n_blocks, 0);      // the count cache itself belongs to the context (pct_solve)
     plan->group_begin.resize((size_t)n_blocks + 1);
     plan->direct_count.resize((size_t)n_blocks);

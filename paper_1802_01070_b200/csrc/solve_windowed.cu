@@ -198,7 +198,7 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
     // ---- c_i and the CTA's fixed-point scale (R17, R21) -----------------------------------------------------------------
     // The scale must not be set by an outlier (an absurd WEPL makes |c_i| orders of magnitude larger than its neighbours'
     // and would coarsen the quantum of all 1024 members) nor by a non-finite value.  So: the CTA takes the MEDIAN binade
-    // of the finite |c_i| (histogram of the FP32 exponents), caps the scale at 64 x that binade, and every member whose
+    // of the finite |c_i| (histogram of the FP32 exponents), caps the scale at 512 x that binade, and every member whose
     // c_i is not finite or lies beyond the cap is "late": it adds nothing to the fixed-point window and instead walks its
     // row once with red.global.add.f32, exactly as the direct kernel does (Inf / NaN propagate the same way).
     float ci = 0.f;
@@ -247,7 +247,7 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
     if (!COUNT && G.max_cnt > 0) fix = min(29, max(FIX_BITS, 30 - (32 - __clz(G.max_cnt))));     // max_cnt < 2^(32 - clz)
     int ex = 0;
     if (mx > 0.f) frexpf(mx, &ex);                               // every finite |c_i| < 2^ex
-    if (e_med >= 0) ex = min(ex, e_med - 120);                   // 64 x the median's binade [2^(e-127), 2^(e-126))
+    if (e_med >= 0) ex = min(ex, e_med - 117);                   // 512 x the median's binade [2^(e-127), 2^(e-126))
     ex = max(ex, fix - 126);                                     // keeps both scales normal FP32 numbers
     const float scale = exp2f((float)(fix - ex)), inv_scale = exp2f((float)(ex - fix));
     const bool late = has && !(aci < ldexpf(1.f, ex));           // beyond the cap, Inf or NaN
