@@ -43,7 +43,7 @@ class Protons(C.Structure):
 
 class PathsStats(C.Structure):
     _fields_ = [(k, C.c_int64) for k in ("m", "total_visits", "n_rejected", "n_ties", "code_bytes", "header_bytes",
-                                          "total_samples")]
+                                          "total_samples", "n_sequential")]
 
 
 class ReconStats(C.Structure):
@@ -83,7 +83,7 @@ def load_library(path: Optional[str] = None):
     global _lib
     if _lib is not None and path is None:
         return _lib
-    path = path or _build.LIB
+    path = path or os.environ.get("PCT_LIBRARY") or _build.LIB      # PCT_LIBRARY: another build of libpct.so (A/B runs)
     if not os.path.exists(path):
         raise PctError(f"{path} is missing: run `python -m paper_1802_01070_b200.build` (no CPU fallback exists)")
     L = C.CDLL(path)
@@ -142,6 +142,7 @@ class Paths:
         ctx._check(ctx._L.pct_paths_info(handle, C.byref(st)))
         self.m, self.total_visits, self.n_rejected, self.n_ties = st.m, st.total_visits, st.n_rejected, st.n_ties
         self.code_bytes, self.header_bytes, self.total_samples = st.code_bytes, st.header_bytes, st.total_samples
+        self.n_sequential = st.n_sequential
 
     def plan_info(self) -> dict:
         """Statistics of the solve plan cached by the last pct_solve (zeros if it used the direct kernel)."""

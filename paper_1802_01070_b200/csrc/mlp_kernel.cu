@@ -117,11 +117,20 @@ __device__ __noinline__ void find_hull(const DevCfg& g, const uint8_t* __restric
     hit.ok = true;
 }
 
-__device__ __forceinline__ double horner6(const double (&c)[6], double x) {
-    double r = c[5];
-#pragma unroll
-    for (int i = 4; i >= 0; --i) r = fma(r, x, c[i]);
-    return r;
+// degree-5 polynomial, Estrin's scheme: the same five FMAs as Horner's rule but a dependent chain of three (x2 = x * x)
+__device__ __forceinline__ double poly5(const double (&c)[6], double x, double x2) {
+    const double p01 = fma(c[1], x, c[0]), p23 = fma(c[3], x, c[2]), p45 = fma(c[5], x, c[4]);
+    return fma(fma(p45, x2, p23), x2, p01);
+}
+
+// 1 / d for a normal, positive d: hardware seed (2^-23) and three Newton steps; not correctly rounded (a few 1e-16), which
+// is all the MLP needs (positions to ~1e-12 mm, R24)
+__device__ __forceinline__ double rcp_newton(double d) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
+    r = fma(r, fma(-d, r, 1.0), r);
+    r = fma(r, fma(-d, r, 1.0), r);
+    return fma(r, fma(-d, r, 1.0), r);
 }
 
 // 16-byte chunk writer: 42 codes, field k at bits 3(k%21) of word k/21; unused fields are 7 (pad).  A code is inserted
@@ -167,6 +176,8 @@ struct alignas(16) HistRec {
     double cq[3][6];                  // Sigma2 moments: J_q(d2) = int_0^d2 r^q f(D - r) dr = d2^(q+1) sum_j cq[q][j] d2^j
     int32_t vin, vout;                // V_s, V_e (linear voxel index)
     uint32_t K, flags;
+    int32_t cin[3];                   // V_s as (ix, iy, iz)
+    int32_t pad_;
 };
 
 // Spatial sort key of a history inside its batch: 2 mm cell of the entry tracker hit, v-major.  Neighbouring threads
@@ -254,6 +265,8 @@ k_hull(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const uint8_t* __r
                 for (int qq = 0; qq < 3; ++qq) r->cq[qq][j] = cj / (double)(j + qq + 1);
             }
         }
+#pragma unroll
+        for (int a = 0; a < 3; ++a) r->cin[a] = h_in.c[a];
         r->vin = h_in.c[0] + g.nx * (h_in.c[1] + g.ny * h_in.c[2]);
         r->vout = h_out.c[0] + g.nx * (h_out.c[1] + g.ny * h_out.c[2]);
     } while (false);
@@ -278,7 +291,7 @@ struct MlpHist {
 
 // A2 / R7: most likely lateral positions (t, v) at depth w1 = k du, 0 < k < K -- the Gaussian-conditioning form of the MLP
 // of ref [3] (positions only):  y = mu + Sigma1 R1^T (R1 Sigma1 R1^T + Sigma2)^-1 (y2 - R1 mu),  mu = R0 y0.
-// Sigma1 moments are Horner polynomials in w1 (DevCfg::s1c), Sigma2 moments in d2 = D - w1 (MlpHist::cq); the two log terms
+// Sigma1 moments are polynomials in w1 (DevCfg::s1c), Sigma2 moments in d2 = D - w1 (MlpHist::cq); the two log terms
 // are ln(w1 / X0) = ln k + ln(du / X0) and ln(d2 / X0) = ln(K - k) + ln(du / X0).
 __device__ __forceinline__ void mlp_sample(const DevCfg& g, const MlpHist& H, const double* __restrict__ logk, int k, int K,
                                            double& w1, double& tk, double& vk) {
@@ -287,15 +300,16 @@ __device__ __forceinline__ void mlp_sample(const DevCfg& g, const MlpHist& H, co
     const double l1 = fma(g.log_coeff, __ldg(logk + k) + H.log_du, 1.0), l2 = fma(g.log_coeff, __ldg(logk + (K - k)) + H.log_du, 1.0);
     const double g1 = l1 * l1, g2 = l2 * l2;
     const double w1_2 = w1 * w1, d2_2 = d2 * d2;
-    const double C1 = g1 * w1 * horner6(g.s1c[0], w1);
-    const double B1 = g1 * w1_2 * horner6(g.s1c[1], w1);
-    const double A1 = g1 * w1_2 * w1 * horner6(g.s1c[2], w1);
-    const double C2 = g2 * d2 * horner6(H.cq[0], d2);
-    const double B2 = g2 * d2_2 * horner6(H.cq[1], d2);
-    const double A2 = g2 * d2_2 * d2 * horner6(H.cq[2], d2);
+    const double gw = g1 * w1, gd = g2 * d2;
+    const double C1 = gw * poly5(g.s1c[0], w1, w1_2);
+    const double B1 = (gw * w1) * poly5(g.s1c[1], w1, w1_2);
+    const double A1 = (gw * w1_2) * poly5(g.s1c[2], w1, w1_2);
+    const double C2 = gd * poly5(H.cq[0], d2, d2_2);
+    const double B2 = (gd * d2) * poly5(H.cq[1], d2, d2_2);
+    const double A2 = (gd * d2_2) * poly5(H.cq[2], d2, d2_2);
     const double P0 = fma(d2, B1, A1), P1 = fma(d2, C1, B1);      // first row / col of Sigma1 R1^T
     const double S00 = fma(d2, P1, P0) + A2, S01 = P1 + B2, S11 = C1 + C2;
-    const double inv_det = 1.0 / (S00 * S11 - S01 * S01);
+    const double inv_det = rcp_newton(fma(S00, S11, -(S01 * S01)));
     const double G00 = (P0 * S11 - B1 * S01) * inv_det, G01 = (B1 * S00 - P0 * S01) * inv_det;
     const double mu_t = fma(w1, H.dt_in, H.t0), mu_v = fma(w1, H.dv_in, H.v0);
     tk = mu_t + G00 * (H.t2 - fma(d2, H.dt_in, mu_t)) + G01 * H.nu_t;
@@ -450,7 +464,7 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const HistRec* __restrict__ recs, c
 // CONSECUTIVE SAMPLES of one history:
 //   * lane l evaluates the MLP at depth k = k0 + l (all lanes converged, FP64) and maps the vertex straight to voxel index
 //     coordinates X = (P - lo) / h (one FMA pair per axis from (u, t, v));
-//   * the voxel of an interior vertex is round(X - 1/2).  A vertex is handled here only if it lies at least 1e-9 voxel
+//   * the voxel of an interior vertex is floor(X).  A vertex is handled here only if it lies at least 2e-9 voxel
 //     widths away from every face: then that voxel is the only closed voxel containing it, so it IS the state the
 //     sequential rule R9 reaches there, whatever happened before.  The segment's steps follow from the voxels of its two
 //     ends (shuffle from lane l-1): at most one per axis; two or three are ordered by their crossing parameters with the
@@ -459,14 +473,37 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const HistRec* __restrict__ recs, c
 //     it, by comparing P_K (mm) with the faces of the voxel the segment starts in;
 //   * a warp scan of the step counts gives every code its place in the row, the codes are collected in shared memory,
 //     packed 21 per word and written to the code stream at a place taken from chunk_counter.
-// Anything else -- a vertex within 1e-9 of a face, a segment that spans more than one voxel, a voxel outside the grid, a
+// Anything else -- a vertex within 2e-9 of a face, a segment that spans more than one voxel, a voxel outside the grid, a
 // row beyond the capacity -- sends the whole history to the sequential kernel (fb_list), which decides it exactly as
 // before.  On the synthetic workloads that is ~1e-6 of the histories.
 constexpr int WK_WARPS = 4;
-constexpr double ROUND_MAGIC = 6755399441055744.0;      // 2^52 + 2^51: (x + M) - M = x rounded to the nearest integer
-constexpr double FACE_GUARD = 1e-9;                     // in voxel widths
+// X + FIX_MAGIC has its unit in the last place at 2^-30 for -2^21 <= X < 2^21: the mantissa then holds X as 22.30 fixed
+// point (plus 2^51), i.e. floor(X) and the fractional part of X can be read off the two register halves.
+constexpr double FIX_MAGIC = 6291456.0;                 // 1.5 * 2^22
+constexpr int FIX_FRAC_BITS = 30;
+constexpr unsigned FIX_FRAC_MASK = (1u << FIX_FRAC_BITS) - 1u;
+constexpr unsigned FACE_GUARD = 2u;                     // 2 * 2^-30 ~ 2e-9 voxel widths
+// (hi:lo) >> 30 of a double in [2^22, 2^23) keeps the exponent field (0x415) above the 22 integer bits; subtracting it
+// together with the 2^21 offset of the fixed-point form leaves floor(X)
+constexpr unsigned FIX_INT_BIAS = (0x415u << 22) + (1u << 21);
 
-__global__ void __launch_bounds__(WK_WARPS * 32, 4)
+__device__ __forceinline__ int fix_floor(double s) { return (int)(__funnelshift_r((unsigned)__double2loint(s), (unsigned)__double2hiint(s), FIX_FRAC_BITS) - FIX_INT_BIAS); }
+// true if the fractional part lies within FACE_GUARD units of 0 or 1
+__device__ __forceinline__ bool fix_near_face(double s) {
+    return (((unsigned)__double2loint(s) & FIX_FRAC_MASK) - FACE_GUARD) > FIX_FRAC_MASK - 2u * FACE_GUARD;
+}
+// sqrt(q), q > 0, to ~1e-14 relative: FP32 reciprocal square root as the seed, one Newton step in FP64 (the polyline length
+// only enters the FP32 mean chord l_i)
+__device__ __forceinline__ double sqrt_fast(double q) {
+    const double y = (double)rsqrtf((float)q);
+    const double r = q * y;
+    return fma(0.5 * y, fma(-r, r, q), r);
+}
+
+#ifndef WK_MIN_BLOCKS
+#define WK_MIN_BLOCKS 4
+#endif
+__global__ void __launch_bounds__(WK_WARPS * 32, WK_MIN_BLOCKS)
 k_mlp_walk_warp(const __grid_constant__ DevCfg g, const HistRec* __restrict__ recs, const uint32_t* __restrict__ order,
                 const double* __restrict__ logk, int64_t i_base, int count, int row_cap, ulonglong2* __restrict__ codes,
                 unsigned long long* __restrict__ chunk_counter, uint64_t* __restrict__ code_off, uint32_t* __restrict__ Nout,
@@ -475,10 +512,12 @@ k_mlp_walk_warp(const __grid_constant__ DevCfg g, const HistRec* __restrict__ re
                 GenStats* __restrict__ stats) {
     extern __shared__ unsigned char row_codes[];            // WK_WARPS rows of row_cap bytes: one step code per byte
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const unsigned lt_mask = (1u << lane) - 1u;
     unsigned char* my_row = row_codes + (size_t)w * row_cap;
     unsigned long long st_vis = 0, st_smp = 0;
-    unsigned st_rej = 0, st_tie = 0;
-    const double o0 = -g.lo[0] * g.inv_h - 0.5, o1 = -g.lo[1] * g.inv_h - 0.5, o2 = -g.lo[2] * g.inv_h - 0.5;
+    unsigned st_rej = 0, st_tie = 0, st_fb = 0;
+    // index coordinates X_a = (P_a - lo_a) / h: faces are the integers
+    const double o0 = -g.lo[0] * g.inv_h, o1 = -g.lo[1] * g.inv_h, o2 = -g.lo[2] * g.inv_h;
     for (int q = blockIdx.x * WK_WARPS + w; q < count; q += gridDim.x * WK_WARPS) {
         const int p = (int)order[count - 1 - q];          // longest first
         const int64_t i = i_base + p;
@@ -495,115 +534,116 @@ k_mlp_walk_warp(const __grid_constant__ DevCfg g, const HistRec* __restrict__ re
         MlpHist H;
         H.load(rec);
         const double cxh = rec->cph * g.inv_h, sxh = rec->sph * g.inv_h;
-        const int vin = rec->vin, vout = rec->vout;
+        const double b0 = rec->pout[0], b1 = rec->pout[1], b2 = rec->pout[2];
+        const double XO0 = fma(b0, g.inv_h, o0), XO1 = fma(b1, g.inv_h, o1), XO2 = fma(b2, g.inv_h, o2);
         // carried from round to round: voxel and index coordinates of the vertex before lane 0's
-        int cP0 = vin % g.nx, cP1 = (vin / g.nx) % g.ny, cP2 = vin / (g.nx * g.ny);
+        int cP0 = rec->cin[0], cP1 = rec->cin[1], cP2 = rec->cin[2];
         double XP0 = fma(rec->pin[0], g.inv_h, o0), XP1 = fma(rec->pin[1], g.inv_h, o1), XP2 = fma(rec->pin[2], g.inv_h, o2);
         double Lsum = 0.0;
         int steps = 0;                                      // codes written so far
         bool tie = false, give_up = false;
-        int cE0 = cP0, cE1 = cP1, cE2 = cP2;                // voxel the walk ends in
+        int cB0 = 0, cB1 = 0, cB2 = 0;
         for (int k0 = 1; k0 <= K; k0 += 32) {
             const int k = k0 + lane;
             const bool valid = k <= K, last = k == K;
-            double X0, X1, X2;
-            int cB0 = 0, cB1 = 0, cB2 = 0;
-            bool odd = false;                               // this lane cannot decide its segment locally
-            if (k < K) {
-                double w1, tk, vk;
-                mlp_sample(g, H, logk, k, K, w1, tk, vk);
-                const double uk = H.u0 + w1;
-                X0 = fma(uk, cxh, fma(tk, -sxh, o0)); X1 = fma(uk, sxh, fma(tk, cxh, o1)); X2 = fma(vk, g.inv_h, o2);
-                const double s0 = X0 + ROUND_MAGIC, s1 = X1 + ROUND_MAGIC, s2 = X2 + ROUND_MAGIC;
-                cB0 = __double2loint(s0); cB1 = __double2loint(s1); cB2 = __double2loint(s2);
-                odd = fabs(X0 - (s0 - ROUND_MAGIC)) > 0.5 - FACE_GUARD || fabs(X1 - (s1 - ROUND_MAGIC)) > 0.5 - FACE_GUARD ||
-                      fabs(X2 - (s2 - ROUND_MAGIC)) > 0.5 - FACE_GUARD;
-            } else {
-                X0 = fma(rec->pout[0], g.inv_h, o0); X1 = fma(rec->pout[1], g.inv_h, o1); X2 = fma(rec->pout[2], g.inv_h, o2);
-            }
+            // every lane evaluates the MLP (the lanes at and beyond k = K redo sample K - 1; lane k = K then takes P_K, the others idle)
+            double w1, tk, vk;
+            mlp_sample(g, H, logk, min(k, K - 1), K, w1, tk, vk);
+            const double uk = H.u0 + w1;
+            double X0 = fma(uk, cxh, fma(tk, -sxh, o0)), X1 = fma(uk, sxh, fma(tk, cxh, o1)), X2 = fma(vk, g.inv_h, o2);
+            const double s0 = X0 + FIX_MAGIC, s1 = X1 + FIX_MAGIC, s2 = X2 + FIX_MAGIC;
+            cB0 = fix_floor(s0); cB1 = fix_floor(s1); cB2 = fix_floor(s2);
+            bool odd = k < K && (fix_near_face(s0) || fix_near_face(s1) || fix_near_face(s2));   // cannot be decided lane-locally
             int cA0 = __shfl_up_sync(0xffffffffu, cB0, 1), cA1 = __shfl_up_sync(0xffffffffu, cB1, 1), cA2 = __shfl_up_sync(0xffffffffu, cB2, 1);
             double XA0 = __shfl_up_sync(0xffffffffu, X0, 1), XA1 = __shfl_up_sync(0xffffffffu, X1, 1), XA2 = __shfl_up_sync(0xffffffffu, X2, 1);
             if (lane == 0) { cA0 = cP0; cA1 = cP1; cA2 = cP2; XA0 = XP0; XA1 = XP1; XA2 = XP2; }
             if (last) {
-                // R9 on the segment into P_K: step across the axes on which P_K lies strictly outside the closed start voxel
-                const double b0 = rec->pout[0], b1 = rec->pout[1], b2 = rec->pout[2];
+                // the segment into P_K, which lies exactly on a face of V_e by construction: R9 as stated -- step across the axes
+                // on which P_K (mm) lies strictly outside the closed start voxel
+                X0 = XO0; X1 = XO1; X2 = XO2;
                 cB0 = cA0 + (b0 > face_coord(g, 0, cA0 + 1) ? 1 : (b0 < face_coord(g, 0, cA0) ? -1 : 0));
                 cB1 = cA1 + (b1 > face_coord(g, 1, cA1 + 1) ? 1 : (b1 < face_coord(g, 1, cA1) ? -1 : 0));
                 cB2 = cA2 + (b2 > face_coord(g, 2, cA2 + 1) ? 1 : (b2 < face_coord(g, 2, cA2) ? -1 : 0));
                 odd = b0 > face_coord(g, 0, cB0 + 1) || b0 < face_coord(g, 0, cB0) || b1 > face_coord(g, 1, cB1 + 1) || b1 < face_coord(g, 1, cB1) ||
                       b2 > face_coord(g, 2, cB2 + 1) || b2 < face_coord(g, 2, cB2);              // more than one voxel away
             }
-            const int d0 = valid ? cB0 - cA0 : 0, d1 = valid ? cB1 - cA1 : 0, d2 = valid ? cB2 - cA2 : 0;
-            if (valid) odd = odd || (unsigned)(d0 + 1) > 2u || (unsigned)(d1 + 1) > 2u || (unsigned)(d2 + 1) > 2u ||
-                             (unsigned)cB0 >= (unsigned)g.nx || (unsigned)cB1 >= (unsigned)g.ny || (unsigned)cB2 >= (unsigned)g.nz;
-            else odd = false;
+            int d0 = cB0 - cA0, d1 = cB1 - cA1, d2 = cB2 - cA2;
+            if (!valid) { d0 = 0; d1 = 0; d2 = 0; }
+            // a step of more than one voxel on some axis, or a voxel outside the grid: not for this kernel
+            odd = odd || max(max((unsigned)(d0 + 1), (unsigned)(d1 + 1)), (unsigned)(d2 + 1)) > 2u ||
+                  (valid && ((unsigned)cB0 >= (unsigned)g.nx || (unsigned)cB1 >= (unsigned)g.ny || (unsigned)cB2 >= (unsigned)g.nz));
             if (__any_sync(0xffffffffu, odd)) { give_up = true; break; }
-            const int n = (d0 != 0) + (d1 != 0) + (d2 != 0);
+            const int n = (d0 & 1) + (d1 & 1) + (d2 & 1);
             // segment length: h |X_B - X_A| (the index map is a rotation scaled by 1/h)
             const double e0 = X0 - XA0, e1 = X1 - XA1, e2 = X2 - XA2;
-            const double seg_len = valid ? g.h * sqrt(fma(e0, e0, fma(e1, e1, e2 * e2))) : 0.0;
+            const double seg_len = valid ? g.h * sqrt_fast(fma(e0, e0, fma(e1, e1, e2 * e2))) : 0.0;
             Lsum += seg_len;
             int r0 = 0, r1 = 0, r2 = 0;                     // place of each axis' step among this segment's steps
             if (n >= 2) {
                 // crossing parameter of axis a: s_a = num_a / den_a, num_a = distance of A from the face, den_a = |B_a - A_a|
-                const double n0 = fabs((double)(cA0 + (d0 > 0 ? 1 : 0)) - 0.5 - XA0), n1 = fabs((double)(cA1 + (d1 > 0 ? 1 : 0)) - 0.5 - XA1),
-                             n2 = fabs((double)(cA2 + (d2 > 0 ? 1 : 0)) - 0.5 - XA2);
+                const double n0 = fabs((double)(cA0 + (d0 > 0 ? 1 : 0)) - XA0), n1 = fabs((double)(cA1 + (d1 > 0 ? 1 : 0)) - XA1),
+                             n2 = fabs((double)(cA2 + (d2 > 0 ? 1 : 0)) - XA2);
                 const double a0 = fabs(e0), a1 = fabs(e1), a2 = fabs(e2);
                 const double l01 = n0 * a1, l10 = n1 * a0, l02 = n0 * a2, l20 = n2 * a0, l12 = n1 * a2, l21 = n2 * a1;
                 const bool p01 = d0 != 0 && d1 != 0, p02 = d0 != 0 && d2 != 0, p12 = d1 != 0 && d2 != 0;
                 // s_a < s_b <=> l_ab < l_ba; on equality the lower axis goes first
-                r0 = (p01 && l10 < l01) + (p02 && l20 < l02);
-                r1 = (p01 && !(l10 < l01)) + (p12 && l21 < l12);
-                r2 = (p02 && !(l20 < l02)) + (p12 && !(l21 < l12));
+                const bool f10 = p01 && l10 < l01, f20 = p02 && l20 < l02, f21 = p12 && l21 < l12;
+                r0 = (int)f10 + (int)f20;
+                r1 = (int)(p01 && !f10) + (int)f21;
+                r2 = (int)(p02 && !f20) + (int)(p12 && !f21);
                 const double te = g.tie_eps;
                 if ((p01 && fabs(l01 - l10) * seg_len < te * (a0 * a1)) || (p02 && fabs(l02 - l20) * seg_len < te * (a0 * a2)) ||
                     (p12 && fabs(l12 - l21) * seg_len < te * (a1 * a2))) tie = true;
             }
-            int incl = n;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += y; }
-            const int total = __shfl_sync(0xffffffffu, incl, 31);
+            // places of this lane's codes in the row: prefix sum of n (0..3) over the lanes from two ballots
+            const unsigned m_lo = __ballot_sync(0xffffffffu, n & 1), m_hi = __ballot_sync(0xffffffffu, n & 2);
+            const int total = __popc(m_lo) + 2 * __popc(m_hi);
             if (steps + total + 1 > g.max_visits) { give_up = true; break; }      // the sequential kernel flags the capacity
-            const int at = steps + incl - n;
-            if (d0 != 0) my_row[at + r0] = (unsigned char)(d0 < 0 ? 1 : 0);
-            if (d1 != 0) my_row[at + r1] = (unsigned char)(d1 < 0 ? 3 : 2);
-            if (d2 != 0) my_row[at + r2] = (unsigned char)(d2 < 0 ? 5 : 4);
+            unsigned char* at = my_row + steps + __popc(m_lo & lt_mask) + 2 * __popc(m_hi & lt_mask);
+            if (d0 != 0) at[r0] = (unsigned char)(d0 < 0 ? 1 : 0);
+            if (d1 != 0) at[r1] = (unsigned char)(d1 < 0 ? 3 : 2);
+            if (d2 != 0) at[r2] = (unsigned char)(d2 < 0 ? 5 : 4);
             steps += total;
-            const int src = min(31, K - k0);                // lane of the last valid vertex of this round
             cP0 = __shfl_sync(0xffffffffu, cB0, 31); cP1 = __shfl_sync(0xffffffffu, cB1, 31); cP2 = __shfl_sync(0xffffffffu, cB2, 31);
             XP0 = __shfl_sync(0xffffffffu, X0, 31); XP1 = __shfl_sync(0xffffffffu, X1, 31); XP2 = __shfl_sync(0xffffffffu, X2, 31);
-            cE0 = __shfl_sync(0xffffffffu, cB0, src); cE1 = __shfl_sync(0xffffffffu, cB1, src); cE2 = __shfl_sync(0xffffffffu, cB2, src);
         }
         if (give_up) {
-            if (lane == 0) fb_list[atomicAdd(fb_count, 1u)] = (uint32_t)p;
+            if (lane == 0) { fb_list[atomicAdd(fb_count, 1u)] = (uint32_t)p; ++st_fb; }
             continue;
         }
         if (__any_sync(0xffffffffu, tie)) flags |= PCT_TIE;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) Lsum += __shfl_xor_sync(0xffffffffu, Lsum, o);
         const int N = steps + 1;
-        const int end_v = cE0 + g.nx * (cE1 + g.ny * cE2);
-        if (end_v != vout) flags |= PCT_END_MISMATCH;                                                        // R10
+        const int src = (K - 1) & 31;                       // lane that held vertex K in the final round
+        const int end_v = __shfl_sync(0xffffffffu, cB0, src) + g.nx * (__shfl_sync(0xffffffffu, cB1, src) + g.ny * __shfl_sync(0xffffffffu, cB2, src));
+        if (end_v != rec->vout) flags |= PCT_END_MISMATCH;                                                   // R10
         const int n_chunks = (steps + CODES_PER_CHUNK - 1) / CODES_PER_CHUNK;
         unsigned long long off = 0ull;
         if (lane == 0 && n_chunks > 0) off = atomicAdd(chunk_counter, (unsigned long long)n_chunks);
         off = __shfl_sync(0xffffffffu, off, 0);
         __syncwarp();
+        // pack 21 codes per 64-bit word: four lanes per word (6 + 6 + 6 + 3 codes), OR-combined by two shuffles
         unsigned long long* out = reinterpret_cast<unsigned long long*>(codes + off);
-        for (int wd = lane; wd < 2 * n_chunks; wd += 32) {
-            unsigned long long word = 0ull;
-            const int base = wd * CODES_PER_WORD;
+        const int part = lane & 3, n_words = 2 * n_chunks;
+        for (int w0 = 0; w0 < n_words; w0 += 8) {
+            const int wd = w0 + (lane >> 2);
+            const int first = wd * CODES_PER_WORD + part * 6;
+            unsigned piece = 0u;
 #pragma unroll
-            for (int j = 0; j < CODES_PER_WORD; ++j) {
-                const unsigned long long c = base + j < steps ? (unsigned long long)my_row[base + j] : 7ull;
-                word |= c << (3 * j);
+            for (int j = 0; j < 6; ++j) {
+                const unsigned c = (first + j < steps) ? (unsigned)my_row[first + j] : 7u;
+                if (part * 6 + j < CODES_PER_WORD) piece |= c << (3 * j);
             }
-            if (base + CODES_PER_WORD > steps) word |= 1ull << 63;     // bit 63 is no code field; set in partial words like the sequential writer's
-            out[wd] = word;
+            unsigned long long word = (unsigned long long)piece << (18 * part);
+            word |= __shfl_xor_sync(0xffffffffu, word, 1);
+            word |= __shfl_xor_sync(0xffffffffu, word, 2);
+            if (wd * CODES_PER_WORD + CODES_PER_WORD > steps) word |= 1ull << 63;   // bit 63 is no code field; set in partial words like the sequential writer's
+            if (part == 0 && wd < n_words) out[wd] = word;
         }
         __syncwarp();
         if (lane == 0) {
-            code_off[i] = off; Nout[i] = (uint32_t)N; start_out[i] = vin; end_out[i] = end_v;
+            code_off[i] = off; Nout[i] = (uint32_t)N; start_out[i] = rec->vin; end_out[i] = end_v;
             ell_out[i] = (float)(Lsum / (double)N);                                                          // R11
             flags_out[i] = (uint8_t)(flags & 0xffu);
             st_vis += (unsigned long long)N; st_smp += (unsigned long long)K; st_tie += (flags & PCT_TIE) ? 1u : 0u;
@@ -614,6 +654,7 @@ k_mlp_walk_warp(const __grid_constant__ DevCfg g, const HistRec* __restrict__ re
         if (st_vis) atomicAdd(&stats->total_visits, st_vis);
         if (st_rej) atomicAdd(&stats->n_rejected, (unsigned long long)st_rej);
         if (st_tie) atomicAdd(&stats->n_ties, (unsigned long long)st_tie);
+        if (st_fb) atomicAdd(&stats->n_sequential, (unsigned long long)st_fb);
     }
 }
 
