@@ -273,7 +273,7 @@ def bench_workload(args, cfg, dev, local, world, dist, steps, warmup, e2e_steps,
             ev[2].record()
         info.update(samples=paths.total_samples, plan=paths.plan_info(), visits=paths.total_visits, rejected=paths.n_rejected,
                     ties=paths.n_ties, code_bytes=paths.code_bytes, header_bytes=paths.header_bytes,
-                    sequential=paths.n_sequential)
+                    general_segments=paths.n_general_segments)
         if "tie_log" not in info and ev is None:      # the logged boundary ties (north_star), once, outside the timed steps
             idx, n = ctx.paths_flagged(paths, binding.TIE, cap=64)
             info["tie_log"] = {"count": n, "fraction": n / max(cfg.m, 1), "history_indices": idx.tolist(),
@@ -403,7 +403,7 @@ def bench_workload(args, cfg, dev, local, world, dist, steps, warmup, e2e_steps,
         "value_definition": "P x iters / whole-step time (pct_generate_mlp + plan + pct_solve)",
         "path_voxel_visits": P, "rejected": info["rejected"], "ties": info["ties"], "tie_log": info.get("tie_log"),
         "code_bytes": info["code_bytes"], "header_bytes": info["header_bytes"],
-        "k1_sequential_histories": info["sequential"],
+        "k1_general_segments": info["general_segments"],
         "solver_updates_per_s": world * updates_per_step * steps / (ms_solve * 1e-3),
         "solver_updates_per_s_definition": "P / t_iter, SURVEY.md 8(d): one sweep of A5-A7, plan build amortised in",
         "solver_ms_per_iter": ms_solve / (steps * cfg.iters),

@@ -79,9 +79,8 @@ typedef struct {
 typedef struct {
     int64_t m, total_visits, n_rejected, n_ties, code_bytes, header_bytes;
     int64_t total_samples; /* sum of K over the accepted histories: MLP segments evaluated (R8); K1's unit of FP64 work */
-    int64_t n_sequential;  /* histories the warp-cooperative walk kernel handed to the sequential one (a vertex within
-                            * 2e-9 voxel widths of a face, a segment spanning more than one voxel, a rejection): same result,
-                            * slower kernel */
+    int64_t n_general_segments; /* polyline segments that took K1's general stepping loop instead of the loop-free path (longer
+                                 * than a voxel on some axis, leaving the grid, row capacity): same result, slower */
 } pct_paths_stats;
 
 typedef struct {

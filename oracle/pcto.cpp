@@ -459,6 +459,52 @@ int pcto_solve(const pcto_paths* P, const float* b, const float* x0, int iters, 
     return 0;
 }
 
+// R27: the same iteration with per-history weights and a box clamp (ref [9]-style options, "standard
+// iterative solver [9]"):  x <- clamp( x + lambda * U_t * sum_{i in B_t} w_i [(b_i - <a_i,x>) / ||a_i||^2] a_i ),
+// U_t as in pcto_solve (visit counts, independent of w), the clamp applied to the voxels the block touched.
+int pcto_solve_ex(const pcto_paths* P, const float* b, const float* x0, const float* w, int iters, int64_t block_size,
+                  double lambda, double clamp_lo, double clamp_hi, float* x_out, double* x_out_f64, int nthreads) {
+    if (!P || !b || !x0 || iters < 0 || block_size < 1 || (!x_out && !x_out_f64)) return -1;
+    (void)nthreads;
+    const int64_t n = P->n_vox, m = P->m;
+    const bool clamp = clamp_lo <= clamp_hi;
+    std::vector<double> x(x0, x0 + n), delta(n, 0.0);
+    std::vector<uint32_t> s(n, 0u);
+    std::vector<int32_t> touched;
+    std::vector<double> c((size_t)std::min(block_size, std::max<int64_t>(m, 1)));
+    for (int it = 0; it < iters; ++it) {
+        for (int64_t i0 = 0; i0 < m; i0 += block_size) {
+            const int64_t i1 = std::min(m, i0 + block_size);
+            for (int64_t i = i0; i < i1; ++i) {                       // R14: residuals against the x of the block's start
+                int64_t N; const int32_t* r = P->row(i, &N);
+                double S = 0.0;
+                for (int64_t k = 0; k < N; ++k) S += x[r[k]];
+                const double l = (double)P->ell[i], wi = w ? (double)w[i] : 1.0;
+                c[i - i0] = N > 0 ? wi * ((double)b[i] - l * S) / ((double)N * l) : 0.0;
+            }
+            for (int64_t i = i0; i < i1; ++i) {
+                int64_t N; const int32_t* r = P->row(i, &N);
+                for (int64_t k = 0; k < N; ++k) {
+                    const int32_t j = r[k];
+                    if (s[j]++ == 0) touched.push_back(j);
+                    delta[j] += c[i - i0];
+                }
+            }
+            for (int32_t j : touched) {
+                x[j] += lambda * delta[j] / (double)std::max<uint32_t>(1u, s[j]);
+                if (clamp) x[j] = std::min(std::max(x[j], clamp_lo), clamp_hi);
+                delta[j] = 0.0; s[j] = 0u;
+            }
+            touched.clear();
+        }
+    }
+    for (int64_t j = 0; j < n; ++j) {
+        if (x_out) x_out[j] = (float)x[j];
+        if (x_out_f64) x_out_f64[j] = x[j];
+    }
+    return 0;
+}
+
 int pcto_scatter_moments(const pcto_mlp_params* p, double w_a, double w_b, double W, double out[3]) {
     if (!p || !out) return -1;
     scatter_moments(p->poly, w_a, w_b, W, out);

@@ -64,6 +64,27 @@ int pcto_column_counts(const pcto_paths*, int64_t i0, int64_t i1, uint32_t* coun
 int pcto_solve(const pcto_paths*, const float* b, const float* x0, int iters, int64_t block_size, double lambda,
                float* x_out, double* x_out_f64 /* may be NULL */, int nthreads);
 
+/* A5-A8 with the options of ref [9]-style solvers (reading R27): per-history weights w_i in [0, 1] (NULL = all one)
+ * multiplying the row's correction, x <- x + lambda U_t sum_i w_i [(b_i - <a_i,x>)/||a_i||^2] a_i, and a box clamp
+ * x_j <- min(max(x_j, clamp_lo), clamp_hi) applied to the voxels a block updates, right after its update
+ * (clamp_lo > clamp_hi = no clamp).  With w = NULL and no clamp this is pcto_solve. */
+int pcto_solve_ex(const pcto_paths*, const float* b, const float* x0, const float* w, int iters, int64_t block_size,
+                  double lambda, double clamp_lo, double clamp_hi, float* x_out, double* x_out_f64, int nthreads);
+
+/* --- preprocessing in front of the hot path (pcto_pre.cpp; readings R25, R26) --- */
+typedef struct {
+    int32_t n_theta;   /* direction bins over [0, 2 pi) */
+    int32_t n_s;       /* lateral bins of width ds_mm, centred on the rotation axis */
+    double ds_mm;
+    int32_t min_count; /* bins with fewer histories count as empty (0) */
+} pcto_fbp_params;
+/* FBP image from tracker records + WEPL.  sino_mean: [nz][n_theta][n_s] mean WEPL per bin, or NULL. */
+int pcto_fbp(const pcto_geometry*, const pcto_protons*, const float* b, const pcto_fbp_params*, double* sino_mean,
+             double* x0_out);
+/* Hull by space carving: voxels crossed (chord > min_chord_mm) by a history with WEPL < wepl_air_mm become 0, all others 1 */
+int pcto_hull_carve(const pcto_geometry*, const pcto_protons*, const float* b, double wepl_air_mm, double min_chord_mm,
+                    uint8_t* hull_out);
+
 /* --- building blocks exposed for the pins in tests/ --- */
 /* out = { int (W-w)^2 f dw, int (W-w) f dw, int f dw } over [w_a, w_b] */
 int pcto_scatter_moments(const pcto_mlp_params*, double w_a, double w_b, double W, double out[3]);

@@ -22,11 +22,11 @@ REJECT_MASK = REJ_MISS | REJ_ORDER | REJ_DEPTH | REJ_LEFT_GRID | REJ_CAPACITY | 
 
 
 def build(force: bool = False) -> str:
-    src = [os.path.join(_DIR, "pcto.cpp"), os.path.join(_DIR, "pcto.h")]
+    src = [os.path.join(_DIR, "pcto.cpp"), os.path.join(_DIR, "pcto_pre.cpp"), os.path.join(_DIR, "pcto.h")]
     if not force and os.path.exists(_SO) and all(os.path.getmtime(_SO) >= os.path.getmtime(s) for s in src):
         return _SO
     cmd = ["g++", "-std=c++17", "-O2", "-fopenmp", "-ffp-contract=off", "-fPIC", "-shared", "-Wall", "-Wextra",
-           "-o", _SO, src[0]]
+           "-o", _SO, src[0], src[1]]
     subprocess.run(cmd, check=True, cwd=_DIR)
     return _SO
 
@@ -43,6 +43,10 @@ class MlpParams(C.Structure):
 
 
 _PD = C.POINTER(C.c_double)
+
+
+class FbpParams(C.Structure):
+    _fields_ = [("n_theta", C.c_int32), ("n_s", C.c_int32), ("ds_mm", C.c_double), ("min_count", C.c_int32)]
 
 
 class Protons(C.Structure):
@@ -74,6 +78,12 @@ def lib():
                                     C.c_void_p, C.c_void_p, C.c_int, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
         L.pcto_walk_polyline.argtypes = [C.POINTER(Geometry), C.c_double, C.c_void_p, C.c_int, C.c_int32,
                                          C.c_void_p, C.c_int, C.POINTER(C.c_int32)]
+        L.pcto_solve_ex.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int64, C.c_double,
+                                    C.c_double, C.c_double, C.c_void_p, C.c_void_p, C.c_int]
+        L.pcto_fbp.argtypes = [C.POINTER(Geometry), C.POINTER(Protons), C.c_void_p, C.POINTER(FbpParams), C.c_void_p,
+                               C.c_void_p]
+        L.pcto_hull_carve.argtypes = [C.POINTER(Geometry), C.POINTER(Protons), C.c_void_p, C.c_double, C.c_double,
+                                      C.c_void_p]
         _lib = L
     return _lib
 
@@ -154,6 +164,17 @@ class Paths:
                                 x64.ctypes.data if f64 else None, nthreads) == 0
         return (x, x64) if f64 else x
 
+    def solve_ex(self, b, x0, w, iters: int, block_size: int, lam: float, clamp_lo: float = 1.0, clamp_hi: float = 0.0):
+        """R27: weighted rows (w float32[m] or None) and box clamp (clamp_lo > clamp_hi = none)."""
+        b = np.ascontiguousarray(b, dtype=np.float32).reshape(-1)
+        x0 = np.ascontiguousarray(x0, dtype=np.float32).reshape(-1)
+        wv = None if w is None else np.ascontiguousarray(w, dtype=np.float32).reshape(-1)
+        assert b.size == self.m and x0.size == self.n and (wv is None or wv.size == self.m)
+        x = np.zeros(self.n, dtype=np.float32)
+        assert lib().pcto_solve_ex(self._h, b.ctypes.data, x0.ctypes.data, wv.ctypes.data if wv is not None else None,
+                                   iters, block_size, lam, clamp_lo, clamp_hi, x.ctypes.data, None, 0) == 0
+        return x
+
     def free(self):
         if self._h:
             lib().pcto_paths_free(self._h)
@@ -201,3 +222,27 @@ def walk_polyline(geom: Geometry, verts: np.ndarray, start_voxel: int, tie_eps_m
     if n < 0:
         return None, 0
     return out[:n].copy(), ties.value
+
+
+def fbp(geom: Geometry, protons: ProtonArrays, b, n_theta: int, n_s: int, ds_mm: float, min_count: int = 1,
+        want_sinogram: bool = False):
+    """R25: FBP image float64[nz, ny, nx] (and the mean-WEPL sinogram [nz, n_theta, n_s] if asked for)."""
+    b = np.ascontiguousarray(b, dtype=np.float32).reshape(-1)
+    assert b.size == protons.m
+    fp = FbpParams(int(n_theta), int(n_s), float(ds_mm), int(min_count))
+    x0 = np.zeros(geom.nx * geom.ny * geom.nz, dtype=np.float64)
+    sino = np.zeros((geom.nz, n_theta, n_s), dtype=np.float64) if want_sinogram else None
+    assert lib().pcto_fbp(C.byref(geom), C.byref(protons.c), b.ctypes.data, C.byref(fp),
+                          sino.ctypes.data if want_sinogram else None, x0.ctypes.data) == 0
+    x0 = x0.reshape(geom.nz, geom.ny, geom.nx)
+    return (x0, sino) if want_sinogram else x0
+
+
+def hull_carve(geom: Geometry, protons: ProtonArrays, b, wepl_air_mm: float, min_chord_mm: float) -> np.ndarray:
+    """R26: uint8[nz, ny, nx], 1 = never crossed (chord > min_chord_mm) by a history with WEPL < wepl_air_mm."""
+    b = np.ascontiguousarray(b, dtype=np.float32).reshape(-1)
+    assert b.size == protons.m
+    out = np.zeros(geom.nx * geom.ny * geom.nz, dtype=np.uint8)
+    assert lib().pcto_hull_carve(C.byref(geom), C.byref(protons.c), b.ctypes.data, float(wepl_air_mm),
+                                 float(min_chord_mm), out.ctypes.data) == 0
+    return out.reshape(geom.nz, geom.ny, geom.nx)

@@ -43,7 +43,7 @@ class Protons(C.Structure):
 
 class PathsStats(C.Structure):
     _fields_ = [(k, C.c_int64) for k in ("m", "total_visits", "n_rejected", "n_ties", "code_bytes", "header_bytes",
-                                          "total_samples", "n_sequential")]
+                                          "total_samples", "n_general_segments")]
 
 
 class ReconStats(C.Structure):
@@ -142,7 +142,7 @@ class Paths:
         ctx._check(ctx._L.pct_paths_info(handle, C.byref(st)))
         self.m, self.total_visits, self.n_rejected, self.n_ties = st.m, st.total_visits, st.n_rejected, st.n_ties
         self.code_bytes, self.header_bytes, self.total_samples = st.code_bytes, st.header_bytes, st.total_samples
-        self.n_sequential = st.n_sequential
+        self.n_general_segments = st.n_general_segments
 
     def plan_info(self) -> dict:
         """Statistics of the solve plan cached by the last pct_solve (zeros if it used the direct kernel)."""

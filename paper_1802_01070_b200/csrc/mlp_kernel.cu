@@ -2,13 +2,11 @@
 // step codes (A3).  PAPER.md:7 ("calculating the individual proton's most likely path [3]" gives the rows of A),
 // PAPER.md:26 ("each proton as an individual thread").  FP64 throughout; readings R1-R12 of DESIGN.md.
 //
-// Three kernels per batch of 2^20 histories: k_hull (one thread per history: hull entry/exit and the per-history part of
-// the MLP), k_mlp_walk_warp (one WARP per history, lane = MLP sample: the bulk of the FP64 work, all lanes converged) and
-// k_mlp_walk (one thread per history, the sequential rule R9 step by step: the few histories the warp kernel hands over).
-// Bound by the FP64 pipe (~100 FP64 instructions per MLP sample, K ~ 2*depth samples), not by memory: 72 B in, ~60-170 B
-// out per history.  Rows are written straight to the code stream; their place comes from an atomic chunk counter.
-#include <cstdlib>
-
+// Two kernels per batch of 2^20 histories, one thread per history: k_hull (hull entry/exit and the per-history part of the
+// MLP) and k_mlp_walk (the MLP sample by sample, the voxel steps of every segment without a data-dependent loop).  Bound by
+// instruction issue: ~90 FP64 instructions per MLP sample (K ~ 2*depth samples), each of which holds the issue port for
+// two cycles on sm_100a, plus the bookkeeping of the walk; memory is irrelevant (72 B in, ~60-170 B out per history).
+// Rows are copied to the code stream at a place taken from an atomic chunk counter.
 #include <cub/device/device_radix_sort.cuh>
 
 #include "pct_internal.cuh"
@@ -316,25 +314,36 @@ __device__ __forceinline__ void mlp_sample(const DevCfg& g, const MlpHist& H, co
     vk = mu_v + G00 * (H.v2 - fma(d2, H.dv_in, mu_v)) + G01 * H.nu_v;
 }
 
-// ---- A2 + A3, sequential form: one thread per history, rule R9 applied step by step --------------------------------------
-// The general routine: it handles every case (vertices that lie exactly on voxel faces, segments longer than a voxel,
-// paths that leave the grid or exceed the row capacity).  k_mlp_walk_warp does the bulk of the work and sends the histories
-// it cannot decide lane-locally here (list / list_count); with list == NULL it walks all `count` histories of the batch
-// (order[]), which is how PCT_K1_SEQUENTIAL=1 runs K1.  Codes go to a staging row per thread and are copied to the code
-// stream once the row's length is known (chunk_counter allocates its place).
+// sqrt(q), q > 0, to ~1e-14 relative: FP32 reciprocal square root as the seed, one Newton step in FP64 (the polyline length
+// only enters the FP32 mean chord l_i)
+__device__ __forceinline__ double sqrt_fast(double q) {
+    const double y = (double)rsqrtf((float)q);
+    const double r = q * y;
+    return fma(0.5 * y, fma(-r, r, q), r);
+}
+
+// ---- A2 + A3: one thread per history, the MLP sample by sample, rule R9 segment by segment ---------------------
+// A segment A -> B of the polyline is at most ~0.7 voxel widths long (R8: du <= h / 2), so it crosses at most ONE face per
+// axis.  The common path therefore has no loop and no data-dependent branch on the axis: per axis the state d_a in
+// {-1, 0, +1} says whether B lies beyond a face of the current voxel, the (up to three) steps are ordered by their crossing
+// parameters only when a lane really has two or three of them, the voxel and its faces move by predicated updates, and the
+// step codes are pushed in crossing order.  All 32 lanes of a warp (32 histories of equal sample count, neighbours in space)
+// run this path together.  A segment that is longer than a voxel on some axis, steps out of the grid or exceeds the row
+// capacity takes the general loop instead (rule R9 step by step, as the oracle states it) from the same, uncommitted state.
+// Codes go to a staging row per thread and are copied to the code stream once the row's length is known (chunk_counter
+// hands out its place).
 __global__ void __launch_bounds__(128, 4)
 k_mlp_walk(const __grid_constant__ DevCfg g, const HistRec* __restrict__ recs, const uint32_t* __restrict__ order,
-           const uint32_t* __restrict__ list, const unsigned* __restrict__ list_count, const double* __restrict__ logk, int64_t i_base,
-           int count, ulonglong2* __restrict__ stage, ulonglong2* __restrict__ codes, unsigned long long* __restrict__ chunk_counter,
-           uint64_t* __restrict__ code_off, uint32_t* __restrict__ Nout, int32_t* __restrict__ start_out, int32_t* __restrict__ end_out,
-           float* __restrict__ ell_out, uint8_t* __restrict__ flags_out, GenStats* __restrict__ stats) {
+           const double* __restrict__ logk, int64_t i_base, int count, ulonglong2* __restrict__ stage, ulonglong2* __restrict__ codes,
+           unsigned long long* __restrict__ chunk_counter, uint64_t* __restrict__ code_off, uint32_t* __restrict__ Nout,
+           int32_t* __restrict__ start_out, int32_t* __restrict__ end_out, float* __restrict__ ell_out, uint8_t* __restrict__ flags_out,
+           GenStats* __restrict__ stats) {
     const int q = blockIdx.x * blockDim.x + threadIdx.x;
-    const int total = list ? (int)min(*list_count, (unsigned)count) : count;
-    const bool active = q < total;
+    const bool active = q < count;
     unsigned flags = 0;
-    unsigned N = 0, n_samples = 0;
+    unsigned N = 0, n_samples = 0, n_general = 0;
     if (active) {
-        const int p = list ? (int)list[q] : (int)order[count - 1 - q];      // longest first: the CTAs launched last are the cheapest
+        const int p = (int)order[count - 1 - q];      // longest first: the CTAs launched last are the cheapest (short tail)
         const int64_t i = i_base + p;
         const HistRec* rec = recs + p;
         flags = rec->flags;
@@ -347,87 +356,120 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const HistRec* __restrict__ recs, c
             MlpHist H;
             H.load(rec);
             const double cph = rec->cph, sph = rec->sph;
-            const double pout[3] = {rec->pout[0], rec->pout[1], rec->pout[2]};
-            const int vin = rec->vin, vout = rec->vout;
-            // R9-R11 walk state
-            int c[3] = {vin % g.nx, (vin / g.nx) % g.ny, vin / (g.nx * g.ny)};
-            start_v = vin;
+            const int vout = rec->vout;
+            // R9-R11 walk state: current voxel, its faces, the previous vertex
+            int c0 = rec->cin[0], c1 = rec->cin[1], c2 = rec->cin[2];
+            start_v = rec->vin;
             CodeWriter cw;
             cw.init(my_stage);
-            double A[3] = {rec->pin[0], rec->pin[1], rec->pin[2]};
-            double f_lo[3], f_hi[3];
-#pragma unroll
-            for (int a = 0; a < 3; ++a) { f_lo[a] = face_coord(g, a, c[a]); f_hi[a] = face_coord(g, a, c[a] + 1); }
+            double A0 = rec->pin[0], A1 = rec->pin[1], A2 = rec->pin[2];
+            double lo0 = face_coord(g, 0, c0), hi0 = face_coord(g, 0, c0 + 1), lo1 = face_coord(g, 1, c1), hi1 = face_coord(g, 1, c1 + 1),
+                   lo2 = face_coord(g, 2, c2), hi2 = face_coord(g, 2, c2 + 1);
             double L = 0.0;
-            unsigned n_vis = 1;
+            int n_vis = 1;
             bool tie = false, bad = false;
-            for (int k = 1; k <= K && !bad; ++k) {
-                double B[3];
+            for (int k = 1; k <= K; ++k) {
+                double B0, B1, B2;
                 if (k < K) {
                     double w1, tk, vk;
                     mlp_sample(g, H, logk, k, K, w1, tk, vk);
                     const double uk = H.u0 + w1;
-                    B[0] = uk * cph - tk * sph; B[1] = uk * sph + tk * cph; B[2] = vk;
+                    B0 = uk * cph - tk * sph; B1 = uk * sph + tk * cph; B2 = vk;
                 } else {
-                    B[0] = pout[0]; B[1] = pout[1]; B[2] = pout[2];
+                    B0 = rec->pout[0]; B1 = rec->pout[1]; B2 = rec->pout[2];
                 }
-                const double dx = B[0] - A[0], dy = B[1] - A[1], dz = B[2] - A[2];
-                const double seg_len = sqrt(dx * dx + dy * dy + dz * dz);
+                const double e0 = B0 - A0, e1 = B1 - A1, e2 = B2 - A2;
+                const double q2 = fma(e0, e0, fma(e1, e1, e2 * e2));
+                const double seg_len = q2 > 0.0 ? sqrt_fast(q2) : 0.0;
                 L += seg_len;
-                // R9 closed-voxel lazy stepping along A -> B.  The faces of the current voxel are kept in registers; d_a is
-                // the state of axis a (B beyond the high face, beyond the low face, inside) and only the axis that moved is
-                // re-examined.  With one candidate the step needs no arithmetic; with several, the crossing parameters
-                // s_a = num_a / den_a (both positive) are compared by cross-multiplication, s_a < s_b <=> num_a den_b <
-                // num_b den_a, and the tie test (s_a - s_b) |B - A| < eps likewise without a quotient; against the quotient
-                // form this can only change a decision whose crossings coincide to rounding, i.e. a tie, which is flagged.
-                int d0 = B[0] > f_hi[0] ? 1 : (B[0] < f_lo[0] ? -1 : 0);
-                int d1 = B[1] > f_hi[1] ? 1 : (B[1] < f_lo[1] ? -1 : 0);
-                int d2 = B[2] > f_hi[2] ? 1 : (B[2] < f_lo[2] ? -1 : 0);
-                while ((d0 | d1 | d2) != 0) {
-                    // lowest candidate axis with the smallest s (strict comparison: x before y before z on equality)
-                    int best = d0 != 0 ? 0 : (d1 != 0 ? 1 : 2);
-                    if ((d0 != 0) + (d1 != 0) + (d2 != 0) > 1) {
-                        const int dir[3] = {d0, d1, d2};
-                        double num[3], den[3];
+                // state of every axis: B beyond the high face, beyond the low face, inside (closed voxel: a point on a face is inside)
+                const int d0 = B0 > hi0 ? 1 : (B0 < lo0 ? -1 : 0), d1 = B1 > hi1 ? 1 : (B1 < lo1 ? -1 : 0), d2 = B2 > hi2 ? 1 : (B2 < lo2 ? -1 : 0);
+                const int n = (d0 & 1) + (d1 & 1) + (d2 & 1);
+                const int t0 = c0 + d0, t1 = c1 + d1, t2 = c2 + d2;
+                const bool plain = fabs(e0) < g.h && fabs(e1) < g.h && fabs(e2) < g.h &&                       // one face per axis at most
+                                   (unsigned)t0 < (unsigned)g.nx && (unsigned)t1 < (unsigned)g.ny && (unsigned)t2 < (unsigned)g.nz &&
+                                   n_vis + n <= g.max_visits;
+                if (plain) {
+                    int r0 = 0, r1 = 0, r2 = 0;             // place of each axis' step among this segment's steps
+                    if (n >= 2) {
+                        // crossing parameter of axis a: s_a = num_a / den_a, num_a = distance of A from the face, den_a = |B_a - A_a|;
+                        // s_a < s_b <=> num_a den_b < num_b den_a, and the tie test (s_a - s_b) |B - A| < eps likewise without a
+                        // quotient; on equality the lower axis goes first (R9)
+                        const double n0 = fabs((d0 > 0 ? hi0 : lo0) - A0), n1 = fabs((d1 > 0 ? hi1 : lo1) - A1), n2 = fabs((d2 > 0 ? hi2 : lo2) - A2);
+                        const double a0 = fabs(e0), a1 = fabs(e1), a2 = fabs(e2);
+                        const bool p01 = d0 != 0 && d1 != 0, p02 = d0 != 0 && d2 != 0, p12 = d1 != 0 && d2 != 0;
+                        const double l01 = n0 * a1, l10 = n1 * a0, l02 = n0 * a2, l20 = n2 * a0, l12 = n1 * a2, l21 = n2 * a1;
+                        const bool f10 = p01 && l10 < l01, f20 = p02 && l20 < l02, f21 = p12 && l21 < l12;
+                        r0 = (int)f10 + (int)f20;
+                        r1 = (int)(p01 && !f10) + (int)f21;
+                        r2 = (int)(p02 && !f20) + (int)(p12 && !f21);
+                        const double te = g.tie_eps;
+                        if ((p01 && fabs(l01 - l10) * seg_len < te * (a0 * a1)) || (p02 && fabs(l02 - l20) * seg_len < te * (a0 * a2)) ||
+                            (p12 && fabs(l12 - l21) * seg_len < te * (a1 * a2))) tie = true;
+                    }
+                    // codes in crossing order: 0:+x 1:-x 2:+y 3:-y 4:+z 5:-z
+                    const int k0c = d0 < 0 ? 1 : 0, k1c = d1 < 0 ? 3 : 2, k2c = d2 < 0 ? 5 : 4;
+                    if (n >= 1) cw.push((d0 != 0 && r0 == 0) ? k0c : ((d1 != 0 && r1 == 0) ? k1c : k2c));
+                    if (n >= 2) cw.push((d0 != 0 && r0 == 1) ? k0c : ((d1 != 0 && r1 == 1) ? k1c : k2c));
+                    if (n == 3) cw.push(r0 == 2 ? k0c : (r1 == 2 ? k1c : k2c));
+                    // move
+                    if (d0 != 0) { c0 = t0; if (d0 > 0) { lo0 = hi0; hi0 = face_coord(g, 0, t0 + 1); } else { hi0 = lo0; lo0 = face_coord(g, 0, t0); } }
+                    if (d1 != 0) { c1 = t1; if (d1 > 0) { lo1 = hi1; hi1 = face_coord(g, 1, t1 + 1); } else { hi1 = lo1; lo1 = face_coord(g, 1, t1); } }
+                    if (d2 != 0) { c2 = t2; if (d2 > 0) { lo2 = hi2; hi2 = face_coord(g, 2, t2 + 1); } else { hi2 = lo2; lo2 = face_coord(g, 2, t2); } }
+                    n_vis += n;
+                } else {
+                    // the general rule R9: while B is strictly outside the closed voxel, step across the candidate face with the
+                    // smallest crossing parameter
+                    ++n_general;
+                    int c[3] = {c0, c1, c2};
+                    double f_lo[3] = {lo0, lo1, lo2}, f_hi[3] = {hi0, hi1, hi2};
+                    const double A[3] = {A0, A1, A2}, B[3] = {B0, B1, B2};
+                    int dd[3] = {d0, d1, d2};
+                    while ((dd[0] | dd[1] | dd[2]) != 0) {
+                        int best = dd[0] != 0 ? 0 : (dd[1] != 0 ? 1 : 2);
+                        if ((dd[0] != 0) + (dd[1] != 0) + (dd[2] != 0) > 1) {
+                            double num[3], den[3];
 #pragma unroll
-                        for (int a = 0; a < 3; ++a) {
-                            num[a] = fabs((dir[a] > 0 ? f_hi[a] : f_lo[a]) - A[a]);
-                            den[a] = fabs(B[a] - A[a]);
+                            for (int a = 0; a < 3; ++a) {
+                                num[a] = fabs((dd[a] > 0 ? f_hi[a] : f_lo[a]) - A[a]);
+                                den[a] = fabs(B[a] - A[a]);
+                            }
+                            double nb = best == 0 ? num[0] : num[1], db_ = best == 0 ? den[0] : den[1];
+                            if (best == 0 && dd[1] != 0 && num[1] * db_ < nb * den[1]) { best = 1; nb = num[1]; db_ = den[1]; }
+                            if (dd[2] != 0 && num[2] * db_ < nb * den[2]) { best = 2; nb = num[2]; db_ = den[2]; }
+#pragma unroll
+                            for (int a = 0; a < 3; ++a)
+                                if (a != best && dd[a] != 0 && fabs(num[a] * db_ - nb * den[a]) * seg_len < g.tie_eps * (den[a] * db_)) tie = true;
                         }
-                        double nb = best == 0 ? num[0] : num[1], db_ = best == 0 ? den[0] : den[1];
-                        if (best == 0 && d1 != 0 && num[1] * db_ < nb * den[1]) { best = 1; nb = num[1]; db_ = den[1]; }
-                        if (d2 != 0 && num[2] * db_ < nb * den[2]) { best = 2; nb = num[2]; db_ = den[2]; }
+                        const int nn[3] = {g.nx, g.ny, g.nz};
+                        int code = 0;
+                        bool inside = true;
 #pragma unroll
                         for (int a = 0; a < 3; ++a)
-                            if (a != best && dir[a] != 0 && (num[a] * db_ - nb * den[a]) * seg_len < g.tie_eps * (den[a] * db_)) tie = true;
+                            if (a == best) {
+                                c[a] += dd[a];
+                                code = 2 * a + (dd[a] < 0 ? 1 : 0);
+                                inside = (unsigned)c[a] < (unsigned)nn[a];
+                                if (dd[a] > 0) { f_lo[a] = f_hi[a]; f_hi[a] = face_coord(g, a, c[a] + 1); }
+                                else { f_hi[a] = f_lo[a]; f_lo[a] = face_coord(g, a, c[a]); }
+                                dd[a] = B[a] > f_hi[a] ? 1 : (B[a] < f_lo[a] ? -1 : 0);
+                            }
+                        ++n_vis;
+                        if (!inside || n_vis > g.max_visits) { flags = !inside ? PCT_REJ_LEFT_GRID : PCT_REJ_CAPACITY; bad = true; break; }
+                        cw.push(code);
                     }
-                    int code;
-                    bool inside;
-#define PCT_MOVE_AXIS(a, d, n_a)                                                                            \
-                    {                                                                                       \
-                        c[a] += d;                                                                          \
-                        code = 2 * a + (d < 0 ? 1 : 0);                                                     \
-                        inside = (unsigned)c[a] < (unsigned)(n_a);                                          \
-                        if (d > 0) { f_lo[a] = f_hi[a]; f_hi[a] = face_coord(g, a, c[a] + 1); }             \
-                        else { f_hi[a] = f_lo[a]; f_lo[a] = face_coord(g, a, c[a]); }                       \
-                        d = B[a] > f_hi[a] ? 1 : (B[a] < f_lo[a] ? -1 : 0);                                 \
-                    }
-                    if (best == 0) PCT_MOVE_AXIS(0, d0, g.nx)
-                    else if (best == 1) PCT_MOVE_AXIS(1, d1, g.ny)
-                    else PCT_MOVE_AXIS(2, d2, g.nz)
-#undef PCT_MOVE_AXIS
-                    ++n_vis;
-                    if (!inside || n_vis > (unsigned)g.max_visits) { flags = !inside ? PCT_REJ_LEFT_GRID : PCT_REJ_CAPACITY; bad = true; break; }
-                    cw.push(code);
+                    if (bad) break;
+                    c0 = c[0]; c1 = c[1]; c2 = c[2];
+                    lo0 = f_lo[0]; lo1 = f_lo[1]; lo2 = f_lo[2]; hi0 = f_hi[0]; hi1 = f_hi[1]; hi2 = f_hi[2];
                 }
-                A[0] = B[0]; A[1] = B[1]; A[2] = B[2];
+                A0 = B0; A1 = B1; A2 = B2;
             }
             if (bad) break;
             n_chunks = cw.finish();
-            N = n_vis;
+            N = (unsigned)n_vis;
             n_samples = (unsigned)K;
             if (tie) flags |= PCT_TIE;
-            end_v = c[0] + g.nx * (c[1] + g.ny * c[2]);
+            end_v = c0 + g.nx * (c1 + g.ny * c2);
             if (end_v != vout) flags |= PCT_END_MISMATCH;                                                    // R10
             ell = (float)(L / (double)N);                                                                    // R11
         } while (false);
@@ -445,232 +487,28 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const HistRec* __restrict__ recs, c
         ell_out[i] = ell;
         flags_out[i] = (uint8_t)flags;
     }
-    // statistics: one atomic per warp
+    // statistics: one atomic per warp and counter
     const unsigned vis = __reduce_add_sync(0xffffffffu, N);
     const unsigned rej = __reduce_add_sync(0xffffffffu, (active && N == 0) ? 1u : 0u);
     const unsigned tie_n = __reduce_add_sync(0xffffffffu, (flags & PCT_TIE) ? 1u : 0u);
     const unsigned smp = __reduce_add_sync(0xffffffffu, n_samples);
+    const unsigned gen = __reduce_add_sync(0xffffffffu, n_general);
     if ((threadIdx.x & 31) == 0) {
         if (smp) atomicAdd(&stats->total_samples, (unsigned long long)smp);
         if (vis) atomicAdd(&stats->total_visits, (unsigned long long)vis);
         if (rej) atomicAdd(&stats->n_rejected, (unsigned long long)rej);
         if (tie_n) atomicAdd(&stats->n_ties, (unsigned long long)tie_n);
+        if (gen) atomicAdd(&stats->n_general, (unsigned long long)gen);
     }
 }
 
-// ---- A2 + A3, warp-cooperative form: one warp per history, lane = MLP sample -----------------------------------------------
-// PAPER.md:26 maps "each proton [to] an individual thread"; on a 32-wide machine the voxel stepping between the samples
-// then diverges (0-3 steps per sample and lane) and half of the lanes idle.  Here the 32 lanes of a warp take 32
-// CONSECUTIVE SAMPLES of one history:
-//   * lane l evaluates the MLP at depth k = k0 + l (all lanes converged, FP64) and maps the vertex straight to voxel index
-//     coordinates X = (P - lo) / h (one FMA pair per axis from (u, t, v));
-//   * the voxel of an interior vertex is floor(X).  A vertex is handled here only if it lies at least 2e-9 voxel
-//     widths away from every face: then that voxel is the only closed voxel containing it, so it IS the state the
-//     sequential rule R9 reaches there, whatever happened before.  The segment's steps follow from the voxels of its two
-//     ends (shuffle from lane l-1): at most one per axis; two or three are ordered by their crossing parameters with the
-//     same cross-multiplied comparison and tie rule as the sequential form;
-//   * the last segment ends in P_K, which lies exactly on a face of V_e by construction: its steps are decided as R9 states
-//     it, by comparing P_K (mm) with the faces of the voxel the segment starts in;
-//   * a warp scan of the step counts gives every code its place in the row, the codes are collected in shared memory,
-//     packed 21 per word and written to the code stream at a place taken from chunk_counter.
-// Anything else -- a vertex within 2e-9 of a face, a segment that spans more than one voxel, a voxel outside the grid, a
-// row beyond the capacity -- sends the whole history to the sequential kernel (fb_list), which decides it exactly as
-// before.  On the synthetic workloads that is ~1e-6 of the histories.
-constexpr int WK_WARPS = 4;
-// X + FIX_MAGIC has its unit in the last place at 2^-30 for -2^21 <= X < 2^21: the mantissa then holds X as 22.30 fixed
-// point (plus 2^51), i.e. floor(X) and the fractional part of X can be read off the two register halves.
-constexpr double FIX_MAGIC = 6291456.0;                 // 1.5 * 2^22
-constexpr int FIX_FRAC_BITS = 30;
-constexpr unsigned FIX_FRAC_MASK = (1u << FIX_FRAC_BITS) - 1u;
-constexpr unsigned FACE_GUARD = 2u;                     // 2 * 2^-30 ~ 2e-9 voxel widths
-// (hi:lo) >> 30 of a double in [2^22, 2^23) keeps the exponent field (0x415) above the 22 integer bits; subtracting it
-// together with the 2^21 offset of the fixed-point form leaves floor(X)
-constexpr unsigned FIX_INT_BIAS = (0x415u << 22) + (1u << 21);
-
-__device__ __forceinline__ int fix_floor(double s) { return (int)(__funnelshift_r((unsigned)__double2loint(s), (unsigned)__double2hiint(s), FIX_FRAC_BITS) - FIX_INT_BIAS); }
-// true if the fractional part lies within FACE_GUARD units of 0 or 1
-__device__ __forceinline__ bool fix_near_face(double s) {
-    return (((unsigned)__double2loint(s) & FIX_FRAC_MASK) - FACE_GUARD) > FIX_FRAC_MASK - 2u * FACE_GUARD;
-}
-// sqrt(q), q > 0, to ~1e-14 relative: FP32 reciprocal square root as the seed, one Newton step in FP64 (the polyline length
-// only enters the FP32 mean chord l_i)
-__device__ __forceinline__ double sqrt_fast(double q) {
-    const double y = (double)rsqrtf((float)q);
-    const double r = q * y;
-    return fma(0.5 * y, fma(-r, r, q), r);
-}
-
-#ifndef WK_MIN_BLOCKS
-#define WK_MIN_BLOCKS 4
-#endif
-__global__ void __launch_bounds__(WK_WARPS * 32, WK_MIN_BLOCKS)
-k_mlp_walk_warp(const __grid_constant__ DevCfg g, const HistRec* __restrict__ recs, const uint32_t* __restrict__ order,
-                const double* __restrict__ logk, int64_t i_base, int count, int row_cap, ulonglong2* __restrict__ codes,
-                unsigned long long* __restrict__ chunk_counter, uint64_t* __restrict__ code_off, uint32_t* __restrict__ Nout,
-                int32_t* __restrict__ start_out, int32_t* __restrict__ end_out, float* __restrict__ ell_out,
-                uint8_t* __restrict__ flags_out, uint32_t* __restrict__ fb_list, unsigned* __restrict__ fb_count,
-                GenStats* __restrict__ stats) {
-    extern __shared__ unsigned char row_codes[];            // WK_WARPS rows of row_cap bytes: one step code per byte
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const unsigned lt_mask = (1u << lane) - 1u;
-    unsigned char* my_row = row_codes + (size_t)w * row_cap;
-    unsigned long long st_vis = 0, st_smp = 0;
-    unsigned st_rej = 0, st_tie = 0, st_fb = 0;
-    // index coordinates X_a = (P_a - lo_a) / h: faces are the integers
-    const double o0 = -g.lo[0] * g.inv_h, o1 = -g.lo[1] * g.inv_h, o2 = -g.lo[2] * g.inv_h;
-    for (int q = blockIdx.x * WK_WARPS + w; q < count; q += gridDim.x * WK_WARPS) {
-        const int p = (int)order[count - 1 - q];          // longest first
-        const int64_t i = i_base + p;
-        const HistRec* rec = recs + p;
-        const int K = (int)rec->K;
-        unsigned flags = rec->flags;
-        if (K == 0) {
-            if (lane == 0) {
-                code_off[i] = 0ull; Nout[i] = 0u; start_out[i] = -1; end_out[i] = -1; ell_out[i] = 0.f; flags_out[i] = (uint8_t)flags;
-                ++st_rej;
-            }
-            continue;
-        }
-        MlpHist H;
-        H.load(rec);
-        const double cxh = rec->cph * g.inv_h, sxh = rec->sph * g.inv_h;
-        const double b0 = rec->pout[0], b1 = rec->pout[1], b2 = rec->pout[2];
-        const double XO0 = fma(b0, g.inv_h, o0), XO1 = fma(b1, g.inv_h, o1), XO2 = fma(b2, g.inv_h, o2);
-        // carried from round to round: voxel and index coordinates of the vertex before lane 0's
-        int cP0 = rec->cin[0], cP1 = rec->cin[1], cP2 = rec->cin[2];
-        double XP0 = fma(rec->pin[0], g.inv_h, o0), XP1 = fma(rec->pin[1], g.inv_h, o1), XP2 = fma(rec->pin[2], g.inv_h, o2);
-        double Lsum = 0.0;
-        int steps = 0;                                      // codes written so far
-        bool tie = false, give_up = false;
-        int cB0 = 0, cB1 = 0, cB2 = 0;
-        for (int k0 = 1; k0 <= K; k0 += 32) {
-            const int k = k0 + lane;
-            const bool valid = k <= K, last = k == K;
-            // every lane evaluates the MLP (the lanes at and beyond k = K redo sample K - 1; lane k = K then takes P_K, the others idle)
-            double w1, tk, vk;
-            mlp_sample(g, H, logk, min(k, K - 1), K, w1, tk, vk);
-            const double uk = H.u0 + w1;
-            double X0 = fma(uk, cxh, fma(tk, -sxh, o0)), X1 = fma(uk, sxh, fma(tk, cxh, o1)), X2 = fma(vk, g.inv_h, o2);
-            const double s0 = X0 + FIX_MAGIC, s1 = X1 + FIX_MAGIC, s2 = X2 + FIX_MAGIC;
-            cB0 = fix_floor(s0); cB1 = fix_floor(s1); cB2 = fix_floor(s2);
-            bool odd = k < K && (fix_near_face(s0) || fix_near_face(s1) || fix_near_face(s2));   // cannot be decided lane-locally
-            int cA0 = __shfl_up_sync(0xffffffffu, cB0, 1), cA1 = __shfl_up_sync(0xffffffffu, cB1, 1), cA2 = __shfl_up_sync(0xffffffffu, cB2, 1);
-            double XA0 = __shfl_up_sync(0xffffffffu, X0, 1), XA1 = __shfl_up_sync(0xffffffffu, X1, 1), XA2 = __shfl_up_sync(0xffffffffu, X2, 1);
-            if (lane == 0) { cA0 = cP0; cA1 = cP1; cA2 = cP2; XA0 = XP0; XA1 = XP1; XA2 = XP2; }
-            if (last) {
-                // the segment into P_K, which lies exactly on a face of V_e by construction: R9 as stated -- step across the axes
-                // on which P_K (mm) lies strictly outside the closed start voxel
-                X0 = XO0; X1 = XO1; X2 = XO2;
-                cB0 = cA0 + (b0 > face_coord(g, 0, cA0 + 1) ? 1 : (b0 < face_coord(g, 0, cA0) ? -1 : 0));
-                cB1 = cA1 + (b1 > face_coord(g, 1, cA1 + 1) ? 1 : (b1 < face_coord(g, 1, cA1) ? -1 : 0));
-                cB2 = cA2 + (b2 > face_coord(g, 2, cA2 + 1) ? 1 : (b2 < face_coord(g, 2, cA2) ? -1 : 0));
-                odd = b0 > face_coord(g, 0, cB0 + 1) || b0 < face_coord(g, 0, cB0) || b1 > face_coord(g, 1, cB1 + 1) || b1 < face_coord(g, 1, cB1) ||
-                      b2 > face_coord(g, 2, cB2 + 1) || b2 < face_coord(g, 2, cB2);              // more than one voxel away
-            }
-            int d0 = cB0 - cA0, d1 = cB1 - cA1, d2 = cB2 - cA2;
-            if (!valid) { d0 = 0; d1 = 0; d2 = 0; }
-            // a step of more than one voxel on some axis, or a voxel outside the grid: not for this kernel
-            odd = odd || max(max((unsigned)(d0 + 1), (unsigned)(d1 + 1)), (unsigned)(d2 + 1)) > 2u ||
-                  (valid && ((unsigned)cB0 >= (unsigned)g.nx || (unsigned)cB1 >= (unsigned)g.ny || (unsigned)cB2 >= (unsigned)g.nz));
-            if (__any_sync(0xffffffffu, odd)) { give_up = true; break; }
-            const int n = (d0 & 1) + (d1 & 1) + (d2 & 1);
-            // segment length: h |X_B - X_A| (the index map is a rotation scaled by 1/h)
-            const double e0 = X0 - XA0, e1 = X1 - XA1, e2 = X2 - XA2;
-            const double seg_len = valid ? g.h * sqrt_fast(fma(e0, e0, fma(e1, e1, e2 * e2))) : 0.0;
-            Lsum += seg_len;
-            int r0 = 0, r1 = 0, r2 = 0;                     // place of each axis' step among this segment's steps
-            if (n >= 2) {
-                // crossing parameter of axis a: s_a = num_a / den_a, num_a = distance of A from the face, den_a = |B_a - A_a|
-                const double n0 = fabs((double)(cA0 + (d0 > 0 ? 1 : 0)) - XA0), n1 = fabs((double)(cA1 + (d1 > 0 ? 1 : 0)) - XA1),
-                             n2 = fabs((double)(cA2 + (d2 > 0 ? 1 : 0)) - XA2);
-                const double a0 = fabs(e0), a1 = fabs(e1), a2 = fabs(e2);
-                const double l01 = n0 * a1, l10 = n1 * a0, l02 = n0 * a2, l20 = n2 * a0, l12 = n1 * a2, l21 = n2 * a1;
-                const bool p01 = d0 != 0 && d1 != 0, p02 = d0 != 0 && d2 != 0, p12 = d1 != 0 && d2 != 0;
-                // s_a < s_b <=> l_ab < l_ba; on equality the lower axis goes first
-                const bool f10 = p01 && l10 < l01, f20 = p02 && l20 < l02, f21 = p12 && l21 < l12;
-                r0 = (int)f10 + (int)f20;
-                r1 = (int)(p01 && !f10) + (int)f21;
-                r2 = (int)(p02 && !f20) + (int)(p12 && !f21);
-                const double te = g.tie_eps;
-                if ((p01 && fabs(l01 - l10) * seg_len < te * (a0 * a1)) || (p02 && fabs(l02 - l20) * seg_len < te * (a0 * a2)) ||
-                    (p12 && fabs(l12 - l21) * seg_len < te * (a1 * a2))) tie = true;
-            }
-            // places of this lane's codes in the row: prefix sum of n (0..3) over the lanes from two ballots
-            const unsigned m_lo = __ballot_sync(0xffffffffu, n & 1), m_hi = __ballot_sync(0xffffffffu, n & 2);
-            const int total = __popc(m_lo) + 2 * __popc(m_hi);
-            if (steps + total + 1 > g.max_visits) { give_up = true; break; }      // the sequential kernel flags the capacity
-            unsigned char* at = my_row + steps + __popc(m_lo & lt_mask) + 2 * __popc(m_hi & lt_mask);
-            if (d0 != 0) at[r0] = (unsigned char)(d0 < 0 ? 1 : 0);
-            if (d1 != 0) at[r1] = (unsigned char)(d1 < 0 ? 3 : 2);
-            if (d2 != 0) at[r2] = (unsigned char)(d2 < 0 ? 5 : 4);
-            steps += total;
-            cP0 = __shfl_sync(0xffffffffu, cB0, 31); cP1 = __shfl_sync(0xffffffffu, cB1, 31); cP2 = __shfl_sync(0xffffffffu, cB2, 31);
-            XP0 = __shfl_sync(0xffffffffu, X0, 31); XP1 = __shfl_sync(0xffffffffu, X1, 31); XP2 = __shfl_sync(0xffffffffu, X2, 31);
-        }
-        if (give_up) {
-            if (lane == 0) { fb_list[atomicAdd(fb_count, 1u)] = (uint32_t)p; ++st_fb; }
-            continue;
-        }
-        if (__any_sync(0xffffffffu, tie)) flags |= PCT_TIE;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) Lsum += __shfl_xor_sync(0xffffffffu, Lsum, o);
-        const int N = steps + 1;
-        const int src = (K - 1) & 31;                       // lane that held vertex K in the final round
-        const int end_v = __shfl_sync(0xffffffffu, cB0, src) + g.nx * (__shfl_sync(0xffffffffu, cB1, src) + g.ny * __shfl_sync(0xffffffffu, cB2, src));
-        if (end_v != rec->vout) flags |= PCT_END_MISMATCH;                                                   // R10
-        const int n_chunks = (steps + CODES_PER_CHUNK - 1) / CODES_PER_CHUNK;
-        unsigned long long off = 0ull;
-        if (lane == 0 && n_chunks > 0) off = atomicAdd(chunk_counter, (unsigned long long)n_chunks);
-        off = __shfl_sync(0xffffffffu, off, 0);
-        __syncwarp();
-        // pack 21 codes per 64-bit word: four lanes per word (6 + 6 + 6 + 3 codes), OR-combined by two shuffles
-        unsigned long long* out = reinterpret_cast<unsigned long long*>(codes + off);
-        const int part = lane & 3, n_words = 2 * n_chunks;
-        for (int w0 = 0; w0 < n_words; w0 += 8) {
-            const int wd = w0 + (lane >> 2);
-            const int first = wd * CODES_PER_WORD + part * 6;
-            unsigned piece = 0u;
-#pragma unroll
-            for (int j = 0; j < 6; ++j) {
-                const unsigned c = (first + j < steps) ? (unsigned)my_row[first + j] : 7u;
-                if (part * 6 + j < CODES_PER_WORD) piece |= c << (3 * j);
-            }
-            unsigned long long word = (unsigned long long)piece << (18 * part);
-            word |= __shfl_xor_sync(0xffffffffu, word, 1);
-            word |= __shfl_xor_sync(0xffffffffu, word, 2);
-            if (wd * CODES_PER_WORD + CODES_PER_WORD > steps) word |= 1ull << 63;   // bit 63 is no code field; set in partial words like the sequential writer's
-            if (part == 0 && wd < n_words) out[wd] = word;
-        }
-        __syncwarp();
-        if (lane == 0) {
-            code_off[i] = off; Nout[i] = (uint32_t)N; start_out[i] = rec->vin; end_out[i] = end_v;
-            ell_out[i] = (float)(Lsum / (double)N);                                                          // R11
-            flags_out[i] = (uint8_t)(flags & 0xffu);
-            st_vis += (unsigned long long)N; st_smp += (unsigned long long)K; st_tie += (flags & PCT_TIE) ? 1u : 0u;
-        }
-    }
-    if (lane == 0) {
-        if (st_smp) atomicAdd(&stats->total_samples, st_smp);
-        if (st_vis) atomicAdd(&stats->total_visits, st_vis);
-        if (st_rej) atomicAdd(&stats->n_rejected, (unsigned long long)st_rej);
-        if (st_tie) atomicAdd(&stats->n_ties, (unsigned long long)st_tie);
-        if (st_fb) atomicAdd(&stats->n_sequential, (unsigned long long)st_fb);
-    }
-}
-
-static bool k1_sequential() {
-    static const bool v = [] { const char* e = getenv("PCT_K1_SEQUENTIAL"); return e && e[0] == '1'; }();
-    return v;
-}
-
-// One batch of K1: spatial sort -> k_hull -> sort by K -> k_mlp_walk_warp -> k_mlp_walk on the histories it handed over.
-// `stage` holds count rows of stage_chunks chunks (used by the sequential kernel only); the code stream must have room for
-// count * stage_chunks more chunks behind *chunk_counter.
+// One batch of K1: spatial sort -> k_hull -> sort by K -> k_mlp_walk.  `stage` holds count rows of stage_chunks chunks; the
+// code stream must have room for count * stage_chunks more chunks behind *chunk_counter.
 int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, int64_t i_base, int count, ulonglong2* stage,
                      unsigned long long* chunk_counter, pct_paths* P, cudaStream_t st) {
     const int threads = 128;
     const int blocks = (count + threads - 1) / threads;
-    // scratch: history records, sort keys/values (double buffered), fallback list + counter, cub temporary storage
+    // scratch: history records, sort keys/values (double buffered), cub temporary storage
     size_t sort_tmp = 0;
     {
         cub::DoubleBuffer<uint32_t> dk(nullptr, nullptr), dv(nullptr, nullptr);
@@ -679,8 +517,7 @@ int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, in
     auto up = [](size_t v) { return (v + 255) & ~(size_t)255; };
     const size_t arr = up(4 * (size_t)count);
     const size_t o_rec = 0, o_k0 = up(sizeof(HistRec) * (size_t)count), o_k1 = o_k0 + arr, o_v0 = o_k1 + arr, o_v1 = o_v0 + arr,
-                 o_k2 = o_v1 + arr, o_k3 = o_k2 + arr, o_v2 = o_k3 + arr, o_v3 = o_v2 + arr, o_fb = o_v3 + arr, o_fbc = o_fb + arr,
-                 o_tmp = o_fbc + 256, total = o_tmp + up(sort_tmp);
+                 o_k2 = o_v1 + arr, o_k3 = o_k2 + arr, o_v2 = o_k3 + arr, o_v3 = o_v2 + arr, o_tmp = o_v3 + arr, total = o_tmp + up(sort_tmp);
     if (total > ctx->gen_scratch_bytes) {
         if (ctx->gen_scratch) PCT_CUDA(ctx, cudaFree(ctx->gen_scratch));
         ctx->gen_scratch = nullptr; ctx->gen_scratch_bytes = 0;
@@ -689,12 +526,9 @@ int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, in
     }
     char* base = (char*)ctx->gen_scratch;
     HistRec* recs = (HistRec*)(base + o_rec);
-    uint32_t* fb_list = (uint32_t*)(base + o_fb);
-    unsigned* fb_count = (unsigned*)(base + o_fbc);
     cub::DoubleBuffer<uint32_t> dk((uint32_t*)(base + o_k0), (uint32_t*)(base + o_k1)), dv((uint32_t*)(base + o_v0), (uint32_t*)(base + o_v1));
     cub::DoubleBuffer<uint32_t> sk((uint32_t*)(base + o_k2), (uint32_t*)(base + o_k3)), sv((uint32_t*)(base + o_v2), (uint32_t*)(base + o_v3));
     ProfScope prof(ctx, 0, st);
-    PCT_CUDA(ctx, cudaMemsetAsync(fb_count, 0, sizeof(unsigned), st));
     {   // spatial order of the batch: 2 mm cells of the entry tracker plane
         const DevCfg& c = ctx->cfg;
         const double ex = fmax(fabs(c.lo[0]), fabs(c.hi[0])), ey = fmax(fabs(c.lo[1]), fabs(c.hi[1]));
@@ -709,24 +543,9 @@ int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, in
     int key_bits = 1;
     while ((1 << key_bits) < ctx->logk_n) ++key_bits;                  // K < logk_n
     PCT_CUDA(ctx, cub::DeviceRadixSort::SortPairs(base + o_tmp, sort_tmp, dk, dv, count, 0, key_bits, st));
-    ctx->launches += 4;
-    const uint32_t* order = dv.Current();
-    if (!k1_sequential()) {
-        const int row_cap = (ctx->cfg.max_visits + 15) & ~15;
-        const size_t smem = (size_t)WK_WARPS * (size_t)row_cap;
-        const int want = (count + WK_WARPS - 1) / WK_WARPS, cap = ctx->num_sms * 16;
-        k_mlp_walk_warp<<<want < cap ? want : cap, WK_WARPS * 32, smem, st>>>(ctx->cfg, recs, order, ctx->logk, i_base, count, row_cap, P->codes,
-                                                                             chunk_counter, P->code_off, P->N, P->start, P->end, P->ell, P->flags,
-                                                                             fb_list, fb_count, ctx->d_stats);
-        // the histories the warp kernel handed over (normally a handful; the grid covers the worst case and exits at once)
-        k_mlp_walk<<<blocks, threads, 0, st>>>(ctx->cfg, recs, order, fb_list, fb_count, ctx->logk, i_base, count, stage, P->codes, chunk_counter,
-                                               P->code_off, P->N, P->start, P->end, P->ell, P->flags, ctx->d_stats);
-        ctx->launches += 2;
-    } else {
-        k_mlp_walk<<<blocks, threads, 0, st>>>(ctx->cfg, recs, order, nullptr, nullptr, ctx->logk, i_base, count, stage, P->codes, chunk_counter,
-                                               P->code_off, P->N, P->start, P->end, P->ell, P->flags, ctx->d_stats);
-        ++ctx->launches;
-    }
+    k_mlp_walk<<<blocks, threads, 0, st>>>(ctx->cfg, recs, dv.Current(), ctx->logk, i_base, count, stage, P->codes, chunk_counter,
+                                           P->code_off, P->N, P->start, P->end, P->ell, P->flags, ctx->d_stats);
+    ctx->launches += 5;
     PCT_CUDA(ctx, cudaGetLastError());
     return PCT_OK;
 }

@@ -332,7 +332,7 @@ int pct_generate_mlp(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hull, v
     GEN_CUDA(cache_alloc((void**)&P->flags, sizeof(uint8_t) * mm));
     GEN_CUDA(cache_alloc((void**)&P->code_off, sizeof(uint64_t) * mm));
     const int batch_max = (int)(m < GEN_BATCH ? (m > 0 ? m : 1) : GEN_BATCH);
-    // rows of the sequential walk kernel (the histories the warp kernel hands over; all of them with PCT_K1_SEQUENTIAL=1)
+    // staging rows of the walk kernel (a row's place in the code stream is known only when its length is)
     GEN_CUDA(cache_alloc((void**)&stage, sizeof(ulonglong2) * (size_t)batch_max * (size_t)ctx->cfg.stage_chunks));
     GEN_CUDA(cudaMemsetAsync(ctx->d_stats, 0, sizeof(GenStats), st));
     // rows are appended to the code stream at places handed out by a device counter (chunks), read back after every batch
@@ -361,7 +361,7 @@ int pct_generate_mlp(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hull, v
     GEN_CUDA(cudaStreamSynchronize(st));
 #undef GEN_CUDA
     cache_free(stage);
-    P->total_visits = (int64_t)hs.total_visits; P->n_rejected = (int64_t)hs.n_rejected; P->total_samples = (int64_t)hs.total_samples; P->n_ties = (int64_t)hs.n_ties; P->n_sequential = (int64_t)hs.n_sequential;
+    P->total_visits = (int64_t)hs.total_visits; P->n_rejected = (int64_t)hs.n_rejected; P->total_samples = (int64_t)hs.total_samples; P->n_ties = (int64_t)hs.n_ties; P->n_general = (int64_t)hs.n_general;
     *out = P;
     return PCT_OK;
 }
@@ -391,7 +391,7 @@ int pct_plan_info(const pct_paths* P, pct_plan_stats* out) {
 int pct_paths_info(const pct_paths* P, pct_paths_stats* out) {
     if (!P || !out) return PCT_E_INVALID_ARG;
     out->m = P->m; out->total_visits = P->total_visits; out->n_rejected = P->n_rejected; out->n_ties = P->n_ties;
-    out->total_samples = P->total_samples; out->n_sequential = P->n_sequential;
+    out->total_samples = P->total_samples; out->n_general_segments = P->n_general;
     out->code_bytes = P->chunks_used * (int64_t)sizeof(ulonglong2);
     out->header_bytes = P->m * (int64_t)(sizeof(uint32_t) + 2 * sizeof(int32_t) + sizeof(float) + sizeof(uint8_t) + sizeof(uint64_t));
     return PCT_OK;

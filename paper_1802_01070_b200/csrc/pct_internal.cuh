@@ -37,7 +37,7 @@ struct ProtonPtrs {
     const double *phi, *t_in, *v_in, *dt_in, *dv_in, *t_out, *v_out, *dt_out, *dv_out;
 };
 
-struct GenStats { unsigned long long total_visits, n_rejected, n_ties, total_samples, n_sequential; };
+struct GenStats { unsigned long long total_visits, n_rejected, n_ties, total_samples, n_general; };
 
 // ---- solve plan: a block's histories regrouped into spatially compact tubes ----------------------
 // A group = up to GROUP histories of one block that travel the same way (class = major axis and direction) and lie
@@ -158,7 +158,7 @@ struct pct_paths {
     uint64_t* code_off;  // first 16-byte chunk of the row in `codes`
     ulonglong2* codes;
     int64_t chunks_used, chunks_cap;
-    int64_t total_visits, n_rejected, n_ties, total_samples, n_sequential;
+    int64_t total_visits, n_rejected, n_ties, total_samples, n_general;
     pct::SolvePlan* plan; // cached by pct_solve for (this, block_size); owned by the paths object
 };
 

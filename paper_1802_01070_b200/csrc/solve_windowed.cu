@@ -107,6 +107,43 @@ __device__ __forceinline__ void walk_slab(const unsigned long long* __restrict__
     }
 }
 
+// One history's row walked with red.global.add.f32 of `c` on every visit (the "late" members of k_block_windowed: outliers
+// and non-finite residuals, R21).  acc[v * stride] is the Delta accumulator of voxel v.
+__device__ __noinline__ void late_walk(int sx, int sy, int sz, const ulonglong2* __restrict__ codes, uint64_t off, int32_t v, uint32_t n_vis,
+                                       float c, float* __restrict__ acc, int stride) {
+    const unsigned long long* cp = reinterpret_cast<const unsigned long long*>(codes + off);
+    unsigned long long w = 0ull;
+    for (uint32_t k = 0; k < n_vis; ++k) {
+        if (k > 0) {
+            const uint32_t f = (k - 1) % CODES_PER_WORD;
+            if (f == 0) w = __ldg(cp++);
+            const int code = (int)((w >> (3 * f)) & 7ull);
+            const int mag = (code >> 1) == 0 ? sx : ((code >> 1) == 1 ? sy : sz);
+            v += (code & 1) ? -mag : mag;
+        }
+        red_add_f32(acc + (size_t)v * stride, c);
+    }
+}
+
+// Median binade of the finite |c_i| of a CTA from the exponent histogram (256 bins); -1 if there is none.  One warp.
+__device__ __noinline__ int median_binade(const unsigned* ehist, int lane) {
+    unsigned mine = 0u;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) mine += ehist[lane * 8 + k];
+    unsigned incl = mine;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const unsigned y = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += y; }
+    const unsigned total = __shfl_sync(0xffffffffu, incl, 31), half = (total + 1u) >> 1;
+    const unsigned at = __ballot_sync(0xffffffffu, incl >= half && total > 0u);
+    int bin = -1;
+    if (total > 0u && lane == __ffs(at) - 1) {
+        unsigned cum = incl - mine;
+        bin = lane * 8;
+        for (int k = 0; k < 8; ++k) { cum += ehist[lane * 8 + k]; if (cum >= half) { bin = lane * 8 + k; break; } }
+    }
+    return __reduce_max_sync(0xffffffffu, bin);
+}
+
 // COUNT = true: fused column counts, {Delta_j, s_j} go to the float2 accumulator `ds` (first sweep over a block, or no
 // count cache).  COUNT = false: s_j^t is already cached per block (it does not depend on x, R15), only Delta_j is
 // accumulated, into `dsum`; the freed half of the window holds a second copy of Delta (odd / even lanes) to halve the
@@ -222,23 +259,7 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
     int* dl = reinterpret_cast<int*>(win);
 #pragma unroll
     for (int k = 0; k < 2 * WIN_SLOTS / GROUP; ++k) dl[tid + k * GROUP] = 0;      // clears Delta and s
-    if (tid < 32) {                               // median binade: lane l owns bins 8l .. 8l+7
-        unsigned mine = 0u;
-#pragma unroll
-        for (int k = 0; k < 8; ++k) mine += ehist[tid * 8 + k];
-        unsigned incl = mine;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { const unsigned y = __shfl_up_sync(0xffffffffu, incl, o); if (tid >= o) incl += y; }
-        const unsigned total = __shfl_sync(0xffffffffu, incl, 31), half = (total + 1u) >> 1;
-        const unsigned at = __ballot_sync(0xffffffffu, incl >= half && total > 0u);
-        if (total == 0u) { if (tid == 0) e_med = -1; }
-        else if (tid == __ffs(at) - 1) {
-            unsigned cum = incl - mine;
-            int bin = tid * 8;
-            for (int k = 0; k < 8; ++k) { cum += ehist[tid * 8 + k]; if (cum >= half) { bin = tid * 8 + k; break; } }
-            e_med = bin;
-        }
-    }
+    if (tid < 32) { const int m = median_binade(ehist, tid); if (tid == 0) e_med = m; }
     __syncthreads();
     mx = red[0];
 #pragma unroll
@@ -254,6 +275,9 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
     unsigned my_max = 0u;
     const int cfix = late ? 0 : __float2int_rn(ci * scale);
 
+    // a late member's Delta contributions go straight to the global accumulator (its visits are counted in the window by
+    // pass 2); done before pass 2, out of line, so that nothing of it stays live across the hot loop
+    if (late) late_walk(g.sx, g.sy, g.sz, codes, code_off[i], start[i], n_vis, ci, COUNT ? &ds[0].x : dsum, COUNT ? 2 : 1);
     // ---- pass 2: {Delta, s} += {c_i, 1} on every visit; flush per slab -------------------------------------------------
     p = win_s + p_init + (COUNT ? 0u : (unsigned)(tid & 1) * (WIN_SLOTS * 4));     // odd lanes: second Delta copy
     w_next = __ldg(my_stream);
@@ -294,22 +318,6 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
             });
         }
         __syncthreads();
-    }
-    if (late) {
-        // this member's Delta contributions go straight to the global accumulator (its visits were counted in the window)
-        const unsigned long long* cp = reinterpret_cast<const unsigned long long*>(codes + code_off[i]);
-        int v = start[i];
-        unsigned long long w = 0ull;
-        for (uint32_t k = 0; k < n_vis; ++k) {
-            if (k > 0) {
-                const uint32_t f = (k - 1) % CODES_PER_WORD;
-                if (f == 0) w = __ldg(cp++);
-                const int code = (int)((w >> (3 * f)) & 7ull);
-                const int mag = (code >> 1) == 0 ? g.sx : ((code >> 1) == 1 ? g.sy : g.sz);
-                v += (code & 1) ? -mag : mag;
-            }
-            red_add_f32(COUNT ? &ds[v].x : dsum + v, ci);
-        }
     }
     if (COUNT) {        // remember the largest slot count for the sweeps that reuse the cached counts
         my_max = __reduce_max_sync(0xffffffffu, my_max);

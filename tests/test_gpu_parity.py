@@ -213,9 +213,8 @@ def test_full_size_sampled(binding, oracle, name):
     pr = synth.generate_protons(cfg, x_true, shadow, device="cuda")
     ctx, paths = gpu_paths(binding, cfg, pr, hull)
     assert paths.m == m and paths.n_rejected < 0.12 * m      # cone beam: ~9 % of the field passes beside the object
-    # K1's bulk kernel (one warp per history) must have done the work: the sequential kernel only takes the rows it cannot decide
-    # (parallel beam at the four axis-aligned gantry angles: every second vertex lies exactly on a voxel face -> sequential)
-    assert paths.n_sequential <= (0.03 if cfg.beam == "parallel90" else 1e-4) * m + 10, paths.n_sequential
+    # K1's loop-free path must have done the work: the general stepping loop only takes the odd segments
+    assert paths.n_general_segments <= 1e-6 * paths.total_samples + 10, paths.n_general_segments
     rng = np.random.default_rng(0)
     starts = np.sort(rng.integers(0, m - 400, 24))
     total_mis = 0
