@@ -78,9 +78,10 @@ typedef struct {
     double ds_mm;
     int32_t min_count; /* bins with fewer histories count as empty (0) */
 } pcto_fbp_params;
-/* FBP image from tracker records + WEPL.  sino_mean: [nz][n_theta][n_s] mean WEPL per bin, or NULL. */
+/* FBP image from tracker records + WEPL.  sino_mean / sino_filtered: [nz][n_theta][n_s] mean WEPL per bin and
+ * its ramp-filtered rows, or NULL. */
 int pcto_fbp(const pcto_geometry*, const pcto_protons*, const float* b, const pcto_fbp_params*, double* sino_mean,
-             double* x0_out);
+             double* sino_filtered, double* x0_out);
 /* Hull by space carving: voxels crossed (chord > min_chord_mm) by a history with WEPL < wepl_air_mm become 0, all others 1 */
 int pcto_hull_carve(const pcto_geometry*, const pcto_protons*, const float* b, double wepl_air_mm, double min_chord_mm,
                     uint8_t* hull_out);

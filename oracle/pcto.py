@@ -81,7 +81,7 @@ def lib():
         L.pcto_solve_ex.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int64, C.c_double,
                                     C.c_double, C.c_double, C.c_void_p, C.c_void_p, C.c_int]
         L.pcto_fbp.argtypes = [C.POINTER(Geometry), C.POINTER(Protons), C.c_void_p, C.POINTER(FbpParams), C.c_void_p,
-                               C.c_void_p]
+                               C.c_void_p, C.c_void_p]
         L.pcto_hull_carve.argtypes = [C.POINTER(Geometry), C.POINTER(Protons), C.c_void_p, C.c_double, C.c_double,
                                       C.c_void_p]
         _lib = L
@@ -226,16 +226,19 @@ def walk_polyline(geom: Geometry, verts: np.ndarray, start_voxel: int, tie_eps_m
 
 def fbp(geom: Geometry, protons: ProtonArrays, b, n_theta: int, n_s: int, ds_mm: float, min_count: int = 1,
         want_sinogram: bool = False):
-    """R25: FBP image float64[nz, ny, nx] (and the mean-WEPL sinogram [nz, n_theta, n_s] if asked for)."""
+    """R25: FBP image float64[nz, ny, nx]; with want_sinogram also the mean-WEPL sinogram and its ramp-filtered rows,
+    both [nz, n_theta, n_s]."""
     b = np.ascontiguousarray(b, dtype=np.float32).reshape(-1)
     assert b.size == protons.m
     fp = FbpParams(int(n_theta), int(n_s), float(ds_mm), int(min_count))
     x0 = np.zeros(geom.nx * geom.ny * geom.nz, dtype=np.float64)
     sino = np.zeros((geom.nz, n_theta, n_s), dtype=np.float64) if want_sinogram else None
+    filt = np.zeros((geom.nz, n_theta, n_s), dtype=np.float64) if want_sinogram else None
     assert lib().pcto_fbp(C.byref(geom), C.byref(protons.c), b.ctypes.data, C.byref(fp),
-                          sino.ctypes.data if want_sinogram else None, x0.ctypes.data) == 0
+                          sino.ctypes.data if want_sinogram else None, filt.ctypes.data if want_sinogram else None,
+                          x0.ctypes.data) == 0
     x0 = x0.reshape(geom.nz, geom.ny, geom.nx)
-    return (x0, sino) if want_sinogram else x0
+    return (x0, sino, filt) if want_sinogram else x0
 
 
 def hull_carve(geom: Geometry, protons: ProtonArrays, b, wepl_air_mm: float, min_chord_mm: float) -> np.ndarray:

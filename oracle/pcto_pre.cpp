@@ -39,7 +39,7 @@ extern "C" {
 // s = -x sin(theta_c) + y cos(theta_c), theta_c the bin centre (full 2 pi of directions, hence pi / n_theta and not
 // 2 pi / n_theta).
 int pcto_fbp(const pcto_geometry* g, const pcto_protons* pr, const float* b, const pcto_fbp_params* fp,
-             double* sino_mean /* [nz][n_theta][n_s] or NULL */, double* x0_out /* [n] */) {
+             double* sino_mean /* [nz][n_theta][n_s] or NULL */, double* sino_filtered /* same shape or NULL */, double* x0_out /* [n] */) {
     if (!g || !pr || !b || !fp || !x0_out || fp->n_theta < 1 || fp->n_s < 2 || !(fp->ds_mm > 0.0) || g->nx <= 0 || g->ny <= 0 ||
         g->nz <= 0 || !(g->h_mm > 0.0)) return -1;
     const int nt = fp->n_theta, ns = fp->n_s, nz = g->nz;
@@ -85,6 +85,7 @@ int pcto_fbp(const pcto_geometry* g, const pcto_protons* pr, const float* b, con
             qr[j] = ds * acc;
         }
     }
+    if (sino_filtered) std::memcpy(sino_filtered, q.data(), sizeof(double) * cells);
     // voxel-driven back projection
     for (int iz = 0; iz < nz; ++iz)
         for (int iy = 0; iy < g->ny; ++iy)
