@@ -126,6 +126,40 @@ int pct_column_counts(pct_ctx* ctx, const pct_paths* paths, int64_t i0, int64_t 
 int pct_solve(pct_ctx* ctx, const pct_paths* paths, const float* b, const float* x0, int iters, int64_t block_size,
               float lambda, float* x_out, void* stream);
 
+/* A5-A8 with the options of ref [9]-style solvers ("standard iterative solver [9]"; reading R27):
+ *   x <- clamp( x + lambda * diag(1/max(1,s_j^t)) * sum_{i in block t} w_i [(b_i - <a_i,x>)/||a_i||^2] a_i )
+ * weights: DEVICE float32[m] in [0, 1] or NULL (= all one); the clamp x_j <- min(max(x_j, clamp_lo), clamp_hi) is applied
+ * to the voxels a block updates, right after its update; clamp_lo > clamp_hi = no clamp.  opts == NULL = pct_solve. */
+typedef struct {
+    const float* weights;
+    float clamp_lo, clamp_hi;
+} pct_solve_opts;
+int pct_solve_ex(pct_ctx* ctx, const pct_paths* paths, const float* b, const float* x0, int iters, int64_t block_size,
+                 float lambda, const pct_solve_opts* opts /* HOST */, float* x_out, void* stream);
+
+/* The FBP image the solver starts from ("Using the FBP image as the initial iterate"; reading R25): every
+ * history is taken as the straight chord between its tracker hits and rebinned to parallel projections (direction
+ * theta = phi + alpha, signed distance s from the rotation axis, height z = mean of the two hits); bins: n_theta sectors
+ * of [0, 2 pi), n_s bins of ds_mm centred on the axis, one per slice; bin value = mean WEPL (0 below min_count histories);
+ * rows filtered with the band-limited ramp (Ram-Lak) kernel by direct convolution; voxel-driven back projection with linear
+ * interpolation, x0 = (pi / n_theta) * sum over directions.  FP64 inside, float32 out.
+ * protons: HOST struct of DEVICE arrays; b: DEVICE float32[m]; x0_out: DEVICE float32[n].  Synchronises `stream` (its
+ * sinogram scratch goes back to the buffer cache). */
+typedef struct {
+    int32_t n_theta, n_s;
+    double ds_mm;
+    int32_t min_count;
+} pct_fbp_params;
+int pct_fbp(pct_ctx* ctx, const pct_protons* protons, const float* b, const pct_fbp_params* params /* HOST */, float* x0_out,
+            void* stream);
+
+/* The object hull from the data (space carving; preprocessing of PAPER.md:102-104; reading R26): hull_out[j] = 0 for every
+ * voxel that the straight chord between the tracker hits of some history with WEPL < wepl_air_mm crosses with a chord
+ * length > min_chord_mm, 1 otherwise.  hull_out: DEVICE uint8[n] (overwritten).  Use min_chord_mm > 0: voxels a chord only
+ * grazes at a corner are decided by rounding otherwise.  Enqueued on `stream`. */
+int pct_hull_carve(pct_ctx* ctx, const pct_protons* protons, const float* b, double wepl_air_mm, double min_chord_mm,
+                   uint8_t* hull_out, void* stream);
+
 /* The whole hot path on HOST buffers (bench e2e): H2D of the tracker arrays, hull and b; pct_generate_mlp;
  * pct_solve; D2H of x.  protons: HOST struct with HOST arrays; hull_host: uint8[n] or NULL; b_host: float32[m];
  * x0_host: float32[n] or NULL (= all ones); x_out_host: float32[n]; stats may be NULL.  Blocking. */
@@ -161,8 +195,8 @@ int pct_plan_info(const pct_paths* paths, pct_plan_stats* out /* HOST */);
  * of the hot kernels with CUDA events on the launching stream; pct_profile_read synchronises the device,
  * ADDS the elapsed times since the last read to out (HOST) and clears the event list.  kind: 0 = MLP + walk (K1),
  * 1 = windowed block projection (K2w), 2 = voxel update (K3), 3 = direct block projection (K2d),
- * 4 = solve-plan construction (sort, grouping, verification). */
-#define PCT_PROFILE_KINDS 5
+ * 4 = solve-plan construction (sort, grouping, verification), 5 = preprocessing (pct_fbp, pct_hull_carve). */
+#define PCT_PROFILE_KINDS 6
 typedef struct {
     double ms[PCT_PROFILE_KINDS];
     int64_t launches[PCT_PROFILE_KINDS];

@@ -21,7 +21,7 @@ REJECT_MASK = REJ_MISS | REJ_ORDER | REJ_DEPTH | REJ_LEFT_GRID | REJ_CAPACITY | 
 EXPORTS = ("pct_create", "pct_destroy", "pct_last_error", "pct_generate_mlp", "pct_paths_info", "pct_paths_free",
            "pct_paths_decode", "pct_forward_project", "pct_column_counts", "pct_solve", "pct_reconstruct_host",
            "pct_launch_count", "pct_profile_enable", "pct_profile_read", "pct_measure_peaks", "pct_solve_config",
-           "pct_plan_info", "pct_trim_cache", "pct_paths_flagged")
+           "pct_plan_info", "pct_trim_cache", "pct_paths_flagged", "pct_solve_ex", "pct_fbp", "pct_hull_carve")
 
 
 class Geometry(C.Structure):
@@ -51,7 +51,7 @@ class ReconStats(C.Structure):
         (k, C.c_double) for k in ("ms_h2d", "ms_mlp", "ms_solve", "ms_d2h")]
 
 
-PROFILE_KINDS = ("mlp", "project_windowed", "update", "project_direct", "plan")
+PROFILE_KINDS = ("mlp", "project_windowed", "update", "project_direct", "plan", "pre")
 
 
 class Profile(C.Structure):
@@ -61,6 +61,14 @@ class Profile(C.Structure):
 class PlanStats(C.Structure):
     _fields_ = [(k, C.c_int64) for k in ("block_size", "n_blocks", "n_groups", "n_direct", "plan_bytes", "stream_bytes",
                                           "cnt_bytes", "staged_slots", "windowed_histories", "windowed_visits")]
+
+
+class SolveOpts(C.Structure):
+    _fields_ = [("weights", C.c_void_p), ("clamp_lo", C.c_float), ("clamp_hi", C.c_float)]
+
+
+class FbpParams(C.Structure):
+    _fields_ = [("n_theta", C.c_int32), ("n_s", C.c_int32), ("ds_mm", C.c_double), ("min_count", C.c_int32)]
 
 
 class Peaks(C.Structure):
@@ -102,6 +110,9 @@ def load_library(path: Optional[str] = None):
     L.pct_forward_project.argtypes = [vp, vp, vp, vp, vp]
     L.pct_column_counts.argtypes = [vp, vp, i64, i64, vp, vp]
     L.pct_solve.argtypes = [vp, vp, vp, vp, C.c_int, i64, C.c_float, vp, vp]
+    L.pct_solve_ex.argtypes = [vp, vp, vp, vp, C.c_int, i64, C.c_float, C.POINTER(SolveOpts), vp, vp]
+    L.pct_fbp.argtypes = [vp, C.POINTER(Protons), vp, C.POINTER(FbpParams), vp, vp]
+    L.pct_hull_carve.argtypes = [vp, C.POINTER(Protons), vp, C.c_double, C.c_double, vp, vp]
     L.pct_reconstruct_host.argtypes = [vp, C.POINTER(Protons), vp, vp, vp, C.c_int, i64, C.c_float, vp,
                                        C.POINTER(ReconStats), vp]
     L.pct_launch_count.argtypes = [vp]
@@ -277,13 +288,45 @@ class Context:
         return c
 
     def solve(self, paths: Paths, b: torch.Tensor, x0: torch.Tensor, iters: int, block_size: int, lam: float,
-              out: Optional[torch.Tensor] = None) -> torch.Tensor:
+              out: Optional[torch.Tensor] = None, weights: Optional[torch.Tensor] = None,
+              clamp: Optional[tuple] = None) -> torch.Tensor:
+        """pct_solve; with weights (float32[m] on the device) and / or clamp = (lo, hi): pct_solve_ex (R27)."""
         x = out if out is not None else torch.empty(self.n, dtype=torch.float32, device=self.device)
-        self._check(self._L.pct_solve(self._h, paths._h, _dev_ptr(b, torch.float32, paths.m, self.device),
-                                      _dev_ptr(x0, torch.float32, self.n, self.device), int(iters), int(block_size),
-                                      float(lam), _dev_ptr(x, torch.float32, self.n, self.device),
-                                      _stream_ptr(self.device)))
+        args = (self._h, paths._h, _dev_ptr(b, torch.float32, paths.m, self.device),
+                _dev_ptr(x0, torch.float32, self.n, self.device), int(iters), int(block_size), float(lam))
+        tail = (_dev_ptr(x, torch.float32, self.n, self.device), _stream_ptr(self.device))
+        if weights is None and clamp is None:
+            self._check(self._L.pct_solve(*args, *tail))
+        else:
+            lo, hi = clamp if clamp is not None else (1.0, 0.0)
+            opts = SolveOpts(_dev_ptr(weights, torch.float32, paths.m, self.device), float(lo), float(hi))
+            self._check(self._L.pct_solve_ex(*args, C.byref(opts), *tail))
         return x
+
+    def _protons_struct(self, protons: Dict[str, torch.Tensor], u_in_mm: float, u_out_mm: float) -> Protons:
+        m = int(protons["phi"].numel())
+        return Protons(m, *[_dev_ptr(protons[k], torch.float64, m, self.device) for k in PROTON_KEYS], float(u_in_mm),
+                       float(u_out_mm))
+
+    def fbp(self, protons: Dict[str, torch.Tensor], u_in_mm: float, u_out_mm: float, b: torch.Tensor, n_theta: int,
+            n_s: int, ds_mm: float, min_count: int = 1, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+        """pct_fbp (R25): the FBP initial iterate, float32[n] on the device."""
+        pr = self._protons_struct(protons, u_in_mm, u_out_mm)
+        x0 = out if out is not None else torch.empty(self.n, dtype=torch.float32, device=self.device)
+        fp = FbpParams(int(n_theta), int(n_s), float(ds_mm), int(min_count))
+        self._check(self._L.pct_fbp(self._h, C.byref(pr), _dev_ptr(b, torch.float32, pr.m, self.device), C.byref(fp),
+                                    _dev_ptr(x0, torch.float32, self.n, self.device), _stream_ptr(self.device)))
+        return x0
+
+    def hull_carve(self, protons: Dict[str, torch.Tensor], u_in_mm: float, u_out_mm: float, b: torch.Tensor,
+                   wepl_air_mm: float, min_chord_mm: float, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+        """pct_hull_carve (R26): uint8[n] hull mask on the device."""
+        pr = self._protons_struct(protons, u_in_mm, u_out_mm)
+        hull = out if out is not None else torch.empty(self.n, dtype=torch.uint8, device=self.device)
+        self._check(self._L.pct_hull_carve(self._h, C.byref(pr), _dev_ptr(b, torch.float32, pr.m, self.device),
+                                           float(wepl_air_mm), float(min_chord_mm),
+                                           _dev_ptr(hull, torch.uint8, self.n, self.device), _stream_ptr(self.device)))
+        return hull
 
     def reconstruct_host(self, protons: Dict[str, torch.Tensor], u_in_mm: float, u_out_mm: float,
                          hull: Optional[torch.Tensor], b: torch.Tensor, x0: Optional[torch.Tensor], iters: int,

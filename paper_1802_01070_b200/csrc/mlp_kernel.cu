@@ -329,7 +329,7 @@ __device__ __forceinline__ double sqrt_fast(double q) {
 // parameters only when a lane really has two or three of them, the voxel and its faces move by predicated updates, and the
 // step codes are pushed in crossing order.  All 32 lanes of a warp (32 histories of equal sample count, neighbours in space)
 // run this path together.  A segment that is longer than a voxel on some axis, steps out of the grid or exceeds the row
-// capacity takes the general loop instead (rule R9 step by step, as the oracle states it) from the same, uncommitted state.
+// capacity takes the general loop instead (rule R9 step by step, as DESIGN.md states it) from the same, uncommitted state.
 // Codes go to a staging row per thread and are copied to the code stream once the row's length is known (chunk_counter
 // hands out its place).
 __global__ void __launch_bounds__(128, 4)
@@ -390,7 +390,7 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const HistRec* __restrict__ recs, c
                                    (unsigned)t0 < (unsigned)g.nx && (unsigned)t1 < (unsigned)g.ny && (unsigned)t2 < (unsigned)g.nz &&
                                    n_vis + n <= g.max_visits;
                 if (plain) {
-                    int r0 = 0, r1 = 0, r2 = 0;             // place of each axis' step among this segment's steps
+                    int r0 = 0, r1 = 0;                     // place of the x / y step among this segment's steps (z takes what is left)
                     if (n >= 2) {
                         // crossing parameter of axis a: s_a = num_a / den_a, num_a = distance of A from the face, den_a = |B_a - A_a|;
                         // s_a < s_b <=> num_a den_b < num_b den_a, and the tie test (s_a - s_b) |B - A| < eps likewise without a
@@ -402,7 +402,6 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const HistRec* __restrict__ recs, c
                         const bool f10 = p01 && l10 < l01, f20 = p02 && l20 < l02, f21 = p12 && l21 < l12;
                         r0 = (int)f10 + (int)f20;
                         r1 = (int)(p01 && !f10) + (int)f21;
-                        r2 = (int)(p02 && !f20) + (int)(p12 && !f21);
                         const double te = g.tie_eps;
                         if ((p01 && fabs(l01 - l10) * seg_len < te * (a0 * a1)) || (p02 && fabs(l02 - l20) * seg_len < te * (a0 * a2)) ||
                             (p12 && fabs(l12 - l21) * seg_len < te * (a1 * a2))) tie = true;

@@ -475,7 +475,15 @@ int pct_column_counts(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, 
 // A8: the iteration driver.  iters x ceil(m/B) x (project+scatter, update) on one stream, no host sync inside.
 int pct_solve(pct_ctx* ctx, const pct_paths* P, const float* b, const float* x0, int iters, int64_t block_size, float lambda,
               float* x_out, void* stream) {
+    return pct_solve_ex(ctx, P, b, x0, iters, block_size, lambda, nullptr, x_out, stream);
+}
+
+int pct_solve_ex(pct_ctx* ctx, const pct_paths* P, const float* b, const float* x0, int iters, int64_t block_size, float lambda,
+                 const pct_solve_opts* opts, float* x_out, void* stream) {
     if (!ctx) return PCT_E_INVALID_ARG;
+    const float* wts = opts ? opts->weights : nullptr;
+    const float clamp_lo = opts ? opts->clamp_lo : 1.f, clamp_hi = opts ? opts->clamp_hi : 0.f;       // lo > hi: no clamp
+    if (opts && (std::isnan(opts->clamp_lo) || std::isnan(opts->clamp_hi))) return set_error(ctx, PCT_E_INVALID_ARG, "NaN clamp bound");
     if (!P || (!b && P->m > 0) || !x0 || !x_out || iters < 0 || block_size < 1 || !std::isfinite(lambda))
         return set_error(ctx, PCT_E_INVALID_ARG, "bad solve arguments");
     if (!same_grid(ctx, P)) return set_error(ctx, PCT_E_INVALID_ARG, "paths were generated on another grid or device");
@@ -530,14 +538,14 @@ int pct_solve(pct_ctx* ctx, const pct_paths* P, const float* b, const float* x0,
                 // (and later calls with the same paths and block size) accumulate Delta only
                 uint32_t* counts = plan_counts ? plan_counts + (size_t)t * (size_t)ctx->n_vox : nullptr;
                 const bool cached = counts && plan->counts_ready[(size_t)t];
-                if ((rc = launch_block_windowed(ctx, P, plan, t, !cached, b, x_out, ctx->ds, ctx->dsum, st)) != PCT_OK) return rc;
+                if ((rc = launch_block_windowed(ctx, P, plan, t, !cached, b, wts, x_out, ctx->ds, ctx->dsum, st)) != PCT_OK) return rc;
                 const int64_t nd = plan->direct_count[(size_t)t];
-                if (nd > 0 && (rc = launch_block_project_scatter(ctx, P, i0, i0 + nd, plan->direct_list, !cached, b, x_out, ctx->ds, ctx->dsum, st)) != PCT_OK) return rc;
-                if ((rc = launch_block_update(ctx, x_out, ctx->ds, ctx->dsum, counts, !cached, lambda, st)) != PCT_OK) return rc;
+                if (nd > 0 && (rc = launch_block_project_scatter(ctx, P, i0, i0 + nd, plan->direct_list, !cached, b, wts, x_out, ctx->ds, ctx->dsum, st)) != PCT_OK) return rc;
+                if ((rc = launch_block_update(ctx, x_out, ctx->ds, ctx->dsum, counts, !cached, lambda, clamp_lo, clamp_hi, st)) != PCT_OK) return rc;
                 if (counts) const_cast<SolvePlan*>(plan)->counts_ready[(size_t)t] = 1;
             } else {
-                if ((rc = launch_block_project_scatter(ctx, P, i0, i1, nullptr, true, b, x_out, ctx->ds, ctx->dsum, st)) != PCT_OK) return rc;
-                if ((rc = launch_block_update(ctx, x_out, ctx->ds, ctx->dsum, nullptr, false, lambda, st)) != PCT_OK) return rc;
+                if ((rc = launch_block_project_scatter(ctx, P, i0, i1, nullptr, true, b, wts, x_out, ctx->ds, ctx->dsum, st)) != PCT_OK) return rc;
+                if ((rc = launch_block_update(ctx, x_out, ctx->ds, ctx->dsum, nullptr, false, lambda, clamp_lo, clamp_hi, st)) != PCT_OK) return rc;
             }
         }
     }

@@ -197,12 +197,13 @@ int launch_decode(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, cons
 int launch_forward_project(pct_ctx* ctx, const pct_paths* P, const float* x, float* b_out, cudaStream_t st);
 int launch_column_counts(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, uint32_t* counts, cudaStream_t st);
 int launch_block_project_scatter(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, const uint32_t* list, bool count,
-                                 const float* b, const float* x, float2* ds, float* dsum, cudaStream_t st);
+                                 const float* b, const float* wts, const float* x, float2* ds, float* dsum, cudaStream_t st);
 int launch_block_windowed(pct_ctx* ctx, const pct_paths* P, const SolvePlan* plan, int64_t block, bool count, const float* b,
-                          const float* x, float2* ds, float* dsum, cudaStream_t st);
+                          const float* wts, const float* x, float2* ds, float* dsum, cudaStream_t st);
 int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaStream_t st, SolvePlan** out);
 void free_solve_plan(SolvePlan* plan);
-int launch_block_update(pct_ctx* ctx, float* x, float2* ds, float* dsum, uint32_t* counts, bool store, float lambda, cudaStream_t st);
+int launch_block_update(pct_ctx* ctx, float* x, float2* ds, float* dsum, uint32_t* counts, bool store, float lambda, float clamp_lo,
+                        float clamp_hi, cudaStream_t st);
 int launch_fill(pct_ctx* ctx, float* p, int64_t n, float value, cudaStream_t st);
 int launch_collect_flagged(pct_ctx* ctx, const pct_paths* P, unsigned mask, uint32_t* idx, int64_t cap, unsigned long long* d_count, cudaStream_t st);
 

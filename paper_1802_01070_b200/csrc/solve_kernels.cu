@@ -98,7 +98,7 @@ __global__ void __launch_bounds__(PROJ_THREADS)
 k_block_project_scatter(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, const int32_t* __restrict__ start,
                         const float* __restrict__ ell, const uint64_t* __restrict__ code_off,
                         const ulonglong2* __restrict__ codes, int64_t i0, int64_t i1, const uint32_t* __restrict__ list,
-                        const float* __restrict__ b, const float* __restrict__ x, float2* __restrict__ ds,
+                        const float* __restrict__ b, const float* __restrict__ wts, const float* __restrict__ x, float2* __restrict__ ds,
                         float* __restrict__ dsum) {
     // list == nullptr: histories [i0, i1); else the histories list[i0 .. i1) (a block's direct list, plan.cu)
     const int lane = threadIdx.x & 31;
@@ -113,7 +113,8 @@ k_block_project_scatter(const __grid_constant__ DevCfg g, const uint32_t* __rest
         for_each_visit(codes, off, st, n, g.sx, g.sy, g.sz, lane, [&](int vox) { S += __ldg(x + vox); });
         S = warp_sum(S);
         const float l = ell[i];
-        const float c = (b[i] - l * S) / ((float)n * l);
+        float c = (b[i] - l * S) / ((float)n * l);
+        if (wts) c *= wts[i];                                   // R27: weighted row
         for_each_visit(codes, off, st, n, g.sx, g.sy, g.sz, lane, [&](int vox) {
             if (COUNT) red_add_v2(ds + vox, c, 1.0f);
             else asm volatile("red.global.add.f32 [%0], %1;" ::"l"(dsum + vox), "f"(c) : "memory");
@@ -122,12 +123,16 @@ k_block_project_scatter(const __grid_constant__ DevCfg g, const uint32_t* __rest
 }
 
 // A7: x_j += lambda * Delta_j / max(1, s_j); clear the accumulator (R15-R16).  Only touched voxels are written.
-__global__ void __launch_bounds__(256) k_block_update(float* __restrict__ x, float2* __restrict__ ds, int64_t n, float lambda) {
+// clamp_of: R27's box clamp on an updated voxel (NaN stays NaN: it is compared, not passed through fminf / fmaxf)
+struct Clamp { float lo, hi; int on; };
+__device__ __forceinline__ float clamp_of(const Clamp& c, float v) { return c.on ? (v < c.lo ? c.lo : (v > c.hi ? c.hi : v)) : v; }
+
+__global__ void __launch_bounds__(256) k_block_update(float* __restrict__ x, float2* __restrict__ ds, int64_t n, float lambda, Clamp cl) {
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += stride) {
         const float2 a = ds[j];
         if (a.y > 0.f) {
-            x[j] += lambda * a.x / a.y;
+            x[j] = clamp_of(cl, x[j] + lambda * a.x / a.y);
             ds[j] = make_float2(0.f, 0.f);
         }
     }
@@ -135,46 +140,51 @@ __global__ void __launch_bounds__(256) k_block_update(float* __restrict__ x, flo
 
 // A7, first sweep over a block with a count cache: as k_block_update, and s_j^t is stored (all voxels: zeros too).
 __global__ void __launch_bounds__(256) k_block_update_store(float* __restrict__ x, float2* __restrict__ ds, int64_t n, float lambda,
-                                                            uint32_t* __restrict__ counts) {
+                                                            uint32_t* __restrict__ counts, Clamp cl) {
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += stride) {
         const float2 a = ds[j];
         counts[j] = (uint32_t)a.y;
         if (a.y > 0.f) {
-            x[j] += lambda * a.x / a.y;
+            x[j] = clamp_of(cl, x[j] + lambda * a.x / a.y);
             ds[j] = make_float2(0.f, 0.f);
         }
     }
 }
 
-// A7 with cached counts: x_j += lambda * Delta_j / s_j^t wherever Delta_j != 0 (a zero sum leaves x_j unchanged anyway)
+// A7 with cached counts: x_j += lambda * Delta_j / s_j^t wherever Delta_j != 0 (a zero sum leaves x_j unchanged anyway).
+// With the clamp on, every voxel the block visits (s_j^t > 0) is clamped, moved or not (R27), so the counts are read for all.
 __global__ void __launch_bounds__(256) k_block_update_cached(float* __restrict__ x, float* __restrict__ dsum, int64_t n, float lambda,
-                                                             const uint32_t* __restrict__ counts) {
+                                                             const uint32_t* __restrict__ counts, Clamp cl) {
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += stride) {
         const float d = dsum[j];
         if (d != 0.f) {
-            x[j] += lambda * d / (float)counts[j];
+            x[j] = clamp_of(cl, x[j] + lambda * d / (float)counts[j]);
             dsum[j] = 0.f;
+        } else if (cl.on && counts[j] > 0u) {
+            x[j] = clamp_of(cl, x[j]);
         }
     }
 }
 
 // the same, four voxels per thread with 16-byte accesses (n divisible by 4, pointers 16-byte aligned)
 __global__ void __launch_bounds__(256) k_block_update_cached4(float4* __restrict__ x, float4* __restrict__ dsum, int64_t n4, float lambda,
-                                                              const uint4* __restrict__ counts) {
+                                                              const uint4* __restrict__ counts, Clamp cl) {
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < n4; j += stride) {
         const float4 d = dsum[j];
-        if (d.x == 0.f && d.y == 0.f && d.z == 0.f && d.w == 0.f) continue;
+        const bool moved = !(d.x == 0.f && d.y == 0.f && d.z == 0.f && d.w == 0.f);
+        if (!moved && !cl.on) continue;
         const uint4 c = counts[j];
+        if (!moved && (c.x | c.y | c.z | c.w) == 0u) continue;
         float4 v = x[j];
-        if (d.x != 0.f) v.x += lambda * d.x / (float)c.x;
-        if (d.y != 0.f) v.y += lambda * d.y / (float)c.y;
-        if (d.z != 0.f) v.z += lambda * d.z / (float)c.z;
-        if (d.w != 0.f) v.w += lambda * d.w / (float)c.w;
+        if (c.x > 0u) v.x = clamp_of(cl, d.x != 0.f ? v.x + lambda * d.x / (float)c.x : v.x);
+        if (c.y > 0u) v.y = clamp_of(cl, d.y != 0.f ? v.y + lambda * d.y / (float)c.y : v.y);
+        if (c.z > 0u) v.z = clamp_of(cl, d.z != 0.f ? v.z + lambda * d.z / (float)c.z : v.z);
+        if (c.w > 0u) v.w = clamp_of(cl, d.w != 0.f ? v.w + lambda * d.w / (float)c.w : v.w);
         x[j] = v;
-        dsum[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (moved) dsum[j] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
 }
 
@@ -209,33 +219,35 @@ int launch_column_counts(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i
 }
 
 int launch_block_project_scatter(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, const uint32_t* list, bool count,
-                                 const float* b, const float* x, float2* ds, float* dsum, cudaStream_t st) {
+                                 const float* b, const float* wts, const float* x, float2* ds, float* dsum, cudaStream_t st) {
     if (i1 <= i0) return PCT_OK;
     ProfScope prof(ctx, 3, st);
     if (count)
         k_block_project_scatter<true><<<proj_grid(ctx, i1 - i0), PROJ_THREADS, 0, st>>>(ctx->cfg, P->N, P->start, P->ell, P->code_off,
-                                                                                        P->codes, i0, i1, list, b, x, ds, dsum);
+                                                                                        P->codes, i0, i1, list, b, wts, x, ds, dsum);
     else
         k_block_project_scatter<false><<<proj_grid(ctx, i1 - i0), PROJ_THREADS, 0, st>>>(ctx->cfg, P->N, P->start, P->ell, P->code_off,
-                                                                                         P->codes, i0, i1, list, b, x, ds, dsum);
+                                                                                         P->codes, i0, i1, list, b, wts, x, ds, dsum);
     ++ctx->launches;
     PCT_CUDA(ctx, cudaGetLastError());
     return PCT_OK;
 }
 
 // counts == nullptr: fused counts in ds.  store: fused counts, and s_j is written to counts.  else: cached counts, dsum.
-int launch_block_update(pct_ctx* ctx, float* x, float2* ds, float* dsum, uint32_t* counts, bool store, float lambda, cudaStream_t st) {
+int launch_block_update(pct_ctx* ctx, float* x, float2* ds, float* dsum, uint32_t* counts, bool store, float lambda, float clamp_lo,
+                        float clamp_hi, cudaStream_t st) {
+    const Clamp cl = {clamp_lo, clamp_hi, clamp_lo <= clamp_hi ? 1 : 0};
     const int64_t n = ctx->n_vox;
     const int64_t want = (n + 255) / 256;
     const int64_t cap = (int64_t)ctx->num_sms * 16;
     const unsigned grid = (unsigned)(want < cap ? want : cap);
     ProfScope prof(ctx, 2, st);
-    if (!counts) k_block_update<<<grid, 256, 0, st>>>(x, ds, n, lambda);
-    else if (store) k_block_update_store<<<grid, 256, 0, st>>>(x, ds, n, lambda, counts);
+    if (!counts) k_block_update<<<grid, 256, 0, st>>>(x, ds, n, lambda, cl);
+    else if (store) k_block_update_store<<<grid, 256, 0, st>>>(x, ds, n, lambda, counts, cl);
     else if (n % 4 == 0 && (((uintptr_t)x | (uintptr_t)dsum | (uintptr_t)counts) & 15) == 0)
         k_block_update_cached4<<<grid, 256, 0, st>>>(reinterpret_cast<float4*>(x), reinterpret_cast<float4*>(dsum), n / 4, lambda,
-                                                     reinterpret_cast<const uint4*>(counts));
-    else k_block_update_cached<<<grid, 256, 0, st>>>(x, dsum, n, lambda, counts);
+                                                     reinterpret_cast<const uint4*>(counts), cl);
+    else k_block_update_cached<<<grid, 256, 0, st>>>(x, dsum, n, lambda, counts, cl);
     ++ctx->launches;
     PCT_CUDA(ctx, cudaGetLastError());
     return PCT_OK;

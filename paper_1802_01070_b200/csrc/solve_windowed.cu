@@ -154,7 +154,8 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
                  const int32_t* __restrict__ start, const uint64_t* __restrict__ code_off, const ulonglong2* __restrict__ codes,
                  const uint32_t* __restrict__ perm, const uint32_t* __restrict__ p0, const uint8_t* __restrict__ pflag,
                  const uint8_t* __restrict__ cnt, const unsigned long long* __restrict__ stream,
-                 PlanGroup* __restrict__ groups, const uint32_t* __restrict__ launch_order, int64_t group0, const float* __restrict__ b, const float* __restrict__ x,
+                 PlanGroup* __restrict__ groups, const uint32_t* __restrict__ launch_order, int64_t group0, const float* __restrict__ b,
+                 const float* __restrict__ wts, const float* __restrict__ x,
                  float2* __restrict__ ds, float* __restrict__ dsum) {
     extern __shared__ __align__(16) unsigned char smem[];
     __shared__ unsigned tbl[8];
@@ -243,6 +244,7 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
     if (has) {
         const float l = ell[i];
         ci = (b[i] - l * S) / ((float)n_vis * l);
+        if (wts) ci *= wts[i];                                   // R27: weighted row
     }
     const float aci = fabsf(ci);
     const bool finite = aci < INFINITY;                                  // false for Inf and NaN
@@ -326,7 +328,7 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
 }
 
 int launch_block_windowed(pct_ctx* ctx, const pct_paths* P, const SolvePlan* plan, int64_t block, bool count, const float* b,
-                          const float* x, float2* ds, float* dsum, cudaStream_t st) {
+                          const float* wts, const float* x, float2* ds, float* dsum, cudaStream_t st) {
     const int64_t g0 = plan->group_begin[(size_t)block], g1 = plan->group_begin[(size_t)block + 1];
     if (g1 <= g0) return PCT_OK;
     if (!ctx->k2w_ready) {
@@ -337,10 +339,10 @@ int launch_block_windowed(pct_ctx* ctx, const pct_paths* P, const SolvePlan* pla
     ProfScope prof(ctx, 1, st);
     if (count)
         k_block_windowed<true><<<(unsigned)(g1 - g0), GROUP, K2W_SMEM, st>>>(ctx->cfg, P->N, P->ell, P->start, P->code_off, P->codes, plan->perm, plan->p0, plan->pflag,
-                                                                            plan->cnt, plan->stream, plan->groups, plan->launch_order, g0, b, x, ds, dsum);
+                                                                            plan->cnt, plan->stream, plan->groups, plan->launch_order, g0, b, wts, x, ds, dsum);
     else
         k_block_windowed<false><<<(unsigned)(g1 - g0), GROUP, K2W_SMEM, st>>>(ctx->cfg, P->N, P->ell, P->start, P->code_off, P->codes, plan->perm, plan->p0, plan->pflag,
-                                                                             plan->cnt, plan->stream, plan->groups, plan->launch_order, g0, b, x, ds, dsum);
+                                                                             plan->cnt, plan->stream, plan->groups, plan->launch_order, g0, b, wts, x, ds, dsum);
     ++ctx->launches;
     PCT_CUDA(ctx, cudaGetLastError());
     return PCT_OK;
