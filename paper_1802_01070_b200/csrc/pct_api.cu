@@ -122,6 +122,9 @@ ProfScope::~ProfScope() {
     ctx->prof_events[kind]->push_back(e);
 }
 
+// up to this many histories a block is run by the persistent sweep kernel: its update costs one atomic exchange per visit,
+// which loses against a streaming pass over the grid (~12 us at 4 M voxels) once a block has more than ~1e6 visits
+constexpr int64_t SMALL_BLOCK_MAX = 4096;
 constexpr int64_t DEFAULT_MIN_PLAN_BLOCK = 32768;   // below this a block is too sparse for shared-memory windows
 
 static double factorial(int k) { double r = 1.0; for (int i = 2; i <= k; ++i) r *= i; return r; }
@@ -529,6 +532,12 @@ int pct_solve_ex(pct_ctx* ctx, const pct_paths* P, const float* b, const float* 
             }
             plan_counts = ctx->counts_buf;
         }
+    }
+    // small blocks on the direct path: all sweeps in one persistent cooperative kernel (solve_kernels.cu); PCT_HOST_SWEEPS=1
+    // keeps the launch-per-block loop (A/B, debugging)
+    if (!plan && n_blocks >= 4 && block_size <= SMALL_BLOCK_MAX && !getenv("PCT_HOST_SWEEPS")) {
+        rc = launch_sweeps_persistent(ctx, P, b, wts, x_out, iters, block_size, lambda, clamp_lo, clamp_hi, st);
+        if (rc != PCT_E_CAPACITY) return rc;
     }
     for (int it = 0; it < iters; ++it) {
         for (int64_t t = 0, i0 = 0; i0 < P->m; i0 += block_size, ++t) {

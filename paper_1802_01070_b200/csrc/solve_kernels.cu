@@ -7,6 +7,8 @@
 // touch consecutive voxels of the path, so gathers of x and reductions into {Delta,s} coalesce per 32-byte sector
 // wherever the path runs along x.  The code stream is the only compulsory HBM traffic (3 bit / visit); x and the
 // accumulator live in L2.
+#include <cooperative_groups.h>
+
 #include "pct_internal.cuh"
 
 namespace pct {
@@ -52,6 +54,32 @@ __device__ __forceinline__ void for_each_visit(const ulonglong2* __restrict__ co
         const int vox = base + warp_inclusive_scan(d, lane);
         if (visit < n) f(vox);
         base = __shfl_sync(0xffffffffu, vox, 31);
+    }
+}
+
+// The same walk, four rounds (128 visits) at a time: all four rounds are decoded first, then `load` is issued for all of
+// them, then `use` consumes the results -- the memory round trips of the four rounds overlap instead of following one
+// another (a warp issues in order: it would stall at the first use of round r before issuing round r + 1).
+template <typename T, typename L, typename U>
+__device__ __forceinline__ void for_each_visit_x4(const ulonglong2* __restrict__ codes, uint64_t off, int32_t start, unsigned n,
+                                                  int sx, int sy, int sz, int lane, L&& load, U&& use) {
+    const unsigned long long* cp = reinterpret_cast<const unsigned long long*>(codes + off);
+    int base = start;
+    for (unsigned v0 = 0; v0 < n; v0 += 128) {
+        int vox[4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const unsigned visit = v0 + 32u * r + lane;
+            int d = 0;
+            if (visit < n && visit > 0) d = step_delta(cp, visit, sx, sy, sz);
+            vox[r] = base + warp_inclusive_scan(d, lane);
+            base = __shfl_sync(0xffffffffu, vox[r], 31);
+        }
+        T val[4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) if (v0 + 32u * r + lane < n) val[r] = load(vox[r]);
+#pragma unroll
+        for (int r = 0; r < 4; ++r) if (v0 + 32u * r + lane < n) use(vox[r], val[r]);
     }
 }
 
@@ -250,6 +278,112 @@ int launch_block_update(pct_ctx* ctx, float* x, float2* ds, float* dsum, uint32_
     else k_block_update_cached<<<grid, 256, 0, st>>>(x, dsum, n, lambda, counts, cl);
     ++ctx->launches;
     PCT_CUDA(ctx, cudaGetLastError());
+    return PCT_OK;
+}
+
+// ---- small blocks: all sweeps in ONE persistent cooperative kernel (A8; block 3200 is 2x slower than
+// 320000) ------------------------------------------------------------------------------------------------------------------
+// With a few thousand histories per block a sweep is tens of thousands of (project, update) pairs of a few microseconds
+// each.  Launched pair by pair (from the host or from a CUDA graph: measured 19-21 us per pair either way at B = 1000) the
+// sweep is bound by launch latency and by the chain of dependent loads every fresh kernel starts with, and an update pass
+// over the whole grid per block adds n voxels x blocks of traffic.  Here the control never leaves the device:
+//   * one cooperative kernel, as many CTAs as a block has work for (all co-resident), loops over iters x blocks; the two
+//     phases of a block are separated by grid-wide barriers instead of kernel boundaries;
+//   * the update does not sweep the grid: every warp walks its rows once more and, at every visit, claims the voxel's
+//     accumulator with an atomic exchange -- the one visit that gets a non-zero count back applies
+//     x_j += lambda Delta_j / s_j (and the clamp), all others see zero and pass.  The accumulator is left cleared;
+//   * a warp keeps the same position in every block; the header of its first row of the next block is loaded, and the row's
+//     codes are pulled into L2, before the barrier.
+// x is read with ld.global.cg (L2): other SMs change it between the phases.
+namespace cg = cooperative_groups;
+
+struct RowHead { unsigned n; int32_t start; uint64_t off; float ell, b, w; };
+
+__device__ __forceinline__ RowHead load_head(const uint32_t* __restrict__ N, const int32_t* __restrict__ start, const float* __restrict__ ell,
+                                             const uint64_t* __restrict__ code_off, const float* __restrict__ b, const float* __restrict__ wts, int64_t i) {
+    RowHead h;
+    h.n = N[i]; h.start = start[i]; h.off = code_off[i]; h.ell = ell[i]; h.b = b[i]; h.w = wts ? wts[i] : 1.f;
+    return h;
+}
+
+// 8 warps per CTA: 1024-thread CTAs (fewer arrivals at the grid barrier) were 35 % slower -- a block of 1000 rows then sits on 32 SMs
+constexpr int PS_THREADS = 256, PS_WARPS = PS_THREADS / 32;
+
+__global__ void __launch_bounds__(PS_THREADS)
+k_sweeps_persistent(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, const int32_t* __restrict__ start,
+                    const float* __restrict__ ell, const uint64_t* __restrict__ code_off, const ulonglong2* __restrict__ codes, int64_t m,
+                    int64_t block_size, int64_t n_blocks, int iters, const float* __restrict__ b, const float* __restrict__ wts, float* x,
+                    float2* ds, float lambda, Clamp cl) {
+    cg::grid_group grid = cg::this_grid();
+    const int lane = threadIdx.x & 31;
+    const int64_t warp = (int64_t)blockIdx.x * PS_WARPS + (threadIdx.x >> 5), warps = (int64_t)gridDim.x * PS_WARPS;
+    const int64_t total = (int64_t)iters * n_blocks;
+    // the header of the first row this warp takes in a block, loaded one block ahead (and its codes pulled into L2)
+    auto first_row = [&](int64_t pair) { const int64_t t = pair % n_blocks; return t * block_size + warp; };
+    auto row_end = [&](int64_t pair) { const int64_t i0 = (pair % n_blocks) * block_size; return (m - i0) < block_size ? m : i0 + block_size; };
+    RowHead next = {};
+    if (first_row(0) < row_end(0)) next = load_head(N, start, ell, code_off, b, wts, first_row(0));
+    for (int64_t pair = 0; pair < total; ++pair) {
+        const int64_t i1 = row_end(pair);
+        // A5 + A6: project and scatter
+        for (int64_t i = first_row(pair); i < i1; i += warps) {
+            const RowHead h = i == first_row(pair) ? next : load_head(N, start, ell, code_off, b, wts, i);
+            if (h.n == 0) continue;
+            float S = 0.f;
+            for_each_visit_x4<float>(codes, h.off, h.start, h.n, g.sx, g.sy, g.sz, lane, [&](int vox) { return __ldcg(x + vox); },
+                                     [&](int, float v) { S += v; });
+            S = warp_sum(S);
+            const float c = h.w * (h.b - h.ell * S) / ((float)h.n * h.ell);
+            for_each_visit(codes, h.off, h.start, h.n, g.sx, g.sy, g.sz, lane, [&](int vox) { red_add_v2(ds + vox, c, 1.0f); });
+        }
+        grid.sync();
+        // A7: the visit that still finds the count owns the voxel's update.  One 64-bit exchange fetches and clears
+        // {Delta_j, s_j}; x_j is loaded alongside it rather than after it.
+        for (int64_t i = first_row(pair); i < i1; i += warps) {
+            const RowHead h = i == first_row(pair) ? next : load_head(N, start, ell, code_off, b, wts, i);
+            if (h.n == 0) continue;
+            struct Got { float xv; unsigned long long old; };
+            for_each_visit_x4<Got>(codes, h.off, h.start, h.n, g.sx, g.sy, g.sz, lane,
+                                   [&](int vox) { Got q; q.xv = __ldcg(x + vox); q.old = atomicExch(reinterpret_cast<unsigned long long*>(ds + vox), 0ull); return q; },
+                                   [&](int vox, const Got& q) {
+                                       const float s = __uint_as_float((unsigned)(q.old >> 32)), d = __uint_as_float((unsigned)q.old);
+                                       if (s > 0.f) x[vox] = clamp_of(cl, q.xv + lambda * d / s);
+                                   });
+        }
+        if (pair + 1 < total && first_row(pair + 1) < row_end(pair + 1)) {
+            next = load_head(N, start, ell, code_off, b, wts, first_row(pair + 1));
+            const char* cp = reinterpret_cast<const char*>(codes + next.off);
+            if (next.n > 0 && (unsigned)lane * 128u < (next.n * 3u + 7u) / 8u) asm volatile("prefetch.global.L2 [%0];" ::"l"(cp + lane * 128));
+        }
+        grid.sync();
+    }
+}
+
+// iters sweeps over all blocks of `block_size` histories in one cooperative launch.  ds must be all zero (it is left so).
+// Returns PCT_E_CAPACITY (and sets no error text) if the device cannot launch cooperatively: the caller falls back.
+int launch_sweeps_persistent(pct_ctx* ctx, const pct_paths* P, const float* b, const float* wts, float* x, int iters, int64_t block_size, float lambda,
+                             float clamp_lo, float clamp_hi, cudaStream_t st) {
+    int64_t n_blocks = (P->m + block_size - 1) / block_size;
+    if (iters <= 0 || n_blocks == 0) return PCT_OK;
+    int coop = 0, per_sm = 0;
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, ctx->device);
+    if (!coop || cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sweeps_persistent, PS_THREADS, 0) != cudaSuccess || per_sm < 1) {
+        cudaGetLastError();
+        return PCT_E_CAPACITY;
+    }
+    Clamp cl = {clamp_lo, clamp_hi, clamp_lo <= clamp_hi ? 1 : 0};
+    const int64_t rows = block_size < P->m ? block_size : P->m;
+    const int64_t want = (rows + PS_WARPS - 1) / PS_WARPS, cap = (int64_t)ctx->num_sms * per_sm;
+    int grid = (int)(want < cap ? want : cap);
+    if (grid < 1) grid = 1;
+    int64_t m = P->m;
+    const uint32_t* N = P->N; const int32_t* start = P->start; const float* ell = P->ell; const uint64_t* code_off = P->code_off;
+    const ulonglong2* codes = P->codes; float2* ds = ctx->ds;
+    void* args[] = {(void*)&ctx->cfg, (void*)&N, (void*)&start, (void*)&ell, (void*)&code_off, (void*)&codes, (void*)&m, (void*)&block_size,
+                    (void*)&n_blocks, (void*)&iters, (void*)&b, (void*)&wts, (void*)&x, (void*)&ds, (void*)&lambda, (void*)&cl};
+    ProfScope prof(ctx, 3, st);
+    PCT_CUDA(ctx, cudaLaunchCooperativeKernel((const void*)k_sweeps_persistent, dim3((unsigned)grid), dim3(PS_THREADS), args, 0, st));
+    ++ctx->launches;
     return PCT_OK;
 }
 
