@@ -13,11 +13,18 @@
  *     the caller and never retained or freed by the library, except the opaque pct_ctx / pct_paths objects,
  *     which the library owns until pct_destroy / pct_paths_free.
  *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Work is enqueued on it; device
- *     results are valid once the caller has synchronised the stream.  pct_generate_mlp and the *_host calls
- *     synchronise the stream themselves (they need sizes on the host).
+ *     results are valid once the caller has synchronised the stream.  Calls that need sizes on the host synchronise
+ *     the stream themselves and say so below: pct_generate_mlp, pct_paths_decode, pct_paths_flagged, pct_fbp, the
+ *     *_host calls, and the FIRST pct_solve / pct_solve_ex on a (paths, block_size) pair that builds a solve plan.
+ *   - Thread safety: a pct_ctx and a pct_paths are each used by one thread at a time.  pct_solve keeps a solve plan
+ *     (a solver-shaped copy of the rows) inside the pct_paths it is given -- hence `pct_paths*`, not const -- and the
+ *     block counts of that plan inside the context.
+ *   - Out-of-range depth is not an error code: a history whose hull chord exceeds poly_max_depth_mm is rejected with
+ *     the flag PCT_REJ_DEPTH (SURVEY.md 8(b) listed PCT_E_DEPTH_RANGE; a per-history condition belongs in the flags).
  *   - Device memory: paths, plans and scratch come from a process-wide cache of device blocks that are reused on an exact
- *     size match (rebuilding the same reconstruction costs no allocation); pct_trim_cache releases the idle blocks.  All
- *     calls on one context must be issued on one stream at a time (a reused block relies on stream order).
+ *     size match (rebuilding the same reconstruction costs no allocation); pct_trim_cache releases the idle blocks, and so
+ *     does pct_destroy of the last context of a device.  All calls on one context must be issued on one stream at a time (a
+ *     reused block relies on stream order).
  *   - Return value: PCT_OK (0) or a negative PCT_E_* code; never throws, never aborts.  pct_last_error(ctx)
  *     gives a human-readable message for the last failure on that context.
  *   - Frames (R1): grid frame (x,y,z), z = rotation axis, voxel (ix,iy,iz) = origin + [i, i+1]*h per axis,
@@ -122,8 +129,12 @@ int pct_column_counts(pct_ctx* ctx, const pct_paths* paths, int64_t i0, int64_t 
 /* A5-A8 (R13-R18): `iters` sweeps of block-iterative DROP with unit weights,
  *   x <- x + lambda * diag(1/max(1,s_j^t)) * sum_{i in block t} [(b_i - <a_i,x>)/||a_i||^2] a_i,
  * blocks = consecutive ranges of block_size histories.  b: DEVICE float32[m]; x0, x_out: DEVICE float32[n],
- * x_out may alias x0.  FP32 arithmetic, FP32 atomics (result unique up to summation order). */
-int pct_solve(pct_ctx* ctx, const pct_paths* paths, const float* b, const float* x0, int iters, int64_t block_size,
+ * x_out may alias x0.  FP32 arithmetic, FP32 atomics (result unique up to summation order).
+ * Blocks of at least 32768 histories (pct_solve_config) run through a solve plan that is built on the first call for this
+ * (paths, block_size), cached in `paths` and rebuilt when block_size changes; building it synchronises `stream` several
+ * times.  Blocks of at most 4096 histories run in one persistent cooperative kernel; sizes in between launch two kernels
+ * per block.  No synchronisation otherwise. */
+int pct_solve(pct_ctx* ctx, pct_paths* paths, const float* b, const float* x0, int iters, int64_t block_size,
               float lambda, float* x_out, void* stream);
 
 /* A5-A8 with the options of ref [9]-style solvers ("standard iterative solver [9]"; reading R27):
@@ -134,7 +145,7 @@ typedef struct {
     const float* weights;
     float clamp_lo, clamp_hi;
 } pct_solve_opts;
-int pct_solve_ex(pct_ctx* ctx, const pct_paths* paths, const float* b, const float* x0, int iters, int64_t block_size,
+int pct_solve_ex(pct_ctx* ctx, pct_paths* paths, const float* b, const float* x0, int iters, int64_t block_size,
                  float lambda, const pct_solve_opts* opts /* HOST */, float* x_out, void* stream);
 
 /* The FBP image the solver starts from ("Using the FBP image as the initial iterate"; reading R25): every

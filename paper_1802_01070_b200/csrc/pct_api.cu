@@ -127,6 +127,9 @@ ProfScope::~ProfScope() {
 constexpr int64_t SMALL_BLOCK_MAX = 4096;
 constexpr int64_t DEFAULT_MIN_PLAN_BLOCK = 32768;   // below this a block is too sparse for shared-memory windows
 
+static int g_ctx_count[64];            // live contexts per device (guarded by g_ctx_mu): the last pct_destroy trims the cache
+static std::mutex g_ctx_mu;
+
 static double factorial(int k) { double r = 1.0; for (int i = 2; i <= k; ++i) r *= i; return r; }
 
 struct DeviceGuard {
@@ -241,6 +244,7 @@ int pct_create(const pct_geometry* geom, const pct_mlp_params* params, int devic
     if (cudaMalloc(&ctx->d_stats, sizeof(GenStats)) != cudaSuccess || cudaMalloc(&ctx->d_total, sizeof(unsigned long long)) != cudaSuccess) {
         cudaGetLastError(); pct_destroy(ctx); return PCT_E_OOM;
     }
+    { std::lock_guard<std::mutex> lock(g_ctx_mu); if (device < 64) ++g_ctx_count[device]; ctx->counted = true; }
     *out = ctx;
     return PCT_OK;
 }
@@ -248,6 +252,9 @@ int pct_create(const pct_geometry* geom, const pct_mlp_params* params, int devic
 void pct_destroy(pct_ctx* ctx) {
     if (!ctx) return;
     DeviceGuard guard(ctx->device);
+    bool last = false;
+    if (ctx->counted) { std::lock_guard<std::mutex> lock(g_ctx_mu); if (ctx->device < 64) last = --g_ctx_count[ctx->device] == 0; }
+    if (last) cache_trim(ctx->device);
     cudaFree(ctx->ds); cudaFree(ctx->dsum); cudaFree(ctx->counts_buf); cudaFree(ctx->scan_tmp); cudaFree(ctx->logk); cudaFree(ctx->gen_scratch); cudaFree(ctx->d_stats); cudaFree(ctx->d_total);
     for (auto& v : ctx->prof_events) { if (v) { for (cudaEvent_t e : *v) cudaEventDestroy(e); delete v; } }
     if (ctx->prof_pool) { for (cudaEvent_t e : *ctx->prof_pool) cudaEventDestroy(e); delete ctx->prof_pool; }
@@ -476,12 +483,12 @@ int pct_column_counts(pct_ctx* ctx, const pct_paths* P, int64_t i0, int64_t i1, 
 }
 
 // A8: the iteration driver.  iters x ceil(m/B) x (project+scatter, update) on one stream, no host sync inside.
-int pct_solve(pct_ctx* ctx, const pct_paths* P, const float* b, const float* x0, int iters, int64_t block_size, float lambda,
+int pct_solve(pct_ctx* ctx, pct_paths* P, const float* b, const float* x0, int iters, int64_t block_size, float lambda,
               float* x_out, void* stream) {
     return pct_solve_ex(ctx, P, b, x0, iters, block_size, lambda, nullptr, x_out, stream);
 }
 
-int pct_solve_ex(pct_ctx* ctx, const pct_paths* P, const float* b, const float* x0, int iters, int64_t block_size, float lambda,
+int pct_solve_ex(pct_ctx* ctx, pct_paths* P, const float* b, const float* x0, int iters, int64_t block_size, float lambda,
                  const pct_solve_opts* opts, float* x_out, void* stream) {
     if (!ctx) return PCT_E_INVALID_ARG;
     const float* wts = opts ? opts->weights : nullptr;
@@ -501,7 +508,7 @@ int pct_solve_ex(pct_ctx* ctx, const pct_paths* P, const float* b, const float* 
     const bool plan_possible = iters > 0 && P->m > 0 && P->m < 0xffffffffLL && n_blocks < (1LL << 24);
     const bool want_plan = ctx->solve_mode == 2 || (ctx->solve_mode == 0 && (P->m < block_size ? P->m : block_size) >= ctx->solve_min_block);
     if (plan_possible && want_plan) {
-        pct_paths* Pm = const_cast<pct_paths*>(P);
+        pct_paths* Pm = P;
         if (Pm->plan && Pm->plan->block_size != block_size) { free_solve_plan(Pm->plan); Pm->plan = nullptr; }
         if (!Pm->plan) {
             ProfScope prof(ctx, 4, st);

@@ -144,6 +144,7 @@ struct pct_ctx {
     std::vector<cudaEvent_t>* prof_events[PCT_PROFILE_KINDS];   // start/stop pairs per kind
     std::vector<cudaEvent_t>* prof_pool;   // recycled events
     bool k2w_ready;      // dynamic shared memory attribute of k_block_windowed set on this device
+    bool counted;        // this context is in the per-device count of live contexts (pct_create completed)
 };
 
 struct pct_paths {
