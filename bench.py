@@ -242,7 +242,8 @@ def read_traffic(cfg_name, kernel):
     return None, None
 
 
-def bench_workload(args, cfg, dev, local, world, dist, steps, warmup, e2e_steps, e2e_warmup, profile_steps, want_cpu, peaks=None):
+def bench_workload(args, cfg, dev, local, world, dist, steps, warmup, e2e_steps, e2e_warmup, profile_steps, want_cpu, peaks=None,
+                   do_pre=True):
     """Runs one workload; returns (measurements for the JSON line, the peaks used)."""
     from paper_1802_01070_b200 import binding
 
@@ -343,6 +344,39 @@ def bench_workload(args, cfg, dev, local, world, dist, steps, warmup, e2e_steps,
                    "fp64_ops_per_sample": FP64_OPS_PER_SAMPLE, "mlp_samples": info["samples"],
                    "share_of_step": k1_ms / ms_prof_step if ms_prof_step > 0 else None, "measured_ms_per_step": k1_ms}
 
+    # ---- SURVEY 8(f) rows next to the hot path (untimed extras): FBP initial iterate, hull from data ---------------------
+    pre = None
+    if args.pre_steps and do_pre:
+        import math
+        n_s = 2 * int(math.ceil(0.5 * math.hypot(cfg.nx, cfg.ny))) + 2
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        ev[0].record()
+        x_fbp = ctx.fbp(protons, -cfg.u_tracker, cfg.u_tracker, b, 180, n_s, cfg.h)
+        ev[1].record()
+        carved = ctx.hull_carve(protons, -cfg.u_tracker, cfg.u_tracker, b, 1.0, 0.25 * cfg.h)
+        ev[2].record()
+        torch.cuda.synchronize()
+        paths = ctx.generate_mlp(protons, -cfg.u_tracker, cfg.u_tracker, hull_flat)
+        k = min(cfg.m, 4 * cfg.block)
+
+        def rms(xx):
+            r = (ctx.forward_project(paths, xx)[:k] - b[:k]).double()
+            return float(torch.sqrt(torch.mean(r * r)))
+        curve = {"x0=1": [rms(x0)], "x0=fbp": [rms(x_fbp)]}
+        xa, xb = x0.clone(), x_fbp.clone()
+        for _ in range(args.pre_steps):          # one sweep at a time: pct_solve resumes from the x it is given
+            ctx.solve(paths, b, xa, 1, cfg.block, cfg.lam, out=xa)
+            ctx.solve(paths, b, xb, 1, cfg.block, cfg.lam, out=xb)
+            curve["x0=1"].append(rms(xa)); curve["x0=fbp"].append(rms(xb))
+        paths.free()
+        hm = hull_flat.bool()
+        pre = {"fbp_ms": ev[0].elapsed_time(ev[1]), "fbp_bins": [cfg.nz, 180, n_s], "hull_carve_ms": ev[1].elapsed_time(ev[2]),
+               "hull_carve": {"wepl_air_mm": 1.0, "min_chord_mm": 0.25 * cfg.h, "voxels_kept": int(carved.sum()),
+                              "analytic_hull_voxels": int(hm.sum()), "analytic_hull_voxels_carved": int((hm & (carved == 0)).sum())},
+               "rms_residual_mm_by_sweep": curve,
+               "note": "rms of b - A x over the first 4 blocks after 0, 1, 2, ... sweeps from x0 = 1 and from the FBP image (PAPER.md:7)"}
+        del x_fbp, carved, xa, xb
+
     # ---- end to end through the C-ABI on pinned HOST buffers ------------------------------------------------
     e2e = None
     if e2e_steps > 0:
@@ -409,7 +443,7 @@ def bench_workload(args, cfg, dev, local, world, dist, steps, warmup, e2e_steps,
         "solver_ms_per_iter": ms_solve / (steps * cfg.iters),
         "mlp_histories_per_s": world * cfg.m * steps / (ms_mlp * 1e-3),
         "recon_s": ms_total * 1e-3 / steps,
-        "roofline": roofline, "roofline_k1": roofline_k1, "cpu_baseline": cpu_baseline, "e2e": e2e,
+        "roofline": roofline, "roofline_k1": roofline_k1, "cpu_baseline": cpu_baseline, "e2e": e2e, "preprocessing": pre,
         "gpu_launches": launches, "clocks": clocks,
     }
     del pr, protons, b, x, x0, hull_flat, hull, x_true
@@ -433,6 +467,7 @@ def main():
     ap.add_argument("--e2e-warmup", type=int, default=2)
     ap.add_argument("--profile-steps", type=int, default=2, choices=range(1, 9),
                     help="instrumented steps for the per-kernel breakdown (outside the headline timing)")
+    ap.add_argument("--pre-steps", type=int, default=5, help="sweeps of the FBP-start vs unit-start residual curve (0: skip the 8(f) extras)")
     ap.add_argument("--oracle-sample", type=int, default=1_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--secondary", default=os.environ.get("PCT_BENCH_SECONDARY", "paperB"),
@@ -472,7 +507,7 @@ def main():
         if torch.cuda.get_device_properties(local).total_memory >= need:
             torch.cuda.empty_cache()
             sec_out, _ = bench_workload(args, synth.CONFIGS[args.secondary], dev, local, world, dist, 2, 3,
-                                        1 if args.e2e_steps > 0 else 0, 1, 1, False, peaks)
+                                        1 if args.e2e_steps > 0 else 0, 1, 1, False, peaks, do_pre=False)
             sec_out.update(steps=2, warmup=3, unit=UNIT)
             secondary = sec_out
     if rank == 0:

@@ -211,8 +211,10 @@ k_hull_carve(const ProtonPtrs pr, const float* __restrict__ b, int64_t m, double
         clip_slab(Am, dm, lo_m, hi_m, m0, m1);                      // dm != 0: it is the largest component and len > 0
         if (!(m0 < m1)) continue;
         const double p10 = fma(m0, d1, A1), p11 = fma(m1, d1, A1), p20 = fma(m0, d2, A2), p21 = fma(m1, d2, A2);
-        const int j1_lo = max(0, (int)floor((fmin(p10, p11) - o1) / h) - 1), j1_hi = min(n1 - 1, (int)floor((fmax(p10, p11) - o1) / h) + 1);
-        const int j2_lo = max(0, (int)floor((fmin(p20, p21) - o2) / h) - 1), j2_hi = min(n2 - 1, (int)floor((fmax(p20, p21) - o2) / h) + 1);
+        // candidates: the voxels between the chord's two end points in this slab (a margin of 1e-6 voxel widths against rounding;
+        // a voxel beyond it could only be touched at a corner, with no chord to speak of)
+        const int j1_lo = max(0, (int)floor((fmin(p10, p11) - o1) / h - 1e-6)), j1_hi = min(n1 - 1, (int)floor((fmax(p10, p11) - o1) / h + 1e-6));
+        const int j2_lo = max(0, (int)floor((fmin(p20, p21) - o2) / h - 1e-6)), j2_hi = min(n2 - 1, (int)floor((fmax(p20, p21) - o2) / h + 1e-6));
         for (int j1 = j1_lo; j1 <= j1_hi; ++j1) {
             double f0 = m0, f1 = m1;
             if (!clip_slab(A1, d1, __dadd_rn(o1, __dmul_rn((double)j1, h)), __dadd_rn(o1, __dmul_rn((double)(j1 + 1), h)), f0, f1) || !(f1 > f0)) continue;
