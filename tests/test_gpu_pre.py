@@ -69,6 +69,25 @@ def test_fbp_matches_oracle(binding, oracle, name, m, n_theta, n_s, ds, mc):
         ctx.fbp(dev, -c.u_tracker, c.u_tracker, b_d, 0, n_s, ds)
 
 
+def test_fbp_and_carving_at_bench_geometry(binding, oracle):
+    """pct_fbp and pct_hull_carve at config 2's full grid (256 x 256 x 128, the bins bench.py uses) on the first 6 M
+    histories of the workload: whole image / whole mask against the oracle."""
+    cfg = synth.scaled(synth.CONFIGS["paperA"], int(os.environ.get("PCT_TEST_PRE_M", 6_000_000)))
+    c, ctx, dev, pa, g, b_d, b_h, hull, x_true = setup(binding, oracle, cfg)
+    n_s = 2 * int(np.ceil(0.5 * np.hypot(c.nx, c.ny))) + 2
+    x_g = ctx.fbp(dev, -c.u_tracker, c.u_tracker, b_d, 180, n_s, c.h).cpu().numpy().reshape(c.nz, c.ny, c.nx)
+    x_o = oracle.fbp(g, pa, b_h, 180, n_s, c.h)
+    scale = np.abs(x_o).max()
+    # a history within an ulp of a bin edge may land in the neighbouring bin (libm vs CUDA atan2 / cos): the bins hold ~1
+    # history each at this sample size, so such a flip moves two bins by a whole WEPL -- allow a handful of them
+    diff = np.abs(x_g - x_o)
+    assert np.linalg.norm(x_g - x_o) / np.linalg.norm(x_o) < 1e-4 and np.quantile(diff, 0.999) < 1e-6 * scale
+    h_g = ctx.hull_carve(dev, -c.u_tracker, c.u_tracker, b_d, 1.0, 0.25 * c.h).cpu().numpy().reshape(c.nz, c.ny, c.nx)
+    h_o = oracle.hull_carve(g, pa, b_h, 1.0, 0.25 * c.h)
+    assert np.array_equal(h_g, h_o), int((h_g != h_o).sum())
+    assert 0 < int((h_g == 0).sum())
+
+
 @pytest.mark.parametrize("name,m,scale", [("tiny", 50000, 1.3), ("head", 300000, 1.15), ("paperB", 200000, 1.0)])
 def test_hull_carve_matches_oracle(binding, oracle, name, m, scale):
     cfg = synth.scaled(synth.CONFIGS[name], m)
