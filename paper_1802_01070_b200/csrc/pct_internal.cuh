@@ -62,7 +62,7 @@ struct PlanGroup {
     int32_t wps;         // 64-bit code words per (slab, thread) in the group's slab-aligned code stream
     uint64_t cnt_off;    // first byte of this group's visits-per-slab table: cnt[cnt_off + slab*GROUP + thread]
     uint64_t stream_off; // first word of the group's code stream: stream[stream_off + (slab*wps + w)*GROUP + thread]
-    // part of the window the verified members actually visit, as offsets from the row's window base (k_plan_verify):
+    // part of the window the verified members actually visit, as offsets from the row's window base (k_plan_walk):
     // n - nbase(r) in [dn_lo, dn_hi], z - zbase(r) in [dz_lo, dz_hi].  Only that part is staged and flushed.
     int32_t dn_lo, dn_hi, dz_lo, dz_hi;
     int32_t max_cnt;     // largest number of visits one window slot of this group receives in a slab, measured by the first

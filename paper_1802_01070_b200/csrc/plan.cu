@@ -11,9 +11,10 @@
 //   2. radix sort       (key, i) pairs -- cub::DeviceRadixSort, the one library primitive used (a plain sort).
 //   3. k_plan_heads     group heads: every change of (block, class, z-row) and every GROUP-th sorted position.
 //   4. k_plan_params    per group: travel class, first row, window centre line (weighted mean of its members).
-//   5. k_plan_verify    WALKS THE CODES of every member and checks that each visit lies inside the group's window,
-//                       that the history never steps against the travel direction and never has more than
-//                       MAX_ROW_VISITS visits in one row; records visits per slab and the packed start coordinate.
+//   5. k_plan_walk      WALKS THE CODES of every member once: checks that each visit lies inside the group's window,
+//                       that the history never steps against the travel direction, never has more than MAX_ROW_VISITS
+//                       visits in one row nor more than the slab's word budget (fixed from the tube's slope in step 4);
+//                       records visits per slab and the packed start coordinate; re-emits the codes slab-aligned.
 //                       A history that fails is appended to its block's direct list.
 // Correctness of the solver never depends on the sort or the centre-line fit: a history is either verified to stay
 // in its group's window or it takes the direct kernel.
@@ -117,7 +118,7 @@ __device__ __forceinline__ T block_reduce_256(T v, Op op, T* scratch /* 8 */) {
 __global__ void __launch_bounds__(256)
 k_plan_params(const __grid_constant__ DevCfg g, const int32_t* __restrict__ start, const int32_t* __restrict__ end,
               const uint32_t* __restrict__ perm, int64_t m, int64_t n_groups, PlanGroup* __restrict__ groups,
-              uint32_t* __restrict__ cnt_len) {
+              uint32_t* __restrict__ cnt_len, uint32_t* __restrict__ stream_len) {
     __shared__ float sf[8];
     __shared__ int si[8];
     const int64_t gi = blockIdx.x;
@@ -125,11 +126,11 @@ k_plan_params(const __grid_constant__ DevCfg g, const int32_t* __restrict__ star
     const uint32_t size = (uint32_t)(((gi + 1 < n_groups) ? (int64_t)groups[gi + 1].start : m) - (int64_t)G.start);
     if (G.cls == 7) {
         if (threadIdx.x == 0) { G.size = size; G.nslab = 0; G.m_first = 0; G.nb0 = G.zb0 = G.sn = G.sz = 0; G.wps = 0; G.cnt_off = G.stream_off = 0;
-                                G.dn_lo = G.dz_lo = 0; G.dn_hi = G.dz_hi = -1; G.max_cnt = 0; groups[gi] = G; cnt_len[gi] = 0; }
+                                G.dn_lo = G.dz_lo = 0; G.dn_hi = G.dz_hi = -1; G.max_cnt = 0; groups[gi] = G; cnt_len[gi] = 0; stream_len[gi] = 0; }
         return;
     }
     const int dir = (G.cls & 1) ? -1 : 1;
-    float w_sum = 0.f, wn = 0.f, wz = 0.f, wsn = 0.f, wsz = 0.f;
+    float w_sum = 0.f, wn = 0.f, wz = 0.f, wsn = 0.f, wsz = 0.f, steep = 0.f;
     int r_lo = INT_MAX, r_hi = INT_MIN;      // dir * m of starts / ends
     for (uint32_t j = threadIdx.x; j < size; j += 256) {
         const uint32_t i = perm[G.start + j];
@@ -138,6 +139,7 @@ k_plan_params(const __grid_constant__ DevCfg g, const int32_t* __restrict__ star
         chord_ref(g, c, n_ref, z_ref, sl_n, sl_z);
         const float w = (float)abs(c.m_e - c.m_s) + 0.25f;
         w_sum += w; wn += w * n_ref; wz += w * z_ref; wsn += w * sl_n; wsz += w * sl_z;
+        steep = fmaxf(steep, fabsf(sl_n) + fabsf(sl_z));              // lateral steps per row of this member's chord
         r_lo = min(r_lo, dir * c.m_s);
         r_hi = max(r_hi, dir * c.m_e);
     }
@@ -147,6 +149,7 @@ k_plan_params(const __grid_constant__ DevCfg g, const int32_t* __restrict__ star
     wz = block_reduce_256(wz, fadd, sf);
     wsn = block_reduce_256(wsn, fadd, sf);
     wsz = block_reduce_256(wsz, fadd, sf);
+    steep = block_reduce_256(steep, [](float a, float b) { return fmaxf(a, b); }, sf);
     r_lo = block_reduce_256(r_lo, [](int a, int b) { return min(a, b); }, si);
     r_hi = block_reduce_256(r_hi, [](int a, int b) { return max(a, b); }, si);
     if (threadIdx.x != 0) return;
@@ -164,12 +167,18 @@ k_plan_params(const __grid_constant__ DevCfg g, const int32_t* __restrict__ star
     G.zb0 = (int)llrint(fmin(fmax(z0 + 0.5, -16000.0), 16000.0) * 65536.0);
     G.sn = (int)llrint((double)s_n * dir * 65536.0);
     G.sz = (int)llrint((double)s_z * dir * 65536.0);
-    G.wps = 0;               // k_plan_verify collects the largest visits-per-slab here
+    // words per (slab, thread) of the slab-aligned code stream, fixed BEFORE the codes are walked so that one walk can both
+    // verify and emit: a member has one visit per row plus one per lateral step, i.e. 1 + |dn/dm| + |dz/dm| per row of its
+    // chord, a slab SLAB rows; the steepest member's chord sets the budget, with 8 % and 3 visits of head room for
+    // curvature.  A member that needs more goes to the direct list like any other that does not fit.
+    const float per_slab = (float)SLAB * (1.f + fminf(steep, 2.f));
+    G.wps = ((int)ceilf(per_slab * 1.08f + 3.f) + CODES_PER_WORD - 1) / CODES_PER_WORD;
     G.cnt_off = G.stream_off = 0;
-    G.dn_lo = WIN_N; G.dn_hi = -1; G.dz_lo = WIN_Z; G.dz_hi = -1;      // empty; k_plan_verify widens them
+    G.dn_lo = WIN_N; G.dn_hi = -1; G.dz_lo = WIN_Z; G.dz_hi = -1;      // empty; k_plan_walk widens them
     G.max_cnt = 0;
     groups[gi] = G;
     cnt_len[gi] = (uint32_t)G.nslab * GROUP;
+    stream_len[gi] = (uint32_t)G.nslab * (uint32_t)G.wps * GROUP;
 }
 
 __global__ void k_plan_cnt_off(const uint64_t* __restrict__ off, int64_t n_groups, PlanGroup* __restrict__ groups) {
@@ -177,7 +186,7 @@ __global__ void k_plan_cnt_off(const uint64_t* __restrict__ off, int64_t n_group
     if (gi < n_groups) groups[gi].cnt_off = off[gi];
 }
 
-// Shared walk of k_plan_verify / k_plan_emit: thread tid of a group's CTA walks the codes of its history (plan_rank) and
+// Start of k_plan_walk: thread tid of a group's CTA walks the codes of its history (plan_rank) and
 // reports every visit as f(row r, code that led to it or PLAN_CODE_FIRST, in-window?) until f returns false.
 struct MemberWalk {
     uint32_t pos, i, n_vis;
@@ -205,13 +214,17 @@ __device__ __forceinline__ bool member_init(const DevCfg& g, const PlanGroup& G,
     return true;
 }
 
-// one CTA per group, one thread per member: walk the codes, verify the window, record visits per slab
+// One CTA per group, one thread per member: ONE walk of the member's codes that verifies the window (every visit inside
+// its row's window, never a step against the travel direction, at most MAX_ROW_VISITS visits per row, at most
+// 21 * wps visits per slab), records visits per slab, the packed start coordinate and the visited extent, and re-emits the
+// codes slab by slab, 21 per word, words [slab][w][thread] (the stream is pre-filled with pad codes; the first visit becomes
+// PLAN_CODE_FIRST).  A member that fails takes back the words it wrote and goes to its block's direct list.
 __global__ void __launch_bounds__(GROUP)
-k_plan_verify(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, const int32_t* __restrict__ start,
-              const uint64_t* __restrict__ code_off, const ulonglong2* __restrict__ codes, const uint32_t* __restrict__ perm,
-              PlanGroup* __restrict__ groups, int64_t block_size, uint32_t* __restrict__ p0_out,
-              uint8_t* __restrict__ pflag, uint8_t* __restrict__ cnt, uint32_t* __restrict__ direct_list,
-              uint32_t* __restrict__ direct_count) {
+k_plan_walk(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, const int32_t* __restrict__ start,
+            const uint64_t* __restrict__ code_off, const ulonglong2* __restrict__ codes, const uint32_t* __restrict__ perm,
+            PlanGroup* __restrict__ groups, int64_t block_size, uint32_t* __restrict__ p0_out, uint8_t* __restrict__ pflag,
+            uint8_t* __restrict__ cnt, unsigned long long* __restrict__ stream, uint32_t* __restrict__ direct_list,
+            uint32_t* __restrict__ direct_count) {
     const PlanGroup G = groups[blockIdx.x];
     MemberWalk mw;
     if (G.cls == 7) {
@@ -223,47 +236,55 @@ k_plan_verify(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, 
     const int r_end = G.nslab * SLAB;
     bool ok = r >= 0 && r < r_end;
     uint8_t* my_cnt = cnt + G.cnt_off + threadIdx.x;
-    unsigned long long w = 0;
-    int nrem = 0, row_cnt = 0, slab_cnt = 0, max_cnt = 0, cur_slab = ok ? r / SLAB : 0;
+    unsigned long long* out = stream + G.stream_off + threadIdx.x;
+    unsigned long long w = 0, acc = ~0ull;
+    int nrem = 0, row_cnt = 0, k = 0, cur_slab = ok ? r / SLAB : 0;          // k = codes emitted in the current slab
+    const int first_slab = cur_slab, slab_cap = G.wps * CODES_PER_WORD;
     int nb = ok ? plan_nbase(G, r) : 0, zb = ok ? plan_zbase(G, r) : 0;
     const uint32_t p0 = win_pack(n, r, z);
     int on_lo = WIN_N, on_hi = -1, oz_lo = WIN_Z, oz_hi = -1;
     for (uint32_t v = 0; v < mw.n_vis && ok; ++v) {
+        int code = PLAN_CODE_FIRST;
         if (v > 0) {
             if (nrem == 0) { w = __ldg(mw.cp++); nrem = CODES_PER_WORD; }
-            const int code = (int)(w & 7ull);
+            code = (int)(w & 7ull);
             w >>= 3; --nrem;
             if (code == G.cls) {
                 ++r; row_cnt = 0;
                 if (r >= r_end) { ok = false; break; }
                 nb = plan_nbase(G, r); zb = plan_zbase(G, r);
                 if ((r / SLAB) != cur_slab) {
-                    my_cnt[(size_t)cur_slab * GROUP] = (uint8_t)slab_cnt;
-                    max_cnt = max(max_cnt, slab_cnt);
-                    cur_slab = r / SLAB; slab_cnt = 0;
+                    if (k % CODES_PER_WORD != 0) out[((size_t)cur_slab * G.wps + k / CODES_PER_WORD) * GROUP] = acc;
+                    my_cnt[(size_t)cur_slab * GROUP] = (uint8_t)k;
+                    cur_slab = r / SLAB; k = 0; acc = ~0ull;
                 }
             } else if (code == (G.cls ^ 1) || code >= 6) { ok = false; break; }
             else if (code >= 4) z += (code & 1) ? -1 : 1;
             else n += (code == mw.n_plus) ? 1 : -1;
         }
-        if ((unsigned)(n - nb) >= (unsigned)WIN_N || (unsigned)(z - zb) >= (unsigned)WIN_Z || ++row_cnt > MAX_ROW_VISITS) { ok = false; break; }
-        ++slab_cnt;
+        if ((unsigned)(n - nb) >= (unsigned)WIN_N || (unsigned)(z - zb) >= (unsigned)WIN_Z || ++row_cnt > MAX_ROW_VISITS || k >= slab_cap) { ok = false; break; }
         on_lo = min(on_lo, n - nb); on_hi = max(on_hi, n - nb); oz_lo = min(oz_lo, z - zb); oz_hi = max(oz_hi, z - zb);
+        acc ^= (unsigned long long)(7 ^ code) << (3 * (k % CODES_PER_WORD));
+        if (++k % CODES_PER_WORD == 0) { out[((size_t)cur_slab * G.wps + k / CODES_PER_WORD - 1) * GROUP] = acc; acc = ~0ull; }
     }
     if (ok) {
+        if (k % CODES_PER_WORD != 0) out[((size_t)cur_slab * G.wps + k / CODES_PER_WORD) * GROUP] = acc;
+        my_cnt[(size_t)cur_slab * GROUP] = (uint8_t)k;
         // widen the group's visited extent (the plain read only filters out the atomics that cannot change anything)
         PlanGroup* Gp = groups + blockIdx.x;
         if (on_lo < *(volatile int32_t*)&Gp->dn_lo) atomicMin(&Gp->dn_lo, on_lo);
         if (on_hi > *(volatile int32_t*)&Gp->dn_hi) atomicMax(&Gp->dn_hi, on_hi);
         if (oz_lo < *(volatile int32_t*)&Gp->dz_lo) atomicMin(&Gp->dz_lo, oz_lo);
         if (oz_hi > *(volatile int32_t*)&Gp->dz_hi) atomicMax(&Gp->dz_hi, oz_hi);
-        my_cnt[(size_t)cur_slab * GROUP] = (uint8_t)slab_cnt;
-        max_cnt = max(max_cnt, slab_cnt);
         p0_out[mw.pos] = p0;
         pflag[mw.pos] = 1;
-        atomicMax(&groups[blockIdx.x].wps, max_cnt);      // visits; turned into words per slab by k_plan_stream_len
     } else {
-        for (int s = 0; s < G.nslab; ++s) my_cnt[(size_t)s * GROUP] = 0;
+        // take back what was written: the thread's words of the slabs it reached are pads again, its counts zero
+        const int last = min(cur_slab, G.nslab - 1);
+        for (int s = max(first_slab, 0); s <= last; ++s) {
+            for (int wi = 0; wi < G.wps; ++wi) out[((size_t)s * G.wps + wi) * GROUP] = ~0ull;
+            my_cnt[(size_t)s * GROUP] = 0;
+        }
         pflag[mw.pos] = 0;
         const uint64_t t = (uint64_t)mw.i / (uint64_t)block_size;
         const uint32_t slot = atomicAdd(direct_count + t, 1u);
@@ -271,53 +292,9 @@ k_plan_verify(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, 
     }
 }
 
-__global__ void k_plan_stream_len(int64_t n_groups, PlanGroup* __restrict__ groups, uint32_t* __restrict__ len) {
-    const int64_t gi = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (gi >= n_groups) return;
-    const int max_cnt = groups[gi].wps;
-    const int wps = max_cnt > 0 ? (max_cnt + CODES_PER_WORD - 1) / CODES_PER_WORD : 0;
-    groups[gi].wps = wps;
-    len[gi] = (uint32_t)(groups[gi].nslab * wps * GROUP);
-}
-
 __global__ void k_plan_stream_off(const uint64_t* __restrict__ off, int64_t n_groups, PlanGroup* __restrict__ groups) {
     const int64_t gi = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (gi < n_groups) groups[gi].stream_off = off[gi];
-}
-
-// second walk of the verified members: re-emit the codes slab by slab, 21 per word, words [slab][w][thread] (the
-// stream is pre-filled with pad codes).  The first visit becomes PLAN_CODE_FIRST.
-__global__ void __launch_bounds__(GROUP)
-k_plan_emit(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, const int32_t* __restrict__ start,
-            const uint64_t* __restrict__ code_off, const ulonglong2* __restrict__ codes, const uint32_t* __restrict__ perm,
-            const PlanGroup* __restrict__ groups, const uint8_t* __restrict__ pflag, unsigned long long* __restrict__ stream) {
-    const PlanGroup G = groups[blockIdx.x];
-    MemberWalk mw;
-    if (G.cls == 7 || G.wps == 0) return;
-    if (!member_init(g, G, N, start, code_off, codes, perm, mw)) return;
-    if (!pflag[mw.pos]) return;
-    unsigned long long* out = stream + G.stream_off + threadIdx.x;
-    int r = mw.r, cur_slab = r / SLAB, k = 0;                 // k = codes emitted in the current slab
-    unsigned long long w = 0, acc = ~0ull;
-    int nrem = 0;
-    for (uint32_t v = 0; v < mw.n_vis; ++v) {
-        int code = PLAN_CODE_FIRST;
-        if (v > 0) {
-            if (nrem == 0) { w = __ldg(mw.cp++); nrem = CODES_PER_WORD; }
-            code = (int)(w & 7ull);
-            w >>= 3; --nrem;
-            if (code == G.cls) {
-                ++r;
-                if ((r / SLAB) != cur_slab) {
-                    if (k % CODES_PER_WORD != 0) out[((size_t)cur_slab * G.wps + k / CODES_PER_WORD) * GROUP] = acc;
-                    cur_slab = r / SLAB; k = 0; acc = ~0ull;
-                }
-            }
-        }
-        acc ^= (unsigned long long)(7 ^ code) << (3 * (k % CODES_PER_WORD));
-        if (++k % CODES_PER_WORD == 0) { out[((size_t)cur_slab * G.wps + k / CODES_PER_WORD - 1) * GROUP] = acc; acc = ~0ull; }
-    }
-    if (k % CODES_PER_WORD != 0) out[((size_t)cur_slab * G.wps + k / CODES_PER_WORD) * GROUP] = acc;
 }
 
 // launch order of a block's groups: key = (block, -work), work = slabs x words per slab x members
@@ -388,11 +365,11 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     plan->perm = nullptr; plan->p0 = nullptr; plan->pflag = nullptr; plan->cnt = nullptr; plan->groups = nullptr;
     plan->direct_list = nullptr; plan->d_direct_count = nullptr; plan->stream = nullptr; plan->stream_words = 0; plan->launch_order = nullptr;
     uint64_t *keysA = nullptr, *keysB = nullptr, *cnt_off = nullptr;
-    uint32_t *valsA = nullptr, *valsB = nullptr, *cnt_len = nullptr;
+    uint32_t *valsA = nullptr, *valsB = nullptr, *cnt_len = nullptr, *stream_len = nullptr;
     void* tmp = nullptr;
     int64_t* d_group_begin = nullptr;
     auto fail = [&](int code) {
-        cache_free(keysA); cache_free(keysB); cache_free(valsA); cache_free(valsB); cache_free(tmp); cache_free(cnt_off); cache_free(cnt_len);
+        cache_free(keysA); cache_free(keysB); cache_free(valsA); cache_free(valsB); cache_free(tmp); cache_free(cnt_off); cache_free(cnt_len); cache_free(stream_len);
         cache_free(d_group_begin);
         free_solve_plan(plan);
         return code;
@@ -450,54 +427,45 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     PLAN_CUDA(cache_alloc((void**)&plan->groups, sizeof(PlanGroup) * (size_t)(n_groups + 1)));
     PLAN_CUDA(cache_alloc((void**)&d_group_begin, sizeof(int64_t) * (size_t)(n_blocks + 1)));
     PLAN_CUDA(cache_alloc((void**)&cnt_len, sizeof(uint32_t) * (size_t)n_groups));
+    PLAN_CUDA(cache_alloc((void**)&stream_len, sizeof(uint32_t) * (size_t)n_groups));
     PLAN_CUDA(cache_alloc((void**)&cnt_off, sizeof(uint64_t) * (size_t)n_groups));
     lap("heads + scan");
     k_plan_starts<<<nb256, 256, 0, st>>>(keys, head, gid, m, plan->groups, d_group_begin);
-    k_plan_params<<<(unsigned)n_groups, 256, 0, st>>>(ctx->cfg, P->start, P->end, plan->perm, m, (int64_t)n_groups, plan->groups, cnt_len);
+    k_plan_params<<<(unsigned)n_groups, 256, 0, st>>>(ctx->cfg, P->start, P->end, plan->perm, m, (int64_t)n_groups, plan->groups, cnt_len, stream_len);
     ctx->launches += 2;
     PLAN_CUDA(cudaGetLastError());
+    // offsets of every group's visit-count table and of its slab-aligned code stream: both sizes are known before the walk
+    unsigned long long cnt_bytes = 0, stream_words = 0;
     if ((rc = launch_scan_u32(ctx, cnt_len, cnt_off, (int64_t)n_groups, 0, ctx->d_total, st)) != PCT_OK) return fail(rc);
-    unsigned long long cnt_bytes = 0;
     PLAN_CUDA(cudaMemcpyAsync(&cnt_bytes, ctx->d_total, sizeof(cnt_bytes), cudaMemcpyDeviceToHost, st));
-    PLAN_CUDA(cudaStreamSynchronize(st));
-    plan->cnt_bytes = (int64_t)cnt_bytes;
     k_plan_cnt_off<<<(unsigned)((n_groups + 255) / 256), 256, 0, st>>>(cnt_off, (int64_t)n_groups, plan->groups);
-    ++ctx->launches;
+    PLAN_CUDA(cudaStreamSynchronize(st));
+    if ((rc = launch_scan_u32(ctx, stream_len, cnt_off, (int64_t)n_groups, 0, ctx->d_total, st)) != PCT_OK) return fail(rc);
+    PLAN_CUDA(cudaMemcpyAsync(&stream_words, ctx->d_total, sizeof(stream_words), cudaMemcpyDeviceToHost, st));
+    k_plan_stream_off<<<(unsigned)((n_groups + 255) / 256), 256, 0, st>>>(cnt_off, (int64_t)n_groups, plan->groups);
+    ctx->launches += 2;
     // the sort buffers are no longer needed once the group table is complete
     PLAN_CUDA(cudaStreamSynchronize(st));
+    plan->cnt_bytes = (int64_t)cnt_bytes;
+    plan->stream_words = (int64_t)stream_words;
     cache_free(keysA); cache_free(keysB); cache_free(valsA); cache_free(valsB); cache_free(tmp);
     keysA = keysB = nullptr; valsA = valsB = nullptr; tmp = nullptr;
-    lap("starts + params + cnt scan");
+    lap("starts + params + scans");
     PLAN_CUDA(cache_alloc((void**)&plan->cnt, cnt_bytes > 0 ? (size_t)cnt_bytes : 16));
     PLAN_CUDA(cudaMemsetAsync(plan->cnt, 0, cnt_bytes > 0 ? (size_t)cnt_bytes : 16, st));
+    PLAN_CUDA(cache_alloc((void**)&plan->stream, stream_words > 0 ? 8 * (size_t)stream_words : 16));
+    PLAN_CUDA(cudaMemsetAsync(plan->stream, 0xFF, stream_words > 0 ? 8 * (size_t)stream_words : 16, st));
     PLAN_CUDA(cache_alloc((void**)&plan->p0, 4 * mm));
     PLAN_CUDA(cache_alloc((void**)&plan->pflag, mm));
     PLAN_CUDA(cache_alloc((void**)&plan->direct_list, 4 * mm));
     PLAN_CUDA(cache_alloc((void**)&plan->d_direct_count, sizeof(uint32_t) * (size_t)n_blocks));
     PLAN_CUDA(cudaMemsetAsync(plan->d_direct_count, 0, sizeof(uint32_t) * (size_t)n_blocks, st));
-    lap("allocs before verify");
-    k_plan_verify<<<(unsigned)n_groups, GROUP, 0, st>>>(ctx->cfg, P->N, P->start, P->code_off, P->codes, plan->perm, plan->groups,
-                                                       block_size, plan->p0, plan->pflag, plan->cnt, plan->direct_list,
-                                                       plan->d_direct_count);
+    lap("allocs + memsets");
+    k_plan_walk<<<(unsigned)n_groups, GROUP, 0, st>>>(ctx->cfg, P->N, P->start, P->code_off, P->codes, plan->perm, plan->groups, block_size,
+                                                     plan->p0, plan->pflag, plan->cnt, plan->stream, plan->direct_list, plan->d_direct_count);
     ++ctx->launches;
     PLAN_CUDA(cudaGetLastError());
-    lap("verify");
-    // slab-aligned code stream of the verified members
-    k_plan_stream_len<<<(unsigned)((n_groups + 255) / 256), 256, 0, st>>>((int64_t)n_groups, plan->groups, cnt_len);
-    if ((rc = launch_scan_u32(ctx, cnt_len, cnt_off, (int64_t)n_groups, 0, ctx->d_total, st)) != PCT_OK) return fail(rc);
-    unsigned long long stream_words = 0;
-    PLAN_CUDA(cudaMemcpyAsync(&stream_words, ctx->d_total, sizeof(stream_words), cudaMemcpyDeviceToHost, st));
-    PLAN_CUDA(cudaStreamSynchronize(st));
-    plan->stream_words = (int64_t)stream_words;
-    PLAN_CUDA(cache_alloc((void**)&plan->stream, stream_words > 0 ? 8 * (size_t)stream_words : 16));
-    PLAN_CUDA(cudaMemsetAsync(plan->stream, 0xFF, stream_words > 0 ? 8 * (size_t)stream_words : 16, st));
-    k_plan_stream_off<<<(unsigned)((n_groups + 255) / 256), 256, 0, st>>>(cnt_off, (int64_t)n_groups, plan->groups);
-    lap("stream alloc + memset");
-    k_plan_emit<<<(unsigned)n_groups, GROUP, 0, st>>>(ctx->cfg, P->N, P->start, P->code_off, P->codes, plan->perm, plan->groups,
-                                                     plan->pflag, plan->stream);
-    ctx->launches += 3;
-    PLAN_CUDA(cudaGetLastError());
-    lap("emit");
+    lap("walk (verify + emit)");
     {   // longest-first launch order inside every block
         uint64_t *wk0 = nullptr, *wk1 = nullptr;
         uint32_t *wv0 = nullptr, *wv1 = nullptr;
@@ -546,7 +514,7 @@ int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaS
     PLAN_CUDA(cudaStreamSynchronize(st));
     plan->group_begin[(size_t)n_blocks] = (int64_t)n_groups;
     for (uint32_t c : plan->direct_count) plan->n_direct += c;
-    cache_free(cnt_off); cache_free(cnt_len); cache_free(d_group_begin);
+    cache_free(cnt_off); cache_free(cnt_len); cache_free(stream_len); cache_free(d_group_begin);
 #undef PLAN_CUDA
     *out = plan;
     return PCT_OK;
