@@ -220,14 +220,16 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
     float S = 0.f;
     stage(0);
     unsigned long long w_next = __ldg(my_stream);
+    int c_next = (int)__ldg(my_cnt);              // visits in the slab; 0 for threads without a (windowed) history
     for (int s = 0; s < G.nslab; ++s) {
-        const int c = (int)my_cnt[(size_t)s * GROUP];       // 0 for threads without a (windowed) history
+        const int c = c_next;
         const unsigned long long w0 = w_next;
         cp_async_wait_all();
         __syncthreads();                          // slab s is staged; slab s - 1 is walked (and tbl is visible)
-        if (s + 1 < G.nslab) {
+        if (s + 1 < G.nslab) {                    // the next slab's x window, first word and count are on their way during the walk
             stage(s + 1);
             w_next = __ldg(my_stream + (size_t)(s + 1) * G.wps * GROUP);
+            c_next = (int)__ldg(my_cnt + (size_t)(s + 1) * GROUP);
         }
         const int cmax = __reduce_max_sync(0xffffffffu, c);
         if (s > 0) p += (s & 1) ? 0x8000u : 0xFFFF8000u;          // switch to the other x buffer (the fields sit below bit 15)
@@ -283,11 +285,14 @@ k_block_windowed(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ 
     // ---- pass 2: {Delta, s} += {c_i, 1} on every visit; flush per slab -------------------------------------------------
     p = win_s + p_init + (COUNT ? 0u : (unsigned)(tid & 1) * (WIN_SLOTS * 4));     // odd lanes: second Delta copy
     w_next = __ldg(my_stream);
+    c_next = (int)__ldg(my_cnt);
     for (int s = 0; s < G.nslab; ++s) {
-        const int c = (int)my_cnt[(size_t)s * GROUP];
-        const int cmax = __reduce_max_sync(0xffffffffu, c);
+        const int cmax = __reduce_max_sync(0xffffffffu, c_next);
         const unsigned long long w0 = w_next;
-        if (s + 1 < G.nslab) w_next = __ldg(my_stream + (size_t)(s + 1) * G.wps * GROUP);
+        if (s + 1 < G.nslab) {
+            w_next = __ldg(my_stream + (size_t)(s + 1) * G.wps * GROUP);
+            c_next = (int)__ldg(my_cnt + (size_t)(s + 1) * GROUP);
+        }
         if (COUNT) {
             walk_slab(my_stream + (size_t)s * G.wps * GROUP, w0, cmax, tbl_s, p, [&](unsigned q) {
                 const unsigned a = win_addr(q);
