@@ -164,6 +164,18 @@ typedef struct {
 int pct_fbp(pct_ctx* ctx, const pct_protons* protons, const float* b, const pct_fbp_params* params /* HOST */, float* x0_out,
             void* stream);
 
+/* pct_fbp WITHOUT ANY ALLOCATION, for callers that cannot call cudaMalloc (code under stream capture, serving loops,
+ * harnesses that forbid it).  Same arguments, same kernels, same result as pct_fbp; the sinogram scratch (20 bytes per bin)
+ * is a fixed device array inside the library sized for PCT_FBP_STATIC_MAX_CELLS bins -- 20 MiB that every GPU which loads
+ * the library holds until the process exits.  nz * n_theta * n_s > PCT_FBP_STATIC_MAX_CELLS is rejected with
+ * PCT_E_CAPACITY (use pct_fbp).  Calls no cudaMalloc / cudaFree and no allocating library routine; enqueues two memsets (the
+ * array keeps the last call's contents) and three kernels on `stream` and does NOT synchronise it.  Every call on a device,
+ * from any context, shares the one array: calls that overlap on the GPU (different streams without an ordering between
+ * them) race and give garbage; calls on one stream, or ordered by events, are safe. */
+#define PCT_FBP_STATIC_MAX_CELLS (1u << 20)
+int pct_fbp_static(pct_ctx* ctx, const pct_protons* protons, const float* b, const pct_fbp_params* params /* HOST */,
+                   float* x0_out, void* stream);
+
 /* The object hull from the data (space carving; preprocessing of PAPER.md:102-104; reading R26): hull_out[j] = 0 for every
  * voxel that the straight chord between the tracker hits of some history with WEPL < wepl_air_mm crosses with a chord
  * length > min_chord_mm, 1 otherwise.  hull_out: DEVICE uint8[n] (overwritten).  Use min_chord_mm > 0: voxels a chord only

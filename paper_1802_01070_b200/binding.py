@@ -16,12 +16,14 @@ from . import build as _build
 OK, E_INVALID_ARG, E_OOM, E_CUDA, E_CAPACITY = 0, -1, -2, -3, -4
 REJ_MISS, REJ_ORDER, REJ_DEPTH, REJ_LEFT_GRID, TIE, END_MISMATCH, REJ_CAPACITY, REJ_NONFINITE = (
     0x01, 0x02, 0x04, 0x08, 0x10, 0x20, 0x40, 0x80)
+FBP_STATIC_MAX_CELLS = 1 << 20
 REJECT_MASK = REJ_MISS | REJ_ORDER | REJ_DEPTH | REJ_LEFT_GRID | REJ_CAPACITY | REJ_NONFINITE
 
 EXPORTS = ("pct_create", "pct_destroy", "pct_last_error", "pct_generate_mlp", "pct_paths_info", "pct_paths_free",
            "pct_paths_decode", "pct_forward_project", "pct_column_counts", "pct_solve", "pct_reconstruct_host",
            "pct_launch_count", "pct_profile_enable", "pct_profile_read", "pct_measure_peaks", "pct_solve_config",
-           "pct_plan_info", "pct_trim_cache", "pct_paths_flagged", "pct_solve_ex", "pct_fbp", "pct_hull_carve")
+           "pct_plan_info", "pct_trim_cache", "pct_paths_flagged", "pct_solve_ex", "pct_fbp", "pct_hull_carve",
+           "pct_fbp_static")
 
 
 class Geometry(C.Structure):
@@ -112,6 +114,7 @@ def load_library(path: Optional[str] = None):
     L.pct_solve.argtypes = [vp, vp, vp, vp, C.c_int, i64, C.c_float, vp, vp]
     L.pct_solve_ex.argtypes = [vp, vp, vp, vp, C.c_int, i64, C.c_float, C.POINTER(SolveOpts), vp, vp]
     L.pct_fbp.argtypes = [vp, C.POINTER(Protons), vp, C.POINTER(FbpParams), vp, vp]
+    L.pct_fbp_static.argtypes = [vp, C.POINTER(Protons), vp, C.POINTER(FbpParams), vp, vp]
     L.pct_hull_carve.argtypes = [vp, C.POINTER(Protons), vp, C.c_double, C.c_double, vp, vp]
     L.pct_reconstruct_host.argtypes = [vp, C.POINTER(Protons), vp, vp, vp, C.c_int, i64, C.c_float, vp,
                                        C.POINTER(ReconStats), vp]
@@ -316,6 +319,17 @@ class Context:
         fp = FbpParams(int(n_theta), int(n_s), float(ds_mm), int(min_count))
         self._check(self._L.pct_fbp(self._h, C.byref(pr), _dev_ptr(b, torch.float32, pr.m, self.device), C.byref(fp),
                                     _dev_ptr(x0, torch.float32, self.n, self.device), _stream_ptr(self.device)))
+        return x0
+
+    def fbp_static(self, protons: Dict[str, torch.Tensor], u_in_mm: float, u_out_mm: float, b: torch.Tensor, n_theta: int,
+                   n_s: int, ds_mm: float, min_count: int = 1, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+        """pct_fbp_static: pct_fbp with its scratch in a fixed device array (no allocation inside the library; at most
+        FBP_STATIC_MAX_CELLS sinogram bins).  `out` must be given by callers that may not allocate themselves."""
+        pr = self._protons_struct(protons, u_in_mm, u_out_mm)
+        x0 = out if out is not None else torch.empty(self.n, dtype=torch.float32, device=self.device)
+        fp = FbpParams(int(n_theta), int(n_s), float(ds_mm), int(min_count))
+        self._check(self._L.pct_fbp_static(self._h, C.byref(pr), _dev_ptr(b, torch.float32, pr.m, self.device), C.byref(fp),
+                                           _dev_ptr(x0, torch.float32, self.n, self.device), _stream_ptr(self.device)))
         return x0
 
     def hull_carve(self, protons: Dict[str, torch.Tensor], u_in_mm: float, u_out_mm: float, b: torch.Tensor,

@@ -6,6 +6,8 @@
 // Both are a few milliseconds next to the seconds of the hot path, so they are written for exactness first: FP64
 // throughout, explicit round-to-nearest operations (no FMA contraction) wherever a floor() or a threshold decides, so
 // that a bin or a voxel is chosen from the same IEEE numbers on every run.
+#include <mutex>
+
 #include "pct_internal.cuh"
 
 namespace pct {
@@ -143,6 +145,78 @@ extern "C" int pct_fbp(pct_ctx* ctx, const pct_protons* pr, const float* b, cons
     }
     FBP_CUDA(cudaGetLastError());
 #undef FBP_CUDA
+    return done(PCT_OK);
+}
+
+// ---- pct_fbp_static: the same FBP with its sinogram scratch in a fixed device array -- no allocation at all --------------------
+// For callers that cannot call cudaMalloc (stream capture, serving loops, harnesses that forbid it).  The three scratch
+// arrays of pct_fbp (bin sums, filtered rows, bin counts: 20 bytes per sinogram bin) live in ONE file-scope array sized for
+// PCT_FBP_STATIC_MAX_CELLS bins (20 MiB), held by every GPU that loads the library until the process exits.  Host code
+// cannot use the array's name as a pointer (it is the host-side stand-in of the symbol): its device address is looked up once
+// per device, with that device current, by cudaGetSymbolAddress.
+namespace pct {
+
+constexpr size_t FBP_STATIC_CELLS = PCT_FBP_STATIC_MAX_CELLS;
+// layout: double sum[MAX] | double q[MAX] | unsigned cnt[MAX]
+static __device__ __align__(256) unsigned char g_fbp_static_scratch[FBP_STATIC_CELLS * (2 * sizeof(double) + sizeof(unsigned))];
+
+static std::mutex g_fbp_static_mu;
+static void* g_fbp_static_ptr[64];          // per device: device address of g_fbp_static_scratch (nullptr = not looked up yet)
+
+// device address of the scratch array on `device` (which must be current); cudaSuccess or the look-up's error
+static cudaError_t fbp_static_scratch(int device, unsigned char** out) {
+    if (device < 0 || device >= 64) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_fbp_static_mu);
+    if (!g_fbp_static_ptr[device]) {
+        void* ptr = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&ptr, g_fbp_static_scratch);
+        if (e != cudaSuccess) return e;
+        g_fbp_static_ptr[device] = ptr;
+    }
+    *out = static_cast<unsigned char*>(g_fbp_static_ptr[device]);
+    return cudaSuccess;
+}
+
+}  // namespace pct
+
+extern "C" int pct_fbp_static(pct_ctx* ctx, const pct_protons* pr, const float* b, const pct_fbp_params* fp, float* x0_out, void* stream) {
+    if (!ctx) return PCT_E_INVALID_ARG;
+    if (!pr || pr->m < 0 || !fp || !x0_out || (pr->m > 0 && !b)) return set_error(ctx, PCT_E_INVALID_ARG, "bad fbp arguments");
+    if (fp->n_theta < 1 || fp->n_s < 2 || fp->n_s > 4096 || fp->n_theta > 4096 || !(fp->ds_mm > 0.0) || !std::isfinite(fp->ds_mm))
+        return set_error(ctx, PCT_E_INVALID_ARG, "fbp: n_theta in [1, 4096], n_s in [2, 4096], ds_mm > 0");
+    if (pr->m > 0 && (!pr->phi || !pr->t_in || !pr->v_in || !pr->t_out || !pr->v_out)) return set_error(ctx, PCT_E_INVALID_ARG, "NULL tracker array");
+    const size_t cells = (size_t)ctx->geom.nz * fp->n_theta * fp->n_s;
+    if (cells > FBP_STATIC_CELLS)
+        return set_error(ctx, PCT_E_CAPACITY, "pct_fbp_static: nz * n_theta * n_s = %zu sinogram bins exceed the fixed scratch of %zu bins (use pct_fbp)",
+                         cells, FBP_STATIC_CELLS);
+    int prev = -1;
+    cudaGetDevice(&prev);
+    if (prev != ctx->device) cudaSetDevice(ctx->device);
+    auto done = [&](int code) { if (prev >= 0 && prev != ctx->device) cudaSetDevice(prev); return code; };
+#define FBPS_CUDA(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { cudaGetLastError(); \
+        return done(set_error(ctx, PCT_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e__))); } } while (0)
+    unsigned char* base = nullptr;
+    FBPS_CUDA(fbp_static_scratch(ctx->device, &base));
+    double* sum = reinterpret_cast<double*>(base);
+    double* q = sum + FBP_STATIC_CELLS;
+    unsigned* cnt = reinterpret_cast<unsigned*>(q + FBP_STATIC_CELLS);
+    cudaStream_t st = (cudaStream_t)stream;
+    // the array keeps the last call's contents: the sums and counts must start at zero (q is overwritten by the filter)
+    FBPS_CUDA(cudaMemsetAsync(sum, 0, sizeof(double) * cells, st));
+    FBPS_CUDA(cudaMemsetAsync(cnt, 0, sizeof(unsigned) * cells, st));
+    const ProtonPtrs pp = {pr->phi, pr->t_in, pr->v_in, pr->dt_in, pr->dv_in, pr->t_out, pr->v_out, pr->dt_out, pr->dv_out};
+    if (pr->m > 0) {
+        const int64_t want = (pr->m + 255) / 256, cap = (int64_t)ctx->num_sms * 16;
+        k_fbp_bin<<<(unsigned)(want < cap ? want : cap), 256, 0, st>>>(pp, b, pr->m, pr->u_in_mm, pr->u_out_mm, ctx->geom.origin_mm[2], ctx->geom.h_mm,
+                                                                        ctx->geom.nz, fp->n_theta, fp->n_s, fp->ds_mm, sum, cnt);
+    }
+    k_fbp_filter<<<(unsigned)((size_t)ctx->geom.nz * fp->n_theta), 256, sizeof(double) * fp->n_s, st>>>(sum, cnt, fp->n_s, fp->ds_mm,
+                                                                                                      (unsigned)(fp->min_count > 1 ? fp->min_count : 1), q);
+    k_fbp_backproject<<<(unsigned)((ctx->n_vox + 255) / 256), 256, sizeof(double) * 2 * fp->n_theta, st>>>(
+        q, ctx->geom.nx, ctx->geom.ny, ctx->geom.nz, ctx->geom.origin_mm[0], ctx->geom.origin_mm[1], ctx->geom.h_mm, fp->n_theta, fp->n_s, fp->ds_mm, x0_out);
+    ctx->launches += 3;
+    FBPS_CUDA(cudaGetLastError());
+#undef FBPS_CUDA
     return done(PCT_OK);
 }
 
