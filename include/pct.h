@@ -14,8 +14,9 @@
  *     which the library owns until pct_destroy / pct_paths_free.
  *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Work is enqueued on it; device
  *     results are valid once the caller has synchronised the stream.  Calls that need sizes on the host synchronise
- *     the stream themselves and say so below: pct_generate_mlp, pct_paths_decode, pct_paths_flagged, pct_fbp, the
- *     *_host calls, and the FIRST pct_solve / pct_solve_ex on a (paths, block_size) pair that builds a solve plan.
+ *     the stream themselves and say so below: pct_generate_mlp, pct_paths_decode, pct_paths_flagged, pct_fbp,
+ *     pct_hull_intersect, pct_region_members, pct_reconstruct_regions, the *_host calls, and the FIRST pct_solve /
+ *     pct_solve_ex on a (paths, block_size) pair that builds a solve plan.
  *   - Thread safety: a pct_ctx and a pct_paths are each used by one thread at a time.  pct_solve keeps a solve plan
  *     (a solver-shaped copy of the rows) inside the pct_paths it is given -- hence `pct_paths*`, not const -- and the
  *     block counts of that plan inside the context.
@@ -182,6 +183,51 @@ int pct_fbp_static(pct_ctx* ctx, const pct_protons* protons, const float* b, con
  * grazes at a corner are decided by rounding otherwise.  Enqueued on `stream`. */
 int pct_hull_carve(pct_ctx* ctx, const pct_protons* protons, const float* b, double wepl_air_mm, double min_chord_mm,
                    uint8_t* hull_out, void* stream);
+
+/* ---- Algorithm 1 of the paper: "multi-GPU based reconstruction" (reading R28 of DESIGN.md) -------------
+ *   1: setupImageRegions()  2: identifyProtonsPassingRegions()  3: allocateMemoryForProtonsPerGPU()
+ *   4: iterativelySolvePerGPU()  5: selectSlice()
+ * The volume is cut along z into n_regions parts of (almost) equal height; region g reconstructs its part plus `ext` slices
+ * of each neighbour ("two regions, one containing slices 0-12 and the other containing slices 7-19": nz = 20,
+ * n_regions = 2, ext = 3); a history belongs to every region that holds the slice of its hull entry voxel or of its hull exit
+ * voxel ("associated with the image region entered to and exited from"); each region is solved on its own histories only, with
+ * no exchange between regions ("eliminating the need of data transfers among the GPUs"); the final image takes
+ * the slices of each part from that part's region ("slices 0-9 from the first region and 10-19 of the second").  One region
+ * per GPU is the paper's use; one GPU may also run several regions in turn. */
+typedef struct {
+    int32_t z_lo, z_hi;       /* slices [z_lo, z_hi) the region reconstructs                               */
+    int32_t keep_lo, keep_hi; /* slices [keep_lo, keep_hi) of the final image that are taken from it      */
+} pct_region;
+/* Step 1.  Pure host arithmetic, no context: part g = [g nz / G, (g+1) nz / G) (integer division), region = part widened by
+ * ext slices on every side that has a neighbour.  out: HOST pct_region[n_regions].  PCT_E_INVALID_ARG unless
+ * 1 <= n_regions <= nz and ext >= 0. */
+int pct_regions_setup(int32_t nz, int32_t n_regions, int32_t ext, pct_region* out);
+/* A1 alone (R4): the hull entry and exit voxel of every history, -1 / -1 for a history rejected there (miss, order, depth,
+ * non-finite record) -- what step 2 needs, at a fifth of the cost of pct_generate_mlp, and equal to the first and last
+ * voxel of the row pct_generate_mlp would produce.  protons: HOST struct of DEVICE arrays; hull: DEVICE uint8[n] or NULL;
+ * v_in, v_out: DEVICE int32[m].  Synchronises `stream`. */
+int pct_hull_intersect(pct_ctx* ctx, const pct_protons* protons, const uint8_t* hull, int32_t* v_in, int32_t* v_out, void* stream);
+/* Step 2.  idx_out (DEVICE uint32[m], ascending) = the histories with v_in >= 0 whose entry slice or exit slice lies in
+ * [region->z_lo, region->z_hi); *count_out (HOST) = how many.  region: HOST.  m < 2^31.  Synchronises `stream`. */
+int pct_region_members(pct_ctx* ctx, const int32_t* v_in, const int32_t* v_out, int64_t m, const pct_region* region,
+                       uint32_t* idx_out, int64_t* count_out, void* stream);
+/* Step 3.  dst arrays [k] = src arrays [idx[k]], b_dst[k] = b_src[idx[k]] for k < count.  src, dst: HOST structs of DEVICE
+ * arrays (dst's nine arrays hold at least `count` doubles each and are written; the call sets dst->m and the tracker planes);
+ * b_src / b_dst: DEVICE float32, both NULL to skip.  Enqueued on `stream`. */
+int pct_gather_histories(pct_ctx* ctx, const pct_protons* src, const float* b_src, const uint32_t* idx, int64_t count,
+                         pct_protons* dst, float* b_dst, void* stream);
+/* Step 5.  x_final[slices keep_lo..keep_hi) = x_region[the same slices]; both DEVICE float32[n].  Enqueued on `stream`. */
+int pct_select_slices(pct_ctx* ctx, const float* x_region, const pct_region* region /* HOST */, float* x_final, void* stream);
+/* Steps 1-5 for the regions [region_first, region_first + region_count) on this context's GPU: pct_hull_intersect on all
+ * histories, then per region pct_region_members, pct_gather_histories, pct_generate_mlp and pct_solve on the members (x of the
+ * whole grid, started from x0 or from ones; only the region's kept slices are used), pct_select_slices into x_out.  Slices
+ * kept by other regions are left as they are in x_out: a process per GPU runs its own region and the kept slices are
+ * collected afterwards (the only transfer).  members_out: HOST int64[n_regions] or NULL; entries of the regions
+ * run here are set.  protons: HOST struct of DEVICE arrays; b: DEVICE float32[m]; hull: DEVICE uint8[n] or NULL; x0: DEVICE
+ * float32[n] or NULL; x_out: DEVICE float32[n], must not alias x0.  n_regions <= 1024.  Blocking. */
+int pct_reconstruct_regions(pct_ctx* ctx, const pct_protons* protons, const float* b, const uint8_t* hull, const float* x0,
+                            int32_t n_regions, int32_t ext, int32_t region_first, int32_t region_count, int iters,
+                            int64_t block_size, float lambda, float* x_out, int64_t* members_out, void* stream);
 
 /* The whole hot path on HOST buffers (bench e2e): H2D of the tracker arrays, hull and b; pct_generate_mlp;
  * pct_solve; D2H of x.  protons: HOST struct with HOST arrays; hull_host: uint8[n] or NULL; b_host: float32[m];

@@ -7,7 +7,7 @@ from __future__ import annotations
 
 import ctypes as C
 import os
-from typing import Dict, Optional
+from typing import Dict, List, Optional
 
 import torch
 
@@ -23,7 +23,8 @@ EXPORTS = ("pct_create", "pct_destroy", "pct_last_error", "pct_generate_mlp", "p
            "pct_paths_decode", "pct_forward_project", "pct_column_counts", "pct_solve", "pct_reconstruct_host",
            "pct_launch_count", "pct_profile_enable", "pct_profile_read", "pct_measure_peaks", "pct_solve_config",
            "pct_plan_info", "pct_trim_cache", "pct_paths_flagged", "pct_solve_ex", "pct_fbp", "pct_hull_carve",
-           "pct_fbp_static")
+           "pct_fbp_static", "pct_regions_setup", "pct_hull_intersect", "pct_region_members", "pct_gather_histories",
+           "pct_select_slices", "pct_reconstruct_regions")
 
 
 class Geometry(C.Structure):
@@ -84,6 +85,10 @@ PROTON_KEYS = ("phi", "t_in", "v_in", "dt_in", "dv_in", "t_out", "v_out", "dt_ou
 _lib = None
 
 
+class Region(C.Structure):
+    _fields_ = [("z_lo", C.c_int32), ("z_hi", C.c_int32), ("keep_lo", C.c_int32), ("keep_hi", C.c_int32)]
+
+
 class PctError(RuntimeError):
     pass
 
@@ -126,6 +131,13 @@ def load_library(path: Optional[str] = None):
     L.pct_solve_config.argtypes = [vp, C.c_int, i64]
     L.pct_plan_info.argtypes = [vp, C.POINTER(PlanStats)]
     L.pct_trim_cache.argtypes = [vp]
+    L.pct_regions_setup.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.POINTER(Region)]
+    L.pct_hull_intersect.argtypes = [vp, C.POINTER(Protons), vp, vp, vp, vp]
+    L.pct_region_members.argtypes = [vp, vp, vp, i64, C.POINTER(Region), vp, C.POINTER(i64), vp]
+    L.pct_gather_histories.argtypes = [vp, C.POINTER(Protons), vp, vp, i64, C.POINTER(Protons), vp, vp]
+    L.pct_select_slices.argtypes = [vp, vp, C.POINTER(Region), vp, vp]
+    L.pct_reconstruct_regions.argtypes = [vp, C.POINTER(Protons), vp, vp, vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32,
+                                          C.c_int, i64, C.c_float, vp, C.POINTER(i64), vp]
     if path == _build.LIB:
         _lib = L
     return L
@@ -192,6 +204,7 @@ class Context:
         p = MlpParams((C.c_double * 6)(*[float(a) for a in params["poly"]]), float(params["poly_max_depth_mm"]),
                       float(params["X0_mm"]), float(params["log_coeff"]), float(params["step_frac"]),
                       float(params["tie_eps_mm"]), int(params["max_visits"]))
+        self.geom = g
         self.n = g.nx * g.ny * g.nz
         h = C.c_void_p()
         rc = self._L.pct_create(C.byref(g), C.byref(p), device, C.byref(h))
@@ -342,6 +355,64 @@ class Context:
                                            _dev_ptr(hull, torch.uint8, self.n, self.device), _stream_ptr(self.device)))
         return hull
 
+    # ---- Algorithm 1 of the paper (reading R28): z-regions, one independent solve per region --------
+    def hull_intersect(self, protons: Dict[str, torch.Tensor], u_in_mm: float, u_out_mm: float,
+                       hull: Optional[torch.Tensor]):
+        """pct_hull_intersect (A1 alone): int32[m] hull entry and exit voxel of every history, -1 if rejected there."""
+        pr = self._protons_struct(protons, u_in_mm, u_out_mm)
+        v_in = torch.empty(max(pr.m, 1), dtype=torch.int32, device=self.device)
+        v_out = torch.empty(max(pr.m, 1), dtype=torch.int32, device=self.device)
+        self._check(self._L.pct_hull_intersect(self._h, C.byref(pr), _dev_ptr(hull, torch.uint8, self.n, self.device),
+                                               v_in.data_ptr(), v_out.data_ptr(), _stream_ptr(self.device)))
+        return v_in[:pr.m], v_out[:pr.m]
+
+    def region_members(self, v_in: torch.Tensor, v_out: torch.Tensor, region: "Region") -> torch.Tensor:
+        """pct_region_members (step 2): the member histories, ascending (indices < 2^31 in an int32 tensor)."""
+        m = int(v_in.numel())
+        idx = torch.empty(max(m, 1), dtype=torch.int32, device=self.device)
+        cnt = C.c_int64(0)
+        self._check(self._L.pct_region_members(self._h, _dev_ptr(v_in.contiguous(), torch.int32, m, self.device),
+                                               _dev_ptr(v_out.contiguous(), torch.int32, m, self.device), m, C.byref(region),
+                                               idx.data_ptr(), C.byref(cnt), _stream_ptr(self.device)))
+        return idx[:cnt.value]
+
+    def gather_histories(self, protons: Dict[str, torch.Tensor], u_in_mm: float, u_out_mm: float,
+                         b: Optional[torch.Tensor], idx: torch.Tensor):
+        """pct_gather_histories (step 3): the members' tracker records (dict of float64 tensors) and WEPLs."""
+        pr = self._protons_struct(protons, u_in_mm, u_out_mm)
+        count = int(idx.numel())
+        out = {k: torch.empty(max(count, 1), dtype=torch.float64, device=self.device) for k in PROTON_KEYS}
+        dst = Protons(count, *[out[k].data_ptr() for k in PROTON_KEYS], 0.0, 0.0)
+        b_dst = torch.empty(max(count, 1), dtype=torch.float32, device=self.device) if b is not None else None
+        self._check(self._L.pct_gather_histories(
+            self._h, C.byref(pr), _dev_ptr(b, torch.float32, pr.m, self.device) if b is not None else None,
+            _dev_ptr(idx.contiguous(), torch.int32, count, self.device) if count else None, count, C.byref(dst),
+            b_dst.data_ptr() if b_dst is not None else None, _stream_ptr(self.device)))
+        return {k: v[:count] for k, v in out.items()}, (b_dst[:count] if b_dst is not None else None)
+
+    def select_slices(self, x_region: torch.Tensor, region: "Region", x_final: torch.Tensor) -> torch.Tensor:
+        """pct_select_slices (step 5): the region's kept slices go into x_final."""
+        self._check(self._L.pct_select_slices(self._h, _dev_ptr(x_region, torch.float32, self.n, self.device), C.byref(region),
+                                              _dev_ptr(x_final, torch.float32, self.n, self.device), _stream_ptr(self.device)))
+        return x_final
+
+    def reconstruct_regions(self, protons: Dict[str, torch.Tensor], u_in_mm: float, u_out_mm: float,
+                            hull: Optional[torch.Tensor], b: torch.Tensor, x0: Optional[torch.Tensor], n_regions: int,
+                            ext: int, iters: int, block_size: int, lam: float, region_first: int = 0,
+                            region_count: Optional[int] = None, out: Optional[torch.Tensor] = None):
+        """pct_reconstruct_regions: steps 1-5 for the regions [region_first, region_first + region_count) on this GPU.
+        Returns (x, members per region; -1 for regions not run); slices kept by regions that were not run keep `out`'s values."""
+        pr = self._protons_struct(protons, u_in_mm, u_out_mm)
+        x = out if out is not None else torch.zeros(self.n, dtype=torch.float32, device=self.device)
+        members = (C.c_int64 * int(n_regions))(*([-1] * int(n_regions)))
+        rc = int(region_count) if region_count is not None else int(n_regions) - int(region_first)
+        self._check(self._L.pct_reconstruct_regions(
+            self._h, C.byref(pr), _dev_ptr(b, torch.float32, pr.m, self.device),
+            _dev_ptr(hull, torch.uint8, self.n, self.device), _dev_ptr(x0, torch.float32, self.n, self.device),
+            int(n_regions), int(ext), int(region_first), rc, int(iters), int(block_size), float(lam),
+            _dev_ptr(x, torch.float32, self.n, self.device), members, _stream_ptr(self.device)))
+        return x, list(members)
+
     def reconstruct_host(self, protons: Dict[str, torch.Tensor], u_in_mm: float, u_out_mm: float,
                          hull: Optional[torch.Tensor], b: torch.Tensor, x0: Optional[torch.Tensor], iters: int,
                          block_size: int, lam: float, x_out: torch.Tensor) -> dict:
@@ -362,3 +433,12 @@ class Context:
                                                  int(block_size), float(lam), x_out.data_ptr(), C.byref(st),
                                                  _stream_ptr(self.device)))
         return {k: getattr(st, k) for k, _ in ReconStats._fields_}
+
+
+def regions_setup(nz: int, n_regions: int, ext: int, lib=None) -> List["Region"]:
+    """pct_regions_setup (step 1; pure host arithmetic): the regions of Algorithm 1 as Region structs."""
+    L = lib or load_library()
+    out = (Region * int(n_regions))()
+    if L.pct_regions_setup(int(nz), int(n_regions), int(ext), out) != OK:
+        raise PctError(f"pct_regions_setup({nz}, {n_regions}, {ext}): invalid arguments")
+    return list(out)

@@ -8,7 +8,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_PKG)
 CSRC = os.path.join(_PKG, "csrc")
 LIB = os.path.join(_PKG, "libpct.so")
-SOURCES = ("pct_api.cu", "mlp_kernel.cu", "solve_kernels.cu", "solve_windowed.cu", "plan.cu", "peaks.cu", "pre_kernels.cu")
+SOURCES = ("pct_api.cu", "mlp_kernel.cu", "solve_kernels.cu", "solve_windowed.cu", "plan.cu", "peaks.cu", "pre_kernels.cu", "regions.cu")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--shared",
               "-Xcompiler", "-fPIC,-Wall", "-Xptxas", "-v", "-cudart", "static"]
 

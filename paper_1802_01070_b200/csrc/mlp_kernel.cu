@@ -501,13 +501,18 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const HistRec* __restrict__ recs, c
     }
 }
 
-// One batch of K1: spatial sort -> k_hull -> sort by K -> k_mlp_walk.  `stage` holds count rows of stage_chunks chunks; the
-// code stream must have room for count * stage_chunks more chunks behind *chunk_counter.
-int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, int64_t i_base, int count, ulonglong2* stage,
-                     unsigned long long* chunk_counter, pct_paths* P, cudaStream_t st) {
+// scratch of one batch: history records, sort keys/values (double buffered), cub temporary storage
+struct BatchScratch {
+    HistRec* recs;
+    cub::DoubleBuffer<uint32_t> dk, dv;     // K-order sort (key = K, value = local index)
+    void* sort_tmp;
+    size_t sort_tmp_bytes;
+};
+
+// A1 of one batch: spatial sort -> k_hull.  Leaves the records in S.recs (batch-local order) and the K keys in S.dk / S.dv.
+static int hull_stage(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, int64_t i_base, int count, cudaStream_t st, BatchScratch& S) {
     const int threads = 128;
     const int blocks = (count + threads - 1) / threads;
-    // scratch: history records, sort keys/values (double buffered), cub temporary storage
     size_t sort_tmp = 0;
     {
         cub::DoubleBuffer<uint32_t> dk(nullptr, nullptr), dv(nullptr, nullptr);
@@ -524,10 +529,11 @@ int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, in
         ctx->gen_scratch_bytes = total;
     }
     char* base = (char*)ctx->gen_scratch;
-    HistRec* recs = (HistRec*)(base + o_rec);
-    cub::DoubleBuffer<uint32_t> dk((uint32_t*)(base + o_k0), (uint32_t*)(base + o_k1)), dv((uint32_t*)(base + o_v0), (uint32_t*)(base + o_v1));
+    S.recs = (HistRec*)(base + o_rec);
+    S.dk = cub::DoubleBuffer<uint32_t>((uint32_t*)(base + o_k0), (uint32_t*)(base + o_k1));
+    S.dv = cub::DoubleBuffer<uint32_t>((uint32_t*)(base + o_v0), (uint32_t*)(base + o_v1));
+    S.sort_tmp = base + o_tmp; S.sort_tmp_bytes = sort_tmp;
     cub::DoubleBuffer<uint32_t> sk((uint32_t*)(base + o_k2), (uint32_t*)(base + o_k3)), sv((uint32_t*)(base + o_v2), (uint32_t*)(base + o_v3));
-    ProfScope prof(ctx, 0, st);
     {   // spatial order of the batch: 2 mm cells of the entry tracker plane
         const DevCfg& c = ctx->cfg;
         const double ex = fmax(fabs(c.lo[0]), fabs(c.hi[0])), ey = fmax(fabs(c.lo[1]), fabs(c.hi[1]));
@@ -536,15 +542,50 @@ int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, in
         k_hull_keys<<<(count + 255) / 256, 256, 0, st>>>(pr, i_base, count, -t_half, c.lo[2], 1.0 / cell, nt, nv, sk.Current(), sv.Current());
         int bits = 1;
         while ((1LL << bits) < (long long)nt * nv) ++bits;
-        PCT_CUDA(ctx, cub::DeviceRadixSort::SortPairs(base + o_tmp, sort_tmp, sk, sv, count, 0, bits, st));
+        PCT_CUDA(ctx, cub::DeviceRadixSort::SortPairs(S.sort_tmp, sort_tmp, sk, sv, count, 0, bits, st));
     }
-    k_hull<<<blocks, threads, 0, st>>>(ctx->cfg, pr, hull, i_base, count, sv.Current(), recs, dk.Current(), dv.Current());
+    k_hull<<<blocks, threads, 0, st>>>(ctx->cfg, pr, hull, i_base, count, sv.Current(), S.recs, S.dk.Current(), S.dv.Current());
+    ctx->launches += 3;
+    PCT_CUDA(ctx, cudaGetLastError());
+    return PCT_OK;
+}
+
+// One batch of K1: spatial sort -> k_hull -> sort by K -> k_mlp_walk.  `stage` holds count rows of stage_chunks chunks; the
+// rows are copied to the code stream at places handed out by the device counter `chunk_counter`.
+int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, int64_t i_base, int count, ulonglong2* stage,
+                     unsigned long long* chunk_counter, pct_paths* P, cudaStream_t st) {
+    const int threads = 128;
+    const int blocks = (count + threads - 1) / threads;
+    ProfScope prof(ctx, 0, st);
+    BatchScratch S;
+    int rc;
+    if ((rc = hull_stage(ctx, pr, hull, i_base, count, st, S)) != PCT_OK) return rc;
     int key_bits = 1;
     while ((1 << key_bits) < ctx->logk_n) ++key_bits;                  // K < logk_n
-    PCT_CUDA(ctx, cub::DeviceRadixSort::SortPairs(base + o_tmp, sort_tmp, dk, dv, count, 0, key_bits, st));
-    k_mlp_walk<<<blocks, threads, 0, st>>>(ctx->cfg, recs, dv.Current(), ctx->logk, i_base, count, stage, P->codes, chunk_counter,
+    PCT_CUDA(ctx, cub::DeviceRadixSort::SortPairs(S.sort_tmp, S.sort_tmp_bytes, S.dk, S.dv, count, 0, key_bits, st));
+    k_mlp_walk<<<blocks, threads, 0, st>>>(ctx->cfg, S.recs, S.dv.Current(), ctx->logk, i_base, count, stage, P->codes, chunk_counter,
                                            P->code_off, P->N, P->start, P->end, P->ell, P->flags, ctx->d_stats);
-    ctx->launches += 5;
+    ctx->launches += 2;
+    PCT_CUDA(ctx, cudaGetLastError());
+    return PCT_OK;
+}
+
+// A1 alone (pct_hull_intersect): the hull entry and exit voxels of a batch, -1 for a history that A1 rejects
+__global__ void __launch_bounds__(256) k_extract_ends(const HistRec* __restrict__ recs, int count, int32_t* __restrict__ v_in, int32_t* __restrict__ v_out) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= count) return;
+    const bool rej = (recs[p].flags & PCT_REJECT_MASK) != 0;
+    v_in[p] = rej ? -1 : recs[p].vin;
+    v_out[p] = rej ? -1 : recs[p].vout;
+}
+
+int launch_hull_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, int64_t i_base, int count, int32_t* v_in, int32_t* v_out, cudaStream_t st) {
+    ProfScope prof(ctx, 0, st);
+    BatchScratch S;
+    int rc;
+    if ((rc = hull_stage(ctx, pr, hull, i_base, count, st, S)) != PCT_OK) return rc;
+    k_extract_ends<<<(count + 255) / 256, 256, 0, st>>>(S.recs, count, v_in + i_base, v_out + i_base);
+    ++ctx->launches;
     PCT_CUDA(ctx, cudaGetLastError());
     return PCT_OK;
 }

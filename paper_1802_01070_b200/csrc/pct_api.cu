@@ -132,11 +132,6 @@ static std::mutex g_ctx_mu;
 
 static double factorial(int k) { double r = 1.0; for (int i = 2; i <= k; ++i) r *= i; return r; }
 
-struct DeviceGuard {
-    int prev = -1;
-    explicit DeviceGuard(int dev) { cudaGetDevice(&prev); if (prev != dev) cudaSetDevice(dev); else prev = -1; }
-    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
-};
 
 // rows are only meaningful on the grid and device they were generated for
 static bool same_grid(const pct_ctx* ctx, const pct_paths* P) {
@@ -181,6 +176,38 @@ static int ensure_codes(pct_ctx* ctx, pct_paths* P, int64_t need, cudaStream_t s
     return PCT_OK;
 }
 
+}  // namespace pct
+
+namespace pct {
+// Before any A1 kernel: the tracker planes of this data set and the clip box of the hull search (find_hull) -- the bounding
+// box of the hull voxels, or the grid.  Synchronises `st` when there is a hull.
+int prepare_hull_search(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hull, cudaStream_t st) {
+    ctx->cfg.u_in = pr->u_in_mm; ctx->cfg.u_out = pr->u_out_mm;
+    const int nn[3] = {ctx->geom.nx, ctx->geom.ny, ctx->geom.nz};
+    for (int a = 0; a < 3; ++a) { ctx->cfg.bmin[a] = 0; ctx->cfg.bmax[a] = nn[a] - 1; }
+    if (hull && pr->m > 0) {
+        int box[6];
+        int* d_box = reinterpret_cast<int*>(ctx->d_stats);      // scratch of 24 bytes; callers clear d_stats afterwards
+        int rc0;
+        if ((rc0 = launch_hull_bbox(ctx, hull, d_box, st)) != PCT_OK) return rc0;
+        PCT_CUDA(ctx, cudaMemcpyAsync(box, d_box, sizeof(box), cudaMemcpyDeviceToHost, st));
+        PCT_CUDA(ctx, cudaStreamSynchronize(st));
+        for (int a = 0; a < 3; ++a) {
+            if (box[3 + a] >= box[a]) { ctx->cfg.bmin[a] = box[a]; ctx->cfg.bmax[a] = box[3 + a]; }
+            else { ctx->cfg.bmin[a] = 0; ctx->cfg.bmax[a] = -1; }               // empty hull: every ray misses
+        }
+    }
+    return PCT_OK;
+}
+
+// argument checks shared by the calls that take tracker records
+int check_protons(pct_ctx* ctx, const pct_protons* pr) {
+    if (!pr || pr->m < 0) return set_error(ctx, PCT_E_INVALID_ARG, "bad protons");
+    if (pr->m > 0 && (!pr->phi || !pr->t_in || !pr->v_in || !pr->dt_in || !pr->dv_in || !pr->t_out || !pr->v_out || !pr->dt_out || !pr->dv_out))
+        return set_error(ctx, PCT_E_INVALID_ARG, "NULL tracker array");
+    if (!std::isfinite(pr->u_in_mm) || !std::isfinite(pr->u_out_mm)) return set_error(ctx, PCT_E_INVALID_ARG, "bad tracker planes");
+    return PCT_OK;
+}
 }  // namespace pct
 
 using namespace pct;
@@ -304,22 +331,9 @@ int pct_generate_mlp(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hull, v
     if (!std::isfinite(pr->u_in_mm) || !std::isfinite(pr->u_out_mm)) return set_error(ctx, PCT_E_INVALID_ARG, "bad tracker planes");
     DeviceGuard guard(ctx->device);
     cudaStream_t st = (cudaStream_t)stream;
-    ctx->cfg.u_in = pr->u_in_mm; ctx->cfg.u_out = pr->u_out_mm;
-    {   // clip box of the hull search (find_hull): bounding box of the hull voxels, or the grid
-        const int nn[3] = {ctx->geom.nx, ctx->geom.ny, ctx->geom.nz};
-        for (int a = 0; a < 3; ++a) { ctx->cfg.bmin[a] = 0; ctx->cfg.bmax[a] = nn[a] - 1; }
-        if (hull && pr->m > 0) {
-            int box[6];
-            int* d_box = reinterpret_cast<int*>(ctx->d_stats);      // scratch of 24 bytes; d_stats is cleared below
-            int rc0;
-            if ((rc0 = launch_hull_bbox(ctx, hull, d_box, st)) != PCT_OK) return rc0;
-            PCT_CUDA(ctx, cudaMemcpyAsync(box, d_box, sizeof(box), cudaMemcpyDeviceToHost, st));
-            PCT_CUDA(ctx, cudaStreamSynchronize(st));
-            for (int a = 0; a < 3; ++a) {
-                if (box[3 + a] >= box[a]) { ctx->cfg.bmin[a] = box[a]; ctx->cfg.bmax[a] = box[3 + a]; }
-                else { ctx->cfg.bmin[a] = 0; ctx->cfg.bmax[a] = -1; }               // empty hull: every ray misses
-            }
-        }
+    {
+        const int rc0 = prepare_hull_search(ctx, pr, hull, st);
+        if (rc0 != PCT_OK) return rc0;
     }
     pct_paths* P = new (std::nothrow) pct_paths();
     if (!P) return set_error(ctx, PCT_E_OOM, "host allocation");

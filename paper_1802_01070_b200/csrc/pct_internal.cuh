@@ -187,6 +187,17 @@ struct ProfScope {
                                   "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e__), __FILE__, __LINE__); \
     } while (0)
 
+// makes `dev` current for the scope of a call
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev) { cudaGetDevice(&prev); if (prev != dev) cudaSetDevice(dev); else prev = -1; }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+int prepare_hull_search(pct_ctx* ctx, const pct_protons* pr, const uint8_t* hull, cudaStream_t st);
+int check_protons(pct_ctx* ctx, const pct_protons* pr);
+int launch_hull_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, int64_t i_base, int count, int32_t* v_in, int32_t* v_out, cudaStream_t st);
+
 // launchers implemented in the .cu files (all enqueue on `st`, none synchronises unless stated)
 int launch_mlp_batch(pct_ctx* ctx, const ProtonPtrs& pr, const uint8_t* hull, int64_t i_base, int count, ulonglong2* stage,
                      unsigned long long* chunk_counter, pct_paths* P, cudaStream_t st);
