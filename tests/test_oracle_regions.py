@@ -100,4 +100,105 @@ def test_membership_by_brute_force(regions_oracle):
     assert thr.size == 0
 
 
-# ORACLE_REGIONS_PART_2
+def tiny_case(oracle, m=3000):
+    cfg = synth.scaled(synth.CONFIGS["tiny"], m)
+    x_true, hull, shadow = synth.make_phantom(cfg)
+    pr = synth.generate_protons(cfg, x_true, shadow)
+    g, p, pa, P = oracle_setup(oracle, cfg, pr, hull)
+    arrays = {k: v.cpu().numpy() for k, v in pr.items() if k != "wepl"}
+    return cfg, g, p, arrays, hull.numpy(), pr["wepl"].numpy(), P
+
+
+def test_special_cases_reproduce_the_plain_solver(oracle, regions_oracle):
+    cfg, g, p, arrays, hull, b, P = tiny_case(oracle)
+    n = cfg.nx * cfg.ny * cfg.nz
+    x_plain = P.solve(b, np.ones(n, np.float32), 2, cfg.block, cfg.lam)
+    flags = P.rows()[3]
+    accepted = int(np.count_nonzero((flags & regions_oracle.A1_REJECT) == 0))
+    # one region: every accepted history is a member, the image is the plain solver's (rejected rows are empty: same sums)
+    x1, mem1, _ = regions_oracle.reconstruct(g, p, arrays, -cfg.u_tracker, cfg.u_tracker, hull, b, None, 1, 0, 2, cfg.block, cfg.lam)
+    assert mem1[0].size == accepted and np.all(np.diff(mem1[0]) > 0)
+    # blocks are consecutive ranges of the MEMBER list: with the rejected histories dropped the block boundaries move, so the
+    # comparison uses one block per sweep (block >= m), where membership cannot change the blocking
+    x_plain_1 = P.solve(b, np.ones(n, np.float32), 2, cfg.m, cfg.lam)
+    x1b, _, _ = regions_oracle.reconstruct(g, p, arrays, -cfg.u_tracker, cfg.u_tracker, hull, b, None, 1, 0, 2, cfg.m, cfg.lam)
+    assert np.abs(x1b - x_plain_1).max() < 1e-5
+    # an extension of nz slices makes every region the whole volume: every region's image is the plain solver's
+    x3, mem3, imgs = regions_oracle.reconstruct(g, p, arrays, -cfg.u_tracker, cfg.u_tracker, hull, b, None, 3, cfg.nz, 2, cfg.m, cfg.lam)
+    assert all(mm.size == accepted for mm in mem3)
+    for img in imgs:
+        assert np.abs(img - x_plain_1).max() < 1e-5
+    assert np.abs(x3 - x_plain_1).max() < 1e-5
+    assert np.abs(x_plain - 1.0).max() > 0.05 and np.abs(x1 - 1.0).max() > 0.05          # the solves did something
+
+
+def test_regions_without_overlap_differ_only_near_the_cuts(oracle, regions_oracle):
+    """Table I of the paper: a path hardly moves along z, so a region solved on its own histories reproduces the joint solve away
+    from the cut; with ext = 0 the slices next to a cut see histories that the neighbour also updates, and may differ."""
+    cfg, g, p, arrays, hull, b, P = tiny_case(oracle, 6000)
+    n, sl = cfg.nx * cfg.ny * cfg.nz, cfg.nx * cfg.ny
+    x_plain = P.solve(b, np.ones(n, np.float32), 3, cfg.m, cfg.lam).reshape(cfg.nz, -1)
+    x2, mem, _ = regions_oracle.reconstruct(g, p, arrays, -cfg.u_tracker, cfg.u_tracker, hull, b, None, 2, 2, 3, cfg.m, cfg.lam)
+    x2 = x2.reshape(cfg.nz, -1)
+    assert 0 < mem[0].size < 6000 and 0 < mem[1].size < 6000
+    assert np.intersect1d(mem[0], mem[1]).size > 0                             # the overlap's histories go to both regions
+    # DROP divides a block's update by the per-voxel count of the BLOCK: dropping far-away histories leaves the near slices'
+    # sums and counts unchanged, so the first and last slices agree with the joint solve to rounding
+    assert np.abs(x2[0] - x_plain[0]).max() < 1e-5 and np.abs(x2[-1] - x_plain[-1]).max() < 1e-5
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    return port
+
+
+def _gloo_worker(rank, world, port, n_regions, nz, slice_elems, out_q):
+    import torch.distributed as dist
+    from paper_1802_01070_b200 import regions
+    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world)
+    try:
+        owner = regions.region_owner(n_regions, world)
+        first, count = regions.my_regions(n_regions, rank, world)
+        cuts = [(g * nz) // n_regions for g in range(n_regions + 1)]
+        keep = [(cuts[g], cuts[g + 1]) for g in range(n_regions)]
+        # every rank fills the kept slices of ITS regions with a value that names (region, slice); the rest stays -1
+        x = torch.full((nz * slice_elems,), -1.0)
+        for g in range(first, first + count):
+            for z in range(*keep[g]):
+                x[z * slice_elems:(z + 1) * slice_elems] = 100.0 * g + z
+        regions.assemble_slices(x, keep, owner, slice_elems)
+        out_q.put((rank, first, count, x.numpy().copy()))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("n_regions", [2, 3])
+def test_slice_assembly_across_two_processes(n_regions):
+    """selectSlice() across ranks (gloo, world_size 2): afterwards every rank holds every slice from the region that keeps it."""
+    import torch.multiprocessing as mp
+    from paper_1802_01070_b200 import regions
+    nz, slice_elems, world = 8, 6, 2
+    assert regions.region_owner(2, 2) == [0, 1] and regions.region_owner(3, 2) == [0, 0, 1] and regions.region_owner(1, 2) == [0]
+    assert regions.my_regions(1, 1, 2) == (0, 0)
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_gloo_worker, args=(r, world, port, n_regions, nz, slice_elems, q)) for r in range(world)]
+    for pr in procs:
+        pr.start()
+    got = [q.get(timeout=120) for _ in range(world)]
+    for pr in procs:
+        pr.join(timeout=60)
+        assert pr.exitcode == 0
+    cuts = [(g * nz) // n_regions for g in range(n_regions + 1)]
+    want = np.empty(nz * slice_elems, dtype=np.float32)
+    for g in range(n_regions):
+        for z in range(cuts[g], cuts[g + 1]):
+            want[z * slice_elems:(z + 1) * slice_elems] = 100.0 * g + z
+    assert sorted(r for r, _, _, _ in got) == [0, 1]
+    assert sum(c for _, _, c, _ in got) == n_regions
+    for _, _, _, x in got:
+        assert np.array_equal(x, want)
