@@ -368,12 +368,41 @@ def bench_workload(args, cfg, dev, local, world, dist, steps, warmup, e2e_steps,
             ctx.solve(paths, b, xa, 1, cfg.block, cfg.lam, out=xa)
             ctx.solve(paths, b, xb, 1, cfg.block, cfg.lam, out=xb)
             curve["x0=1"].append(rms(xa)); curve["x0=fbp"].append(rms(xb))
-        paths.free()
+        # Algorithm 1 of the paper (R28) on this one GPU: the regions run in turn, each timed on its own
+        # -- what each GPU of a G-GPU run would do; no multi-GPU number is claimed -- and the image compared with the joint solve
+        alg1 = None
+        if args.regions > 1:
+            ext = max(1, int(round(7.5 / cfg.h)))            # the paper's 3 slices of 2.5 mm
+            x_joint = ctx.solve(paths, b, x0, cfg.iters, cfg.block, cfg.lam)
+            paths.free()
+            x_a1 = torch.zeros_like(x_joint)
+            per_region, members = [], []
+            for r in range(args.regions):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                _, mem = ctx.reconstruct_regions(protons, -cfg.u_tracker, cfg.u_tracker, hull_flat, b, None, args.regions, ext,
+                                                 cfg.iters, cfg.block, cfg.lam, region_first=r, region_count=1, out=x_a1)
+                e1.record()
+                torch.cuda.synchronize()
+                per_region.append(e0.elapsed_time(e1)); members.append(mem[r])
+            inside = hull_flat.bool()
+            d = (x_a1 - x_joint)[inside].double()
+            alg1 = {"n_regions": args.regions, "ext_slices": ext, "members": members, "histories": cfg.m,
+                    "ms_per_region": per_region, "ms_slowest_region": max(per_region),
+                    "vs_joint_solve": {"rel_l2_in_hull": float(d.norm() / x_joint[inside].double().norm()),
+                                       "max_abs_in_hull": float(d.abs().max()), "mean_abs_in_hull": float(d.abs().mean())},
+                    "note": "each region = pct_hull_intersect on all histories + membership + gather + pct_generate_mlp + pct_solve "
+                            "on its members, timed alone on this GPU; Algorithm 1 is an approximation of the joint solve "
+                            "(PAPER.md Tables VIII/IX: RSP errors move by <= 0.35 %)"}
+            del x_joint, x_a1
+        else:
+            paths.free()
         hm = hull_flat.bool()
         pre = {"fbp_ms": ev[0].elapsed_time(ev[1]), "fbp_bins": [cfg.nz, 180, n_s], "hull_carve_ms": ev[1].elapsed_time(ev[2]),
                "hull_carve": {"wepl_air_mm": 1.0, "min_chord_mm": 0.25 * cfg.h, "voxels_kept": int(carved.sum()),
                               "analytic_hull_voxels": int(hm.sum()), "analytic_hull_voxels_carved": int((hm & (carved == 0)).sum())},
                "rms_residual_mm_by_sweep": curve,
+               "algorithm1": alg1,
                "note": "rms of b - A x over the first 4 blocks after 0, 1, 2, ... sweeps from x0 = 1 and from the FBP image (PAPER.md:7)"}
         del x_fbp, carved, xa, xb
 
@@ -467,6 +496,7 @@ def main():
     ap.add_argument("--e2e-warmup", type=int, default=2)
     ap.add_argument("--profile-steps", type=int, default=2, choices=range(1, 9),
                     help="instrumented steps for the per-kernel breakdown (outside the headline timing)")
+    ap.add_argument("--regions", type=int, default=2, help="z-regions of the Algorithm-1 extra (PAPER.md:59-67); < 2: skip")
     ap.add_argument("--pre-steps", type=int, default=5, help="sweeps of the FBP-start vs unit-start residual curve (0: skip the 8(f) extras)")
     ap.add_argument("--oracle-sample", type=int, default=1_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
