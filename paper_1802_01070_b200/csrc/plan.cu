@@ -237,38 +237,63 @@ k_plan_walk(const __grid_constant__ DevCfg g, const uint32_t* __restrict__ N, co
     bool ok = r >= 0 && r < r_end;
     uint8_t* my_cnt = cnt + G.cnt_off + threadIdx.x;
     unsigned long long* out = stream + G.stream_off + threadIdx.x;
-    unsigned long long w = 0, acc = ~0ull;
-    int nrem = 0, row_cnt = 0, k = 0, cur_slab = ok ? r / SLAB : 0;          // k = codes emitted in the current slab
+    int cur_slab = ok ? r / SLAB : 0;
     const int first_slab = cur_slab, slab_cap = G.wps * CODES_PER_WORD;
-    int nb = ok ? plan_nbase(G, r) : 0, zb = ok ? plan_zbase(G, r) : 0;
     const uint32_t p0 = win_pack(n, r, z);
     int on_lo = WIN_N, on_hi = -1, oz_lo = WIN_Z, oz_hi = -1;
-    for (uint32_t v = 0; v < mw.n_vis && ok; ++v) {
+    // The loop below runs once per visit of 1.6e10 (config 2): it is written without divisions and with selects instead of
+    // branches.  State: the window bases as 16.16 fixed-point accumulators (nacc = nb0 + r sn: plan_nbase without the
+    // multiplication), the word being assembled (`acc`: every code enters at the top and moves down 3 bits per push, so no
+    // variable shift per visit), kw = codes in it, k = codes in the slab, op = where the next word of the slab goes.
+    long long nacc = (long long)G.nb0 + (long long)r * G.sn, zacc = (long long)G.zb0 + (long long)r * G.sz;
+    unsigned long long w = 0, acc = ~0ull;
+    unsigned long long* op = out + (size_t)cur_slab * G.wps * GROUP;
+    int nrem = 0, row_cnt = 0, k = 0, kw = 0;
+    // codes sit at the top 3 kw bits of acc, oldest lowest: move them down, pads (all ones) above; bit 63 of a full word is a pad bit
+    auto finish_word = [&]() -> unsigned long long {
+        return kw == CODES_PER_WORD ? ((acc >> 1) | 0x8000000000000000ull) : ((acc >> (64 - 3 * kw)) | (~0ull << (3 * kw)));
+    };
+    const int cls = G.cls;
+    // one exit test per visit: a failed check sets `bad`, the visit is not emitted, and the loop condition ends the walk
+    bool bad = !ok;
+    for (uint32_t v = 0; v < mw.n_vis && !bad; ++v) {
         int code = PLAN_CODE_FIRST;
         if (v > 0) {
             if (nrem == 0) { w = __ldg(mw.cp++); nrem = CODES_PER_WORD; }
-            code = (int)(w & 7ull);
+            code = (int)((unsigned)w & 7u);
             w >>= 3; --nrem;
-            if (code == G.cls) {
-                ++r; row_cnt = 0;
-                if (r >= r_end) { ok = false; break; }
-                nb = plan_nbase(G, r); zb = plan_zbase(G, r);
-                if ((r / SLAB) != cur_slab) {
-                    if (k % CODES_PER_WORD != 0) out[((size_t)cur_slab * G.wps + k / CODES_PER_WORD) * GROUP] = acc;
+            const bool is_row = code == cls;
+            bad = (code == (cls ^ 1)) | (code >= 6);                                  // against the travel direction, or not a step
+            const int sign = 1 - 2 * (code & 1);                                      // even code = +1 along its axis
+            const bool is_z = code >= 4;
+            z += is_z ? sign : 0;
+            n += (is_z | is_row) ? 0 : sign;
+            r += is_row ? 1 : 0;
+            nacc += is_row ? (long long)G.sn : 0ll;
+            zacc += is_row ? (long long)G.sz : 0ll;
+            row_cnt = is_row ? 0 : row_cnt;
+            if (is_row && (r & (SLAB - 1)) == 0) {                                    // first row of the next slab
+                if (r >= r_end) bad = true;
+                else {
+                    if (kw != 0) *op = finish_word();
                     my_cnt[(size_t)cur_slab * GROUP] = (uint8_t)k;
-                    cur_slab = r / SLAB; k = 0; acc = ~0ull;
+                    ++cur_slab; k = 0; kw = 0; acc = ~0ull;
+                    op = out + (size_t)cur_slab * G.wps * GROUP;
                 }
-            } else if (code == (G.cls ^ 1) || code >= 6) { ok = false; break; }
-            else if (code >= 4) z += (code & 1) ? -1 : 1;
-            else n += (code == mw.n_plus) ? 1 : -1;
+            }
         }
-        if ((unsigned)(n - nb) >= (unsigned)WIN_N || (unsigned)(z - zb) >= (unsigned)WIN_Z || ++row_cnt > MAX_ROW_VISITS || k >= slab_cap) { ok = false; break; }
-        on_lo = min(on_lo, n - nb); on_hi = max(on_hi, n - nb); oz_lo = min(oz_lo, z - zb); oz_hi = max(oz_hi, z - zb);
-        acc ^= (unsigned long long)(7 ^ code) << (3 * (k % CODES_PER_WORD));
-        if (++k % CODES_PER_WORD == 0) { out[((size_t)cur_slab * G.wps + k / CODES_PER_WORD - 1) * GROUP] = acc; acc = ~0ull; }
+        const int dn = n - (int)(nacc >> 16), dz = z - (int)(zacc >> 16);
+        bad |= ((unsigned)dn >= (unsigned)WIN_N) | ((unsigned)dz >= (unsigned)WIN_Z) | (++row_cnt > MAX_ROW_VISITS) | (k >= slab_cap);
+        if (!bad) {
+            on_lo = min(on_lo, dn); on_hi = max(on_hi, dn); oz_lo = min(oz_lo, dz); oz_hi = max(oz_hi, dz);
+            acc = (acc >> 3) | ((unsigned long long)(unsigned)code << 61);
+            ++k;
+            if (++kw == CODES_PER_WORD) { *op = (acc >> 1) | 0x8000000000000000ull; op += GROUP; kw = 0; acc = ~0ull; }
+        }
     }
+    ok = !bad;
     if (ok) {
-        if (k % CODES_PER_WORD != 0) out[((size_t)cur_slab * G.wps + k / CODES_PER_WORD) * GROUP] = acc;
+        if (kw != 0) *op = finish_word();
         my_cnt[(size_t)cur_slab * GROUP] = (uint8_t)k;
         // widen the group's visited extent (the plain read only filters out the atomics that cannot change anything)
         PlanGroup* Gp = groups + blockIdx.x;
