@@ -380,6 +380,7 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const HistRec* __restrict__ recs, c
             double A0 = rec->pin[0], A1 = rec->pin[1], A2 = rec->pin[2];
             double lo0 = face_coord(g, 0, c0), hi0 = face_coord(g, 0, c0 + 1), lo1 = face_coord(g, 1, c1), hi1 = face_coord(g, 1, c1 + 1),
                    lo2 = face_coord(g, 2, c2), hi2 = face_coord(g, 2, c2 + 1);
+            double cd0 = (double)c0, cd1 = (double)c1, cd2 = (double)c2;
             double L = 0.0;
             int n_vis = 1;
             bool tie = false, bad = false;
@@ -424,9 +425,15 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const HistRec* __restrict__ recs, c
                     const int cb = d2 != 0 ? k2c : k1c;                            // n == 2: the other one
                     cw.push_upto2(b_first ? cb : ca, b_first ? ca : cb, n);
                     // move
-                    if (d0 != 0) { c0 = t0; if (d0 > 0) { lo0 = hi0; hi0 = face_coord(g, 0, t0 + 1); } else { hi0 = lo0; lo0 = face_coord(g, 0, t0); } }
-                    if (d1 != 0) { c1 = t1; if (d1 > 0) { lo1 = hi1; hi1 = face_coord(g, 1, t1 + 1); } else { hi1 = lo1; lo1 = face_coord(g, 1, t1); } }
-                    if (d2 != 0) { c2 = t2; if (d2 > 0) { lo2 = hi2; hi2 = face_coord(g, 2, t2 + 1); } else { hi2 = lo2; lo2 = face_coord(g, 2, t2); } }
+                    // (no branch: the voxel index, kept as a double too, follows d, and both faces are recomputed from it with
+                    // face_coord's own fma -- the same values, also for an axis that did not move)
+                    c0 = t0; c1 = t1; c2 = t2;
+                    cd0 += B0 > hi0 ? 1.0 : (B0 < lo0 ? -1.0 : 0.0);
+                    cd1 += B1 > hi1 ? 1.0 : (B1 < lo1 ? -1.0 : 0.0);
+                    cd2 += B2 > hi2 ? 1.0 : (B2 < lo2 ? -1.0 : 0.0);
+                    lo0 = fma(cd0, g.h, g.lo[0]); hi0 = fma(cd0 + 1.0, g.h, g.lo[0]);
+                    lo1 = fma(cd1, g.h, g.lo[1]); hi1 = fma(cd1 + 1.0, g.h, g.lo[1]);
+                    lo2 = fma(cd2, g.h, g.lo[2]); hi2 = fma(cd2 + 1.0, g.h, g.lo[2]);
                     n_vis += n;
                 } else {
                     // the general rule R9: while B is strictly outside the closed voxel, step across the candidate face with the
@@ -471,6 +478,7 @@ k_mlp_walk(const __grid_constant__ DevCfg g, const HistRec* __restrict__ recs, c
                     }
                     if (bad) break;
                     c0 = c[0]; c1 = c[1]; c2 = c[2];
+                    cd0 = (double)c0; cd1 = (double)c1; cd2 = (double)c2;
                     lo0 = f_lo[0]; lo1 = f_lo[1]; lo2 = f_lo[2]; hi0 = f_hi[0]; hi1 = f_hi[1]; hi2 = f_hi[2];
                 }
                 A0 = B0; A1 = B1; A2 = B2;
