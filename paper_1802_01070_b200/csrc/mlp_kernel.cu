@@ -131,49 +131,35 @@ __device__ __forceinline__ double rcp_newton(double d) {
     return fma(r, fma(-d, r, 1.0), r);
 }
 
-// 16-byte chunk writer: 42 codes, field k at bits 3(k%21) of word k/21; unused fields are 7 (pad).  A code is inserted
-// at the top of the word being filled and the word shifted down by one field per push, so that after 21 pushes the first
-// code sits in field 0 (one funnel shift and one OR per code, no variable shifts).
+// Row writer: 16-byte chunks of 42 codes, field k at bits 3(k%21) of word k/21; unused fields are 7 (pad).  A code is
+// inserted at the top of the 64-bit word being filled and the word shifted down by one field per push, so that after 21
+// pushes the first code sits in field 0 (one funnel shift and one OR per code, no variable shifts); a full word is stored
+// through a running pointer (the two words of a chunk are consecutive in memory).
 struct CodeWriter {
-    unsigned long long acc, w0;   // word being filled; finished first word of the chunk
-    int nc, chunk;                // codes in the current chunk (0..41); chunks written
-    ulonglong2* stage;            // stage[chunk]
-    __device__ __forceinline__ void init(ulonglong2* s) { acc = 0ull; w0 = 0ull; nc = 0; chunk = 0; stage = s; }
+    unsigned long long acc;       // word being filled
+    int nc;                       // codes in it (0..20)
+    unsigned long long *wp, *w0;  // next word to store; first word of the row
+    __device__ __forceinline__ void init(ulonglong2* s) { acc = 0ull; nc = 0; wp = w0 = reinterpret_cast<unsigned long long*>(s); }
     __device__ __forceinline__ void push(int code) {
         acc = (acc >> 3) | ((unsigned long long)code << 60);
-        ++nc;
-        if (nc == CODES_PER_WORD) { w0 = acc; acc = 0ull; }
-        else if (nc == CODES_PER_CHUNK) {
-            stage[chunk] = make_ulonglong2(w0, acc);
-            acc = 0ull; nc = 0; ++chunk;
-        }
+        if (++nc == CODES_PER_WORD) { *wp++ = acc; acc = 0ull; nc = 0; }
     }
     // n = 0, 1 or 2 codes at once (c1 first): one converged path for all lanes of a warp whatever their n -- the shift is
     // 3 n bits and the codes enter the upper 32-bit half only.  A pair that straddles a word boundary goes code by code.
     __device__ __forceinline__ void push_upto2(int c1, int c2, int n) {
-        if (n == 2 && (nc == CODES_PER_WORD - 1 || nc == CODES_PER_CHUNK - 1)) { push(c1); push(c2); return; }
+        if (n == 2 && nc == CODES_PER_WORD - 1) { push(c1); push(c2); return; }
         const unsigned sh = 3u * (unsigned)n;
         const unsigned bits = n == 2 ? (unsigned)(c1 | (c2 << 3)) : (unsigned)c1;
         const unsigned ins = n == 0 ? 0u : bits << (n == 2 ? 25 : 28);
         acc = (acc >> sh) | ((unsigned long long)ins << 32);
         nc += n;
-        if (n > 0 && nc == CODES_PER_WORD) { w0 = acc; acc = 0ull; }
-        else if (nc == CODES_PER_CHUNK) {
-            stage[chunk] = make_ulonglong2(w0, acc);
-            acc = 0ull; nc = 0; ++chunk;
-        }
+        if (nc == CODES_PER_WORD) { *wp++ = acc; acc = 0ull; nc = 0; }
     }
-    // a word holding k < 21 codes: shift them down to field 0 and fill the rest with pads
-    __device__ __forceinline__ static unsigned long long partial(unsigned long long a, int k) {
-        return k == 0 ? ~0ull : ((a >> (3 * (CODES_PER_WORD - k))) | (~0ull << (3 * k)));
-    }
+    // the last word (k < 21 codes: shifted down to field 0, the rest pads) and a pad word if the chunk is half full; -> chunks
     __device__ __forceinline__ int finish() {
-        if (nc > 0) {
-            stage[chunk] = nc >= CODES_PER_WORD ? make_ulonglong2(w0, partial(acc, nc - CODES_PER_WORD))
-                                                : make_ulonglong2(partial(acc, nc), ~0ull);
-            ++chunk;
-        }
-        return chunk;
+        if (nc > 0) *wp++ = (acc >> (3 * (CODES_PER_WORD - nc))) | (~0ull << (3 * nc));
+        if ((wp - w0) & 1) *wp++ = ~0ull;
+        return (int)((wp - w0) >> 1);
     }
 };
 
