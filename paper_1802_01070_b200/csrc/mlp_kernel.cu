@@ -82,19 +82,24 @@ __device__ __noinline__ void find_hull(const DevCfg& g, const uint8_t* __restric
             if (s_next[2] < sb) { ax = 2; sb = s_next[2]; }
             if (sb == INFINITY) return;                                     // the chord ends without meeting the hull
             if ((ax != 0 && s_next[0] - sb < tie_s) || (ax != 1 && s_next[1] - sb < tie_s) || (ax != 2 && s_next[2] - sb < tie_s)) hit.tie = true;
-#define PCT_HULL_ADVANCE(a)                                                                                    \
-            {                                                                                                  \
-                c[a] += step[a];                                                                               \
-                if (--left[a] < 0) return;                     /* left the hull's bounding box: miss */         \
-                lin += dlin[a];                                                                                \
-                const double f = face_coord(g, a, c[a] + (step[a] > 0 ? 1 : 0));                               \
-                const bool cand = step[a] > 0 ? E[a] > f : E[a] < f;                                           \
-                s_next[a] = cand ? (f - T[a]) * inv[a] : INFINITY;                                             \
+            // advance across the face of axis `ax`: the axis' quantities are selected, stepped once and put back -- one
+            // converged path for the lanes of a warp, whichever axis each of them steps along
+            {
+                const bool a0 = ax == 0, a1 = ax == 1;
+                const int st = a0 ? step[0] : (a1 ? step[1] : step[2]);
+                const int cn = (a0 ? c[0] : (a1 ? c[1] : c[2])) + st;
+                const int lf = (a0 ? left[0] : (a1 ? left[1] : left[2])) - 1;
+                if (lf < 0) return;                                        // left the hull's bounding box: miss
+                lin += a0 ? dlin[0] : (a1 ? dlin[1] : dlin[2]);
+                const double lo_a = a0 ? g.lo[0] : (a1 ? g.lo[1] : g.lo[2]), E_a = a0 ? E[0] : (a1 ? E[1] : E[2]);
+                const double T_a = a0 ? T[0] : (a1 ? T[1] : T[2]), inv_a = a0 ? inv[0] : (a1 ? inv[1] : inv[2]);
+                const double f = fma((double)(cn + (st > 0 ? 1 : 0)), g.h, lo_a);             // face_coord of the next face
+                const bool cand = st > 0 ? E_a > f : E_a < f;
+                const double sn = cand ? (f - T_a) * inv_a : INFINITY;
+                c[0] = a0 ? cn : c[0]; c[1] = a1 ? cn : c[1]; c[2] = (a0 | a1) ? c[2] : cn;
+                left[0] = a0 ? lf : left[0]; left[1] = a1 ? lf : left[1]; left[2] = (a0 | a1) ? left[2] : lf;
+                s_next[0] = a0 ? sn : s_next[0]; s_next[1] = a1 ? sn : s_next[1]; s_next[2] = (a0 | a1) ? s_next[2] : sn;
             }
-            if (ax == 0) PCT_HULL_ADVANCE(0)
-            else if (ax == 1) PCT_HULL_ADVANCE(1)
-            else PCT_HULL_ADVANCE(2)
-#undef PCT_HULL_ADVANCE
             crossed = ax;
         }
     }
@@ -200,7 +205,7 @@ k_hull_keys(const ProtonPtrs pr, int64_t i_base, int count, double t_lo, double 
 // A1 / R3-R5: tracker record -> hull entry/exit and the per-history part of the MLP.  Thread q takes history
 // p = order[q] (spatial order, k_hull_keys).  Also emits, in that order, the sort key K: the walk kernels run the batch in
 // order of K (longest first), so that concurrently running warps have the same trip count.
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, 8)
 k_hull(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const uint8_t* __restrict__ hull, int64_t i_base, int count,
        const uint32_t* __restrict__ order, HistRec* __restrict__ recs, uint32_t* __restrict__ keys, uint32_t* __restrict__ vals) {
     const int q = blockIdx.x * blockDim.x + threadIdx.x;
