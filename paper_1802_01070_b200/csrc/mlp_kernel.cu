@@ -25,7 +25,7 @@ struct Hit { bool ok, tie; int c[3]; double P[3]; };
 // grid faces and that box is skipped.  Decisions (which face comes first) are those of rule R9 applied to the chord of
 // the ray in the box; two faces closer than tie_eps along the ray set the tie flag.  Inside the loop s_next uses one
 // reciprocal per axis; P_0 is computed from the exact quotient of the face that was crossed last.
-__device__ __noinline__ void find_hull(const DevCfg& g, const uint8_t* __restrict__ hull, const double (&T)[3],
+__device__ __forceinline__ void find_hull(const DevCfg& g, const uint8_t* __restrict__ hull, const double (&T)[3],
                                        const double (&d)[3], Hit& hit) {
     hit.ok = false; hit.tie = false;
     const double d_len = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
@@ -205,7 +205,7 @@ k_hull_keys(const ProtonPtrs pr, int64_t i_base, int count, double t_lo, double 
 // A1 / R3-R5: tracker record -> hull entry/exit and the per-history part of the MLP.  Thread q takes history
 // p = order[q] (spatial order, k_hull_keys).  Also emits, in that order, the sort key K: the walk kernels run the batch in
 // order of K (longest first), so that concurrently running warps have the same trip count.
-__global__ void __launch_bounds__(128, 8)
+__global__ void __launch_bounds__(128, 5)
 k_hull(const __grid_constant__ DevCfg g, const ProtonPtrs pr, const uint8_t* __restrict__ hull, int64_t i_base, int count,
        const uint32_t* __restrict__ order, HistRec* __restrict__ recs, uint32_t* __restrict__ keys, uint32_t* __restrict__ vals) {
     const int q = blockIdx.x * blockDim.x + threadIdx.x;
