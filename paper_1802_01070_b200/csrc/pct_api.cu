@@ -535,7 +535,8 @@ int pct_solve_ex(pct_ctx* ctx, pct_paths* P, const float* b, const float* x0, in
     // count cache (R23): one buffer per context, owned by the plan that filled it last
     uint32_t* plan_counts = nullptr;
     if (plan) {
-        const size_t need = 4 * (size_t)plan->n_blocks * (size_t)ctx->n_vox;
+        // n_blocks x n_vox counts, then 8 ints per block: the bounding box of the voxels the block visits
+        const size_t need = 4 * (size_t)plan->n_blocks * (size_t)ctx->n_vox + 32 * (size_t)plan->n_blocks;
         if (need > ctx->counts_cap) {
             size_t free_b = 0, total_b = 0;
             if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && need <= (free_b + ctx->counts_cap) / 4 && need <= ((size_t)32 << 30)) {
@@ -568,14 +569,15 @@ int pct_solve_ex(pct_ctx* ctx, pct_paths* P, const float* b, const float* x0, in
                 // (and later calls with the same paths and block size) accumulate Delta only
                 uint32_t* counts = plan_counts ? plan_counts + (size_t)t * (size_t)ctx->n_vox : nullptr;
                 const bool cached = counts && plan->counts_ready[(size_t)t];
+                int* box6 = counts ? reinterpret_cast<int*>(plan_counts + (size_t)plan->n_blocks * (size_t)ctx->n_vox) + 8 * t : nullptr;
                 if ((rc = launch_block_windowed(ctx, P, plan, t, !cached, b, wts, x_out, ctx->ds, ctx->dsum, st)) != PCT_OK) return rc;
                 const int64_t nd = plan->direct_count[(size_t)t];
                 if (nd > 0 && (rc = launch_block_project_scatter(ctx, P, i0, i0 + nd, plan->direct_list, !cached, b, wts, x_out, ctx->ds, ctx->dsum, st)) != PCT_OK) return rc;
-                if ((rc = launch_block_update(ctx, x_out, ctx->ds, ctx->dsum, counts, !cached, lambda, clamp_lo, clamp_hi, st)) != PCT_OK) return rc;
+                if ((rc = launch_block_update(ctx, x_out, ctx->ds, ctx->dsum, counts, !cached, lambda, clamp_lo, clamp_hi, box6, st)) != PCT_OK) return rc;
                 if (counts) const_cast<SolvePlan*>(plan)->counts_ready[(size_t)t] = 1;
             } else {
                 if ((rc = launch_block_project_scatter(ctx, P, i0, i1, nullptr, true, b, wts, x_out, ctx->ds, ctx->dsum, st)) != PCT_OK) return rc;
-                if ((rc = launch_block_update(ctx, x_out, ctx->ds, ctx->dsum, nullptr, false, lambda, clamp_lo, clamp_hi, st)) != PCT_OK) return rc;
+                if ((rc = launch_block_update(ctx, x_out, ctx->ds, ctx->dsum, nullptr, false, lambda, clamp_lo, clamp_hi, nullptr, st)) != PCT_OK) return rc;
             }
         }
     }

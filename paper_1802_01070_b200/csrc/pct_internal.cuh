@@ -215,7 +215,7 @@ int launch_block_windowed(pct_ctx* ctx, const pct_paths* P, const SolvePlan* pla
 int build_solve_plan(pct_ctx* ctx, const pct_paths* P, int64_t block_size, cudaStream_t st, SolvePlan** out);
 void free_solve_plan(SolvePlan* plan);
 int launch_block_update(pct_ctx* ctx, float* x, float2* ds, float* dsum, uint32_t* counts, bool store, float lambda, float clamp_lo,
-                        float clamp_hi, cudaStream_t st);
+                        float clamp_hi, int* box6, cudaStream_t st);
 int launch_fill(pct_ctx* ctx, float* p, int64_t n, float value, cudaStream_t st);
 int launch_sweeps_persistent(pct_ctx* ctx, const pct_paths* P, const float* b, const float* wts, float* x, int iters, int64_t block_size, float lambda,
                         float clamp_lo, float clamp_hi, cudaStream_t st);
