@@ -168,30 +168,51 @@ __global__ void __launch_bounds__(256) k_block_update(float* __restrict__ x, flo
     }
 }
 
-// A7, first sweep over a block with a count cache: as k_block_update, and s_j^t is stored (all voxels: zeros too).  box6
-// (pre-set to {max.., -1..}) receives the bounding box {x0, y0, z0, x1, y1, z1} of the voxels the block visits: the later
-// sweeps over this block only look there (k_block_update_cached4_box).
+// A7, first sweep over a block with a count cache: as k_block_update, and s_j^t is stored (all voxels: zeros too).
 __global__ void __launch_bounds__(256) k_block_update_store(float* __restrict__ x, float2* __restrict__ ds, int64_t n, float lambda,
-                                                            uint32_t* __restrict__ counts, Clamp cl, int nx, int ny, int* __restrict__ box6) {
+                                                            uint32_t* __restrict__ counts, Clamp cl) {
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    int lo0 = INT_MAX, lo1 = INT_MAX, lo2 = INT_MAX, hi0 = -1, hi1 = -1, hi2 = -1;
     for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += stride) {
         const float2 a = ds[j];
         counts[j] = (uint32_t)a.y;
         if (a.y > 0.f) {
             x[j] = clamp_of(cl, x[j] + lambda * a.x / a.y);
             ds[j] = make_float2(0.f, 0.f);
-            const int r = (int)(j / nx), cx = (int)(j - (int64_t)r * nx), cz = r / ny, cy = r - cz * ny;
-            lo0 = min(lo0, cx); hi0 = max(hi0, cx); lo1 = min(lo1, cy); hi1 = max(hi1, cy); lo2 = min(lo2, cz); hi2 = max(hi2, cz);
         }
     }
-    if (box6) {
-        lo0 = __reduce_min_sync(0xffffffffu, lo0); lo1 = __reduce_min_sync(0xffffffffu, lo1); lo2 = __reduce_min_sync(0xffffffffu, lo2);
-        hi0 = __reduce_max_sync(0xffffffffu, hi0); hi1 = __reduce_max_sync(0xffffffffu, hi1); hi2 = __reduce_max_sync(0xffffffffu, hi2);
-        if ((threadIdx.x & 31) == 0 && hi0 >= 0) {
-            atomicMin(box6 + 0, lo0); atomicMin(box6 + 1, lo1); atomicMin(box6 + 2, lo2);
-            atomicMax(box6 + 3, hi0); atomicMax(box6 + 4, hi1); atomicMax(box6 + 5, hi2);
+}
+
+// Bounding box {x0, y0, z0, x1, y1, z1} of the voxels a block visits (counts > 0), into box6 (pre-set to {large.., -1..}): the
+// later sweeps over this block only look there (k_block_update_cached4_box).  One warp per grid row (y, z), lanes along x.
+__global__ void __launch_bounds__(256) k_counts_bbox(const uint4* __restrict__ counts4, int nx4, int ny, int nz, int* __restrict__ box6) {
+    const int lane = threadIdx.x & 31, rows = ny * nz;
+    int lo0 = INT_MAX, hi0 = -1, lo1 = INT_MAX, hi1 = -1, lo2 = INT_MAX, hi2 = -1;
+    for (int row = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); row < rows; row += gridDim.x * (blockDim.x >> 5)) {
+        const uint4* c = counts4 + (size_t)row * nx4;
+        int first = INT_MAX, last = -1;
+        for (int q = lane; q < nx4; q += 32) {                 // 16 bytes per lane: 128 voxels of the row per warp and turn
+            const uint4 v = __ldg(c + q);
+            const unsigned m = (v.x ? 1u : 0u) | (v.y ? 2u : 0u) | (v.z ? 4u : 0u) | (v.w ? 8u : 0u);
+            if (m) { first = min(first, 4 * q + __ffs(m) - 1); last = max(last, 4 * q + 31 - __clz(m)); }
         }
+        first = __reduce_min_sync(0xffffffffu, first);
+        last = __reduce_max_sync(0xffffffffu, last);
+        if (last >= 0) {
+            const int z = row / ny, y = row - z * ny;
+            lo0 = min(lo0, first); hi0 = max(hi0, last); lo1 = min(lo1, y); hi1 = max(hi1, y); lo2 = min(lo2, z); hi2 = max(hi2, z);
+        }
+    }
+    // one set of atomics per CTA (same-address atomics serialise in L2); the plain read filters out those that cannot change anything
+    __shared__ int sh[6][8];
+    if (lane == 0) { const int w = threadIdx.x >> 5; sh[0][w] = lo0; sh[1][w] = lo1; sh[2][w] = lo2; sh[3][w] = hi0; sh[4][w] = hi1; sh[5][w] = hi2; }
+    __syncthreads();
+    if (threadIdx.x < 6) {
+        const int k = threadIdx.x;
+        int v = sh[k][0];
+        for (int w = 1; w < 8; ++w) v = k < 3 ? min(v, sh[k][w]) : max(v, sh[k][w]);
+        volatile int* vb = box6;
+        if (k < 3) { if (v < vb[k]) atomicMin(box6 + k, v); }
+        else if (v > vb[k]) atomicMax(box6 + k, v);
     }
 }
 
@@ -314,11 +335,17 @@ int launch_block_update(pct_ctx* ctx, float* x, float2* ds, float* dsum, uint32_
     ProfScope prof(ctx, 2, st);
     if (!counts) k_block_update<<<grid, 256, 0, st>>>(x, ds, n, lambda, cl);
     else if (store) {
-        if (box6) {
+        k_block_update_store<<<grid, 256, 0, st>>>(x, ds, n, lambda, counts, cl);
+        if (box6 && n < 0x7fffffffLL) {
             PCT_CUDA(ctx, cudaMemsetAsync(box6, 0x7f, 3 * sizeof(int), st));          // mins: a large int
             PCT_CUDA(ctx, cudaMemsetAsync(box6 + 3, 0xff, 3 * sizeof(int), st));      // maxes: -1
+            if (ctx->geom.nx % 4 == 0 && ((uintptr_t)counts & 15) == 0) {         // the box kernel's own conditions
+                const int rows = ctx->geom.ny * ctx->geom.nz;
+                k_counts_bbox<<<(unsigned)min((rows + 7) / 8, ctx->num_sms * 4), 256, 0, st>>>(reinterpret_cast<const uint4*>(counts), ctx->geom.nx / 4, ctx->geom.ny,
+                                                                         ctx->geom.nz, box6);
+                ++ctx->launches;
+            }
         }
-        k_block_update_store<<<grid, 256, 0, st>>>(x, ds, n, lambda, counts, cl, ctx->geom.nx, ctx->geom.ny, box6);
     } else if (box6 && ctx->geom.nx % 4 == 0 && n < 0x7fffffffLL && (((uintptr_t)x | (uintptr_t)dsum | (uintptr_t)counts) & 15) == 0)
         k_block_update_cached4_box<<<grid, 256, 0, st>>>(reinterpret_cast<float4*>(x), reinterpret_cast<float4*>(dsum), ctx->geom.nx / 4, ctx->geom.ny,
                                                          lambda, reinterpret_cast<const uint4*>(counts), cl, box6);
