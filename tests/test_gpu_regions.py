@@ -156,3 +156,28 @@ def test_regions_through_the_plan_path_reproduce_the_plain_solve(binding):
     x_2 = x_2.cpu().numpy()
     far = np.r_[0:(cfg.nz // 2 - 16) * sl, (cfg.nz // 2 + 16) * sl:cfg.nz * sl]
     assert np.abs(x_2[far] - x_joint[far]).max() <= MAX_ABS_TOL and np.abs(x_2 - 1.0).max() > 0.05
+
+
+def test_one_process_runs_all_regions_through_the_distributed_entry(binding):
+    """paper_1802_01070_b200.regions with a process group of one rank: that rank owns every region, the result is
+    pct_reconstruct_regions' (the multi-rank slice assembly itself is covered on gloo in tests/test_oracle_regions.py)."""
+    import socket
+    import torch.distributed as dist
+    from paper_1802_01070_b200 import regions
+    cfg = synth.scaled(synth.CONFIGS["tiny"], 4000)
+    x_true, hull, shadow = synth.make_phantom(cfg, "cuda")
+    pr = synth.generate_protons(cfg, x_true, shadow, device="cuda")
+    ctx = binding.Context(synth.geometry(cfg), synth.mlp_params(cfg), 0)
+    dev = {k: pr[k].cuda().contiguous() for k in binding.PROTON_KEYS}
+    b = pr["wepl"].cuda().contiguous()
+    u = cfg.u_tracker
+    hull_d = hull.reshape(-1).cuda().contiguous()
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=0, world_size=1)
+    try:
+        x_d, mem_d = regions.reconstruct_regions_distributed(ctx, dev, -u, u, hull_d, b, None, 1, 2, cfg.block, cfg.lam, n_regions=2)
+    finally:
+        dist.destroy_process_group()
+    x_r, mem_r = ctx.reconstruct_regions(dev, -u, u, hull_d, b, None, 2, 1, 2, cfg.block, cfg.lam)
+    assert mem_d == mem_r and all(v > 0 for v in mem_r)
+    assert np.abs(x_d.cpu().numpy() - x_r.cpu().numpy()).max() <= MAX_ABS_TOL
